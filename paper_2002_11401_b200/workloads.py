@@ -1,0 +1,213 @@
+"""Seeded synthetic input generators (geometries, coercive fields, spins, field protocols).
+
+This module serves BOTH the CPU oracle (tests, ``bench.py --impl reference``) and the CUDA path.
+It holds none of the method's arithmetic: no dipolar field, no astroid, no relaxation, no thermal
+draw.  It only produces the *inputs* the paper's model takes ("each magnetic dipole is
+modelled with a position r_i and rotation theta_i ... each magnet is assigned a coercive field"),
+in the shapes of BASELINE.json's five configs.  numpy only.
+
+Recipes:
+
+* geometries, PAPER.md:140-148 (section II.I, Fig. 3): square closed/open, kagome, pinwheel diamond,
+  ising, plus "rotated square" (BASELINE.json config 3).
+* coercive-field disorder, PAPER.md:118 (section II.G): h_k^(i) ~ N(h_k, (k_disorder h_k)^2), kept
+  positive by redrawing.
+* field protocols, PAPER.md:63 / :124: a discrete series of global fields, relaxed at each value.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+SQRT3 = math.sqrt(3.0)
+
+
+# --------------------------------------------------------------------------- geometries
+def square_closed(n: int):
+    """Square ASI, closed edges, n x n cells -> N = 2 n (n+1)   (Fig. 3a).
+
+    Horizontals (i+1/2, j), i<n, j<=n, theta=0, index j*n+i; then verticals (i, j+1/2), i<=n, j<n,
+    theta=pi/2, index Nh + j*(n+1)+i.  Lattice spacing 1.
+    """
+    j, i = np.meshgrid(np.arange(n + 1), np.arange(n), indexing="ij")
+    hpos = np.stack([i.ravel() + 0.5, j.ravel().astype(np.float64)], axis=1)
+    j, i = np.meshgrid(np.arange(n), np.arange(n + 1), indexing="ij")
+    vpos = np.stack([i.ravel().astype(np.float64), j.ravel() + 0.5], axis=1)
+    pos = np.concatenate([hpos, vpos]).astype(np.float64)
+    angle = np.concatenate([np.zeros(len(hpos)), np.full(len(vpos), math.pi / 2)])
+    return np.ascontiguousarray(pos), np.ascontiguousarray(angle)
+
+
+def square_open(n: int):
+    """Square ASI, open edges: n x n vertices, magnets on the edges between them -> N = 2 n (n-1)
+    (Fig. 3b; the geometry of the paper's Fig. 9 throughput test)."""
+    j, i = np.meshgrid(np.arange(n), np.arange(n - 1), indexing="ij")
+    hpos = np.stack([i.ravel() + 0.5, j.ravel().astype(np.float64)], axis=1)
+    j, i = np.meshgrid(np.arange(n - 1), np.arange(n), indexing="ij")
+    vpos = np.stack([i.ravel().astype(np.float64), j.ravel() + 0.5], axis=1)
+    pos = np.concatenate([hpos, vpos]).astype(np.float64)
+    angle = np.concatenate([np.zeros(len(hpos)), np.full(len(vpos), math.pi / 2)])
+    return np.ascontiguousarray(pos), np.ascontiguousarray(angle)
+
+
+def rotated_square(n: int, rot: float = math.pi / 4):
+    """BASELINE.json config 3: closed-square positions, every magnet rotated `rot` about its centre."""
+    pos, angle = square_closed(n)
+    return pos, angle + rot
+
+
+def pinwheel_diamond(n: int, rot: float = math.pi / 4):
+    """Pinwheel "diamond" with 2 n^2 magnets (PAPER.md:286: 25x25 -> 1250; :288: 708x708 -> >1e6).
+
+    One horizontal (i+1/2, j) and one vertical (i, j+1/2) magnet per cell i,j<n, each rotated `rot`.
+    """
+    j, i = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")
+    hpos = np.stack([i.ravel() + 0.5, j.ravel().astype(np.float64)], axis=1)
+    vpos = np.stack([i.ravel().astype(np.float64), j.ravel() + 0.5], axis=1)
+    pos = np.concatenate([hpos, vpos]).astype(np.float64)
+    angle = np.concatenate([np.zeros(len(hpos)), np.full(len(vpos), math.pi / 2)]) + rot
+    return np.ascontiguousarray(pos), np.ascontiguousarray(angle)
+
+
+def ising(nx: int, ny: int):
+    """Ising geometry (Fig. 3f): nx x ny collinear magnets on a unit square grid, theta=0."""
+    j, i = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    pos = np.stack([i.ravel().astype(np.float64), j.ravel().astype(np.float64)], axis=1)
+    return np.ascontiguousarray(pos), np.zeros(nx * ny)
+
+
+def kagome(n: int):
+    """Kagome ASI: honeycomb of n x n flat-top hexagons, edge length 1, one magnet per unique edge at
+    its midpoint along the edge direction (0, 60, 120 degrees)  -> N = 3 n^2 + 4 n - 1
+    (29 x 29 hexagons = 2638 magnets; Fig. 3c).
+
+    Hexagon centres (1.5 c, sqrt3 r + (sqrt3/2 if c odd)), c,r in [0,n).  Index order = first
+    occurrence iterating c (outer), r (inner), then the six edges counter-clockwise from the edge
+    whose midpoint lies at 30 degrees.  Midpoints are stored on the exact lattice
+    (x = q/4, y = p*sqrt3/4 with integers q,p) so equal edges coincide bit-exactly.
+    """
+    seen = {}
+    qs, ps, ths = [], [], []
+    # edge midpoints of a unit flat-top hexagon in units (1/4, sqrt3/4): angle 30+60k at radius sqrt3/2
+    mids = [(3, 1), (0, 2), (-3, 1), (-3, -1), (0, -2), (3, -1)]
+    dirs = [2, 0, 1, 2, 0, 1]  # edge direction = multiples of 60 degrees: 120, 0, 60, 120, 0, 60
+    for c in range(n):
+        for r in range(n):
+            cq = 6 * c                      # 1.5 c  in units of 1/4
+            cp = 4 * r + (2 if c % 2 else 0)  # sqrt3 r + sqrt3/2 in units of sqrt3/4
+            for (dq, dp), d in zip(mids, dirs):
+                key = (cq + dq, cp + dp)
+                if key in seen:
+                    continue
+                seen[key] = len(qs)
+                qs.append(key[0]); ps.append(key[1]); ths.append(d)
+    pos = np.stack([np.array(qs) * 0.25, np.array(ps) * (SQRT3 / 4.0)], axis=1).astype(np.float64)
+    angle = np.array(ths, dtype=np.float64) * (math.pi / 3.0)
+    return np.ascontiguousarray(pos), np.ascontiguousarray(angle)
+
+
+# --------------------------------------------------------------------------- per-magnet inputs
+def coercive_fields(N: int, hk: float = 0.2, k_disorder: float = 0.05, seed: int = 0, replicas: int = 0):
+    """h_k^(i) ~ N(h_k, (k_disorder h_k)^2), redrawn until positive.
+
+    Uses numpy's counter-based Philox bit generator keyed by `seed` (an input recipe, not the
+    method's thermal stream).  `replicas` > 0 returns [replicas, N] with seeds seed, seed+1, ...
+    """
+    def one(sd):
+        rng = np.random.Generator(np.random.Philox(key=sd))
+        hc = hk * (1.0 + k_disorder * rng.standard_normal(N))
+        bad = hc <= 0
+        while bad.any():
+            hc[bad] = hk * (1.0 + k_disorder * rng.standard_normal(int(bad.sum())))
+            bad = hc <= 0
+        return hc
+    if replicas > 0:
+        return np.ascontiguousarray(np.stack([one(seed + r) for r in range(replicas)]))
+    return np.ascontiguousarray(one(seed))
+
+
+def random_spins(N: int, seed: int = 1):
+    rng = np.random.Generator(np.random.Philox(key=seed))
+    return (2 * rng.integers(0, 2, size=N, dtype=np.int8) - 1).astype(np.int8)
+
+
+# --------------------------------------------------------------------------- field protocols
+def ramp(A: float, B: float, K: int, phi_deg: float, legs: int = 1):
+    """K+1 global field vectors t=0..K at angle phi (reading C-13).
+
+    one leg : H_t = A + (B-A) t/K;   two legs: H_t = A + (B-A) (1 - |1 - 2t/K|)   (A -> B -> A).
+    Returns [K+1, 2] (hx, hy).
+    """
+    t = np.arange(K + 1, dtype=np.float64)
+    if legs == 1:
+        H = A + (B - A) * t / K
+    else:
+        H = A + (B - A) * (1.0 - np.abs(1.0 - 2.0 * t / K))
+    phi = math.radians(phi_deg)
+    return np.ascontiguousarray(np.stack([H * math.cos(phi), H * math.sin(phi)], axis=1))
+
+
+# --------------------------------------------------------------------------- the five configs
+@dataclass
+class Workload:
+    name: str
+    pos: np.ndarray
+    angle: np.ndarray
+    hc: np.ndarray
+    spins: np.ndarray
+    params: dict           # alpha, b, c, beta, gamma, neighbor_distance
+    fields: np.ndarray     # [T, 2] global field per step (step key = row index)
+    sigma_th: float = 0.0
+    thermal_seed: int = 0
+    note: str = ""
+    extra: dict = field(default_factory=dict)
+
+    @property
+    def N(self):
+        return int(self.pos.shape[0])
+
+
+def _params(alpha, b, c, beta, gamma, nd):
+    return dict(alpha=float(alpha), b=float(b), c=float(c), beta=float(beta), gamma=float(gamma),
+                neighbor_distance=float(nd))
+
+
+def config(which, scale: int | None = None) -> Workload:
+    """BASELINE.json configs 1..5 (and '2b').  `scale` overrides the lattice size n (parity tests
+    at reduced size use the same recipe)."""
+    which = str(which)
+    if which == "1":
+        n = scale or 10
+        pos, ang = square_closed(n)
+        return Workload(f"cfg1_square_closed_{n}x{n}", pos, ang, coercive_fields(len(ang)),
+                        np.ones(len(ang), np.int8), _params(0.001, 1, 1, 3, 3, 1.0),
+                        ramp(0.2, -0.2, 500, 45.0, legs=2))
+    if which in ("2", "2b"):
+        n = scale or (50 if which == "2" else 70)
+        pos, ang = kagome(n)
+        return Workload(f"cfg{which}_kagome_{n}x{n}", pos, ang, coercive_fields(len(ang)),
+                        np.ones(len(ang), np.int8), _params(0.001, 1, 1, 3, 3, SQRT3),
+                        ramp(-0.15, 0.15, 1000, 5.0, legs=2))
+    if which == "3":
+        n = scale or 200
+        pos, ang = rotated_square(n)
+        return Workload(f"cfg3_rotated_square_{n}x{n}", pos, ang, coercive_fields(len(ang)),
+                        np.ones(len(ang), np.int8), _params(0.0013, 0.38, 1, 1.7, 3, 3.0),
+                        ramp(0.12, -0.12, 2000, -40.0, legs=2))
+    if which == "4":
+        n = scale or 1000
+        pos, ang = square_closed(n)
+        return Workload(f"cfg4_square_closed_{n}x{n}_thermal", pos, ang, coercive_fields(len(ang)),
+                        np.ones(len(ang), np.int8), _params(0.001, 1, 1, 3, 3, 1.0),
+                        ramp(0.2, -0.2, 200, 45.0, legs=1), sigma_th=0.01, thermal_seed=0)
+    if which == "5":
+        n = scale or 500
+        pos, ang = square_closed(n)
+        phi = math.radians(45.0)
+        return Workload(f"cfg5_square_closed_{n}x{n}_nd10", pos, ang, coercive_fields(len(ang)),
+                        random_spins(len(ang), seed=1), _params(0.001, 1, 1, 3, 3, 10.0),
+                        np.array([[0.10 * math.cos(phi), 0.10 * math.sin(phi)]]),
+                        note="field + scan only, spins not flipped")
+    raise ValueError(f"unknown config {which!r}")
