@@ -1,0 +1,160 @@
+/* flatspin.h -- C ABI of the B200-native flatspin hot path (libflatspin_b200.so).
+ *
+ * What it computes is defined by /root/reference/PAPER.md (arxiv 2002.11401, "flatspin: A Large-Scale
+ * Artificial Spin Ice Simulator"); citations below are PAPER.md lines.  SURVEY.md section 8(b) lists
+ * the entry points.  No torch types cross this boundary: plain pointers (each marked DEVICE or HOST)
+ * and sizes.  All kernels are hand-written CUDA for sm_100a (paper_2002_11401_b200/csrc/flatspin.cu).
+ *
+ * Model (Eq. 1): N binary macro spins s_i in {-1,+1} at positions r_i with rotation
+ * theta_i and coercive field h_c^(i) (== h_k^(i) of Eq. 5, reading C-4).
+ *
+ * Conventions
+ *   - Every DEVICE pointer is caller-owned CUDA global memory (a torch tensor's data_ptr()).  Inputs
+ *     of fs_create* are consumed during the call and may be freed afterwards.  The workspace is
+ *     caller-owned and must outlive the handle.  Outputs are written to caller-owned buffers.
+ *   - HOST pointers to scalars (n_flips_out ...) are written after a stream synchronise; passing NULL
+ *     skips the synchronise (the call is then fully asynchronous on `stream`).
+ *   - All work is enqueued on the stream given at creation (a cudaStream_t passed as void*; NULL =
+ *     the legacy default stream).
+ *   - Fields are (parallel, perpendicular) pairs in the FIXED geometric frame of theta_i:
+ *       par = h . (cos theta_i, sin theta_i),  perp = h . (-sin theta_i, cos theta_i)
+ *     (Fig. 2; reading C-2).  Eq. 6 then reads s_i * par < 0.
+ *   - Ensembles: R independent replicas share the geometry and differ in h_c, spins
+ *     and thermal seed (seed + r).  Arrays carry a leading [R] dimension.  R == 1 for fs_create.
+ *   - Return value: FS_OK (0) or a negative FS_ERR_* code; fs_last_error() gives a message for the
+ *     calling thread.  No exception crosses the ABI.  There is NO CPU fallback: without a CUDA
+ *     device every compute entry point returns FS_ERR_CUDA.
+ */
+#ifndef FLATSPIN_B200_H
+#define FLATSPIN_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fs_sim fs_sim; /* opaque; owned by the library; freed by fs_destroy */
+
+/* alpha: dipolar coupling strength (Eq. 3).  b, c, beta, gamma: generalized
+ * Stoner-Wohlfarth astroid (Eq. 5).  neighbor_distance: neighbourhood radius in
+ * lattice units; j is a neighbour of i iff j != i and |r_i-r_j|^2 <= nd^2 (1+1e-9)
+ * (reading A-7). */
+typedef struct {
+    double alpha, b, c, beta, gamma, neighbor_distance;
+} fs_params;
+
+enum {
+    FS_OK = 0,
+    FS_ERR_ARG = -1,        /* null pointer, N<=0, R<=0, hc<=0 or non-finite, b,c,beta,gamma,nd <= 0, K too large */
+    FS_ERR_COINCIDENT = -2, /* two distinct spins at the same position (Eq. 3 singular; reading C-8) */
+    FS_ERR_WORKSPACE = -3,  /* workspace too small or misaligned (needs 256-byte alignment) */
+    FS_ERR_CUDA = -4,       /* CUDA runtime error, or no device */
+    FS_ERR_MAXFLIPS = -5    /* fs_relax stopped at max_flips with switchable spins left; state valid */
+};
+
+/* Which field fs_get_fields returns (Eq. 2): h_i = h_dip + h_ext + h_th. */
+enum { FS_FIELD_TOTAL = 0, FS_FIELD_DIP = 1, FS_FIELD_EXT = 2, FS_FIELD_THERMAL = 3 };
+
+/* Gather kernel variants for fs_update_fields:
+ *   0 = auto, 1 = ELL with fp64 weight pairs streamed from HBM (20 B / interaction),
+ *   2 = ELL with 16-bit ids into a shared-memory table of unique weight pairs, the per-sublattice
+ *       stencil table (6 B / interaction); falls back to 1 if the geometry has > 65535 unique pairs. */
+enum { FS_GATHER_AUTO = 0, FS_GATHER_ELL_F64 = 1, FS_GATHER_ELL_DICT = 2 };
+
+/* Bytes of workspace fs_create[_ensemble] needs for this geometry (runs the cell-grid neighbour count,
+ * PAPER.md:57, to find the maximum degree K).  pos_dev: DEVICE [N,2] row-major fp64.
+ * bytes_out: HOST.  Synchronises `stream`. */
+int fs_workspace_bytes(int64_t N, int32_t R, const double* pos_dev, const fs_params* p,
+                       size_t* bytes_out, void* stream);
+
+/* Build a simulation: frame tables (Eq. 1), cell-grid neighbour lists, couplings
+ * alpha*g_ij (Eq. 3) in row-major ELL.  Spins start at +1 (fs_set_spins to change).
+ * pos_dev DEVICE [N,2]; angle_dev DEVICE [N] radians; hc_dev DEVICE [N] (fs_create) or [R,N]
+ * (fs_create_ensemble), all > 0.  workspace_dev: DEVICE, 256-byte aligned, >= fs_workspace_bytes.
+ * Synchronises `stream` once (to read K and the validation flags). */
+int fs_create(fs_sim** out, int64_t N, const double* pos_dev, const double* angle_dev,
+              const double* hc_dev, const fs_params* p, void* workspace_dev, size_t workspace_bytes,
+              void* stream);
+int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev,
+                       const double* angle_dev, const double* hc_dev, const fs_params* p,
+                       void* workspace_dev, size_t workspace_bytes, void* stream);
+int fs_destroy(fs_sim* sim);
+
+/* Geometry queries (HOST outputs, no synchronise). */
+int fs_get_info(const fs_sim* sim, int64_t* N, int32_t* R, int32_t* K /*max degree*/,
+                int64_t* n_interactions /*sum of degrees*/);
+
+/* s_dev: DEVICE [R,N] int8, values +1/-1.  Marks h_dip stale (recomputed lazily by the next call
+ * that needs it, or explicitly by fs_update_fields). */
+int fs_set_spins(fs_sim* sim, const int8_t* s_dev);
+int fs_get_spins(fs_sim* sim, int8_t* s_dev_out /*DEVICE [R,N]*/);
+
+/* Thermal field: per spin and step two components sigma_th * N(0,1) in global x,y from
+ * Philox4x32-10 keyed (seed + replica; step; spin) + Box-Muller (reading C-11), constant
+ * during a relaxation.  sigma_th = 0 switches it off (default). */
+int fs_set_thermal(fs_sim* sim, double sigma_th, uint64_t seed);
+
+/* Global external field for all replicas, and the step key of the thermal stream. */
+int fs_set_field(fs_sim* sim, double hx, double hy, uint32_t step);
+/* Per-replica global fields: h_host HOST [R,2] (hx,hy). */
+int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step);
+
+/* Choose the gather kernel variant (FS_GATHER_*).  Default auto. */
+int fs_set_gather_variant(fs_sim* sim, int variant);
+
+/* Full dipolar-field gather h_dip,i = sum_k s[nbr[i][k]] * w[i][k] for every spin (Eq. 3 over the
+ * neighbourhood).  Asynchronous. */
+int fs_update_fields(fs_sim* sim);
+
+/* Fused total field + astroid + switching margin + arg-max (Eqs. 2, 5, 6), replica 0
+ * of an ensemble unless *_ensemble.  Outputs HOST: number of switchable spins, the index of the
+ * spin furthest outside its astroid (lowest index among exact ties; -1 if none) and its Eq. 5
+ * left-hand side.  Synchronises. */
+int fs_scan(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, double* best_L);
+int fs_scan_ensemble(fs_sim* sim, int64_t* n_switchable /*HOST [R]*/, int64_t* best_index /*HOST [R]*/,
+                     double* best_L /*HOST [R]*/);
+
+/* Relaxation: repeat { flip the switchable spin with the greatest Eq. 5 left-hand
+ * side; update its neighbours' h_dip incrementally } until no spin is switchable, entirely on the
+ * device.  max_flips <= 0: unlimited.  n_flips_out HOST (sum over replicas for an ensemble; NULL =
+ * asynchronous, read later with fs_get_counters).  Returns FS_ERR_MAXFLIPS if the cap stopped it
+ * (only detected when n_flips_out != NULL). */
+int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out);
+int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out /*HOST [R]*/);
+
+/* Counters accumulated on the device since creation / the last reset: HOST [R] each (any may be
+ * NULL).  Synchronises. */
+int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset);
+
+/* h_dev_out DEVICE [R,N,2] (par, perp) in the fixed theta_i frame; `which` = FS_FIELD_*. */
+int fs_get_fields(fs_sim* sim, int which, double* h_dev_out);
+
+/* Flip log of the last fs_relax of replica `replica`: idx_dev_out DEVICE [cap] int32 in flip order;
+ * n_out HOST = number of flips of that relax (may exceed what was logged: the internal log holds
+ * 4N+1024 entries).  Synchronises. */
+int fs_get_flip_log(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out);
+
+/* Neighbour table: idx_dev_out DEVICE [N,K] row-major int32, ascending, -1 padded; K_out HOST. */
+int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out);
+
+/* Host-buffer convenience for end-to-end timing: H2D spins [R,N] -> gather -> scan -> D2H total fields
+ * [R,N,2], all on the simulation's stream, then synchronise.  s_host / h_host_out HOST (pinned for
+ * full speed).  Scan outputs as fs_scan (replica 0). */
+int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t* n_switchable,
+                 int64_t* best_index, double* best_L);
+
+/* Host-buffer relaxation step: set the field, relax, D2H spins [R,N].  n_flips_out HOST (sum). */
+int fs_relax_host(fs_sim* sim, double hx, double hy, uint32_t step, int8_t* s_host_out,
+                  int64_t* n_flips_out);
+
+/* Number of kernels this library launched since load (all sims), for the benchmark's launch count. */
+int64_t fs_kernel_launches(void);
+
+const char* fs_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLATSPIN_B200_H */

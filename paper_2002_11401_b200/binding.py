@@ -1,0 +1,241 @@
+"""Thin ctypes binding of include/flatspin.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/flatspin.cu.  torch is used for device
+memory (tensors own the buffers whose pointers cross the C ABI) and for the stream.  There is no CPU
+fallback: if the shared library is missing or no CUDA device is present, construction raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+FS_OK, FS_ERR_ARG, FS_ERR_COINCIDENT, FS_ERR_WORKSPACE, FS_ERR_CUDA, FS_ERR_MAXFLIPS = 0, -1, -2, -3, -4, -5
+FIELD_TOTAL, FIELD_DIP, FIELD_EXT, FIELD_THERMAL = 0, 1, 2, 3
+GATHER_AUTO, GATHER_ELL_F64, GATHER_ELL_DICT = 0, 1, 2
+
+EXPORTS = [
+    "fs_workspace_bytes", "fs_create", "fs_create_ensemble", "fs_destroy", "fs_get_info", "fs_set_spins",
+    "fs_get_spins", "fs_set_thermal", "fs_set_field", "fs_set_field_ensemble", "fs_set_gather_variant",
+    "fs_update_fields", "fs_scan", "fs_scan_ensemble", "fs_relax", "fs_relax_ensemble", "fs_get_counters",
+    "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
+    "fs_kernel_launches", "fs_last_error",
+]
+
+
+class FsParams(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("alpha", "b", "c", "beta", "gamma", "neighbor_distance")]
+
+
+class FlatspinError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"flatspin error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: str | None = None):
+    """dlopen libflatspin_b200.so and declare the prototypes.  Fails loudly if it is missing."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or _build.LIB
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not built: run `python -c 'import __graft_entry__ as g; g.build()'`")
+    L = C.CDLL(path)
+    vp, i64, i32, dbl, P = C.c_void_p, C.c_int64, C.c_int32, C.c_double, C.POINTER
+    sig = {
+        "fs_workspace_bytes": [i64, i32, vp, P(FsParams), P(C.c_size_t), vp],
+        "fs_create": [P(vp), i64, vp, vp, vp, P(FsParams), vp, C.c_size_t, vp],
+        "fs_create_ensemble": [P(vp), i64, i32, vp, vp, vp, P(FsParams), vp, C.c_size_t, vp],
+        "fs_destroy": [vp],
+        "fs_get_info": [vp, P(i64), P(i32), P(i32), P(i64)],
+        "fs_set_spins": [vp, vp], "fs_get_spins": [vp, vp],
+        "fs_set_thermal": [vp, dbl, C.c_uint64],
+        "fs_set_field": [vp, dbl, dbl, C.c_uint32],
+        "fs_set_field_ensemble": [vp, vp, C.c_uint32],
+        "fs_set_gather_variant": [vp, i32],
+        "fs_update_fields": [vp],
+        "fs_scan": [vp, P(i64), P(i64), P(dbl)],
+        "fs_scan_ensemble": [vp, vp, vp, vp],
+        "fs_relax": [vp, i64, P(i64)],
+        "fs_relax_ensemble": [vp, i64, vp],
+        "fs_get_counters": [vp, vp, vp, i32],
+        "fs_get_fields": [vp, i32, vp],
+        "fs_get_flip_log": [vp, i32, vp, i64, P(i64)],
+        "fs_get_neighbors": [vp, vp, P(i32)],
+        "fs_step_host": [vp, vp, vp, P(i64), P(i64), P(dbl)],
+        "fs_relax_host": [vp, dbl, dbl, C.c_uint32, vp, P(i64)],
+        "fs_kernel_launches": [],
+        "fs_last_error": [],
+    }
+    for name, args in sig.items():
+        fn = getattr(L, name)
+        fn.argtypes = args
+        fn.restype = C.c_int
+    L.fs_kernel_launches.restype = C.c_int64
+    L.fs_last_error.restype = C.c_char_p
+    if path == _build.LIB:
+        _lib = L
+    return L
+
+
+def _check(L, rc, allow=()):
+    if rc != FS_OK and rc not in allow:
+        raise FlatspinError(rc, L.fs_last_error().decode())
+    return rc
+
+
+def kernel_launches() -> int:
+    return int(load_library().fs_kernel_launches())
+
+
+class Sim:
+    """One simulation handle (R >= 1 replicas).  Mirrors the fs_* entry points one to one."""
+
+    def __init__(self, pos, angle, hc, params: dict, device="cuda:0", stream: torch.cuda.Stream | None = None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("flatspin_b200 needs a CUDA device; there is no CPU fallback")
+        self.L = load_library()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._sp = C.c_void_p(self.stream.cuda_stream)
+        f64 = dict(dtype=torch.float64, device=self.device)
+        with torch.cuda.stream(self.stream):
+            pos_d = torch.as_tensor(np.ascontiguousarray(pos, np.float64)).to(**f64).contiguous()
+            ang_d = torch.as_tensor(np.ascontiguousarray(angle, np.float64)).to(**f64).contiguous()
+            hc_np = np.ascontiguousarray(hc, np.float64)
+            hc_d = torch.as_tensor(hc_np).to(**f64).contiguous()
+        self.N = int(ang_d.shape[0])
+        self.R = 1 if hc_np.ndim == 1 else int(hc_np.shape[0])
+        assert pos_d.shape == (self.N, 2) and hc_d.numel() == self.R * self.N
+        self.params = FsParams(*[float(params[k]) for k in ("alpha", "b", "c", "beta", "gamma", "neighbor_distance")])
+        nbytes = C.c_size_t(0)
+        _check(self.L, self.L.fs_workspace_bytes(self.N, self.R, pos_d.data_ptr(), C.byref(self.params),
+                                                 C.byref(nbytes), self._sp))
+        self.workspace_bytes = int(nbytes.value)
+        self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        self._ws_ptr = (base + 255) // 256 * 256
+        h = C.c_void_p()
+        _check(self.L, self.L.fs_create_ensemble(C.byref(h), self.N, self.R, pos_d.data_ptr(), ang_d.data_ptr(),
+                                                 hc_d.data_ptr(), C.byref(self.params), self._ws_ptr,
+                                                 self.workspace_bytes, self._sp))
+        self.h = h
+        n, r, k, i = C.c_int64(), C.c_int32(), C.c_int32(), C.c_int64()
+        _check(self.L, self.L.fs_get_info(self.h, C.byref(n), C.byref(r), C.byref(k), C.byref(i)))
+        self.K, self.n_interactions = int(k.value), int(i.value)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.fs_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- state
+    def set_spins(self, s):
+        t = s if isinstance(s, torch.Tensor) else torch.as_tensor(np.ascontiguousarray(s, np.int8))
+        t = t.to(device=self.device, dtype=torch.int8).contiguous()
+        assert t.numel() == self.R * self.N
+        _check(self.L, self.L.fs_set_spins(self.h, t.data_ptr()))
+        self.stream.synchronize()   # `t` may be a temporary
+
+    def get_spins(self) -> torch.Tensor:
+        out = torch.empty((self.R, self.N) if self.R > 1 else (self.N,), dtype=torch.int8, device=self.device)
+        _check(self.L, self.L.fs_get_spins(self.h, out.data_ptr()))
+        return out
+
+    def set_thermal(self, sigma_th, seed):
+        _check(self.L, self.L.fs_set_thermal(self.h, float(sigma_th), int(seed)))
+
+    def set_field(self, hx, hy, step=0):
+        _check(self.L, self.L.fs_set_field(self.h, float(hx), float(hy), int(step)))
+
+    def set_field_ensemble(self, h, step=0):
+        h = np.ascontiguousarray(h, np.float64); assert h.shape == (self.R, 2)
+        _check(self.L, self.L.fs_set_field_ensemble(self.h, h.ctypes.data, int(step)))
+
+    def set_gather_variant(self, v):
+        _check(self.L, self.L.fs_set_gather_variant(self.h, int(v)))
+
+    # ---- compute
+    def update_fields(self):
+        _check(self.L, self.L.fs_update_fields(self.h))
+
+    def scan(self):
+        n, b, l = C.c_int64(), C.c_int64(), C.c_double()
+        _check(self.L, self.L.fs_scan(self.h, C.byref(n), C.byref(b), C.byref(l)))
+        return int(n.value), int(b.value), float(l.value)
+
+    def scan_async(self):
+        _check(self.L, self.L.fs_scan(self.h, None, None, None))
+
+    def scan_ensemble(self):
+        n = np.zeros(self.R, np.int64); b = np.zeros(self.R, np.int64); l = np.zeros(self.R, np.float64)
+        _check(self.L, self.L.fs_scan_ensemble(self.h, n.ctypes.data, b.ctypes.data, l.ctypes.data))
+        return n, b, l
+
+    def relax(self, max_flips=0, sync=True):
+        if not sync:
+            _check(self.L, self.L.fs_relax(self.h, int(max_flips), None))
+            return None
+        n = C.c_int64()
+        _check(self.L, self.L.fs_relax(self.h, int(max_flips), C.byref(n)), allow=(FS_ERR_MAXFLIPS,))
+        return int(n.value)
+
+    def relax_ensemble(self, max_flips=0):
+        n = np.zeros(self.R, np.int64)
+        _check(self.L, self.L.fs_relax_ensemble(self.h, int(max_flips), n.ctypes.data), allow=(FS_ERR_MAXFLIPS,))
+        return n
+
+    def counters(self, reset=False):
+        tot = np.zeros(self.R, np.int64); last = np.zeros(self.R, np.int64)
+        _check(self.L, self.L.fs_get_counters(self.h, tot.ctypes.data, last.ctypes.data, int(reset)))
+        return tot, last
+
+    def get_fields(self, which=FIELD_TOTAL) -> torch.Tensor:
+        shape = (self.R, self.N, 2) if self.R > 1 else (self.N, 2)
+        out = torch.empty(shape, dtype=torch.float64, device=self.device)
+        _check(self.L, self.L.fs_get_fields(self.h, int(which), out.data_ptr()))
+        return out
+
+    def get_flip_log(self, replica=0, cap=None) -> torch.Tensor:
+        cap = int(cap if cap is not None else 4 * self.N + 1024)
+        out = torch.empty(cap, dtype=torch.int32, device=self.device)
+        n = C.c_int64()
+        _check(self.L, self.L.fs_get_flip_log(self.h, int(replica), out.data_ptr(), cap, C.byref(n)))
+        self.last_log_count = int(n.value)
+        return out[:min(int(n.value), cap)]
+
+    def get_neighbors(self) -> torch.Tensor:
+        out = torch.empty((self.N, max(self.K, 1)), dtype=torch.int32, device=self.device)
+        k = C.c_int32()
+        _check(self.L, self.L.fs_get_neighbors(self.h, out.data_ptr(), C.byref(k)))
+        return out[:, :self.K]
+
+    # ---- host-buffer entry points (end-to-end timing)
+    def step_host(self, s_host: torch.Tensor, h_host_out: torch.Tensor):
+        assert s_host.dtype == torch.int8 and not s_host.is_cuda and s_host.numel() == self.R * self.N
+        assert h_host_out.dtype == torch.float64 and not h_host_out.is_cuda and h_host_out.numel() == 2 * self.R * self.N
+        n, b, l = C.c_int64(), C.c_int64(), C.c_double()
+        _check(self.L, self.L.fs_step_host(self.h, s_host.data_ptr(), h_host_out.data_ptr(), C.byref(n), C.byref(b), C.byref(l)))
+        return int(n.value), int(b.value), float(l.value)
+
+    def relax_host(self, hx, hy, step, s_host_out: torch.Tensor):
+        assert s_host_out.dtype == torch.int8 and not s_host_out.is_cuda and s_host_out.numel() == self.R * self.N
+        n = C.c_int64()
+        _check(self.L, self.L.fs_relax_host(self.h, float(hx), float(hy), int(step), s_host_out.data_ptr(), C.byref(n)))
+        return int(n.value)

@@ -1,0 +1,1180 @@
+// flatspin.cu -- B200 (sm_100a) kernels + C ABI of the flatspin hot path (include/flatspin.h).
+//
+// Written from /root/reference/PAPER.md (arxiv 2002.11401); PAPER.md lines are cited per kernel.
+// Shares no code with oracle/ (the CPU oracle) and never calls it.  No CPU fallback.
+//
+// Kernels (DESIGN.md "Kernels" has the roofline of each):
+//   k_frame            A0  cos/sin tables, hc validation                      (Eq. 1)
+//   k_bbox, k_cell_*   A1  cell grid (counting sort)
+//   k_count_neighbors  A1  degree of every spin, coincidence check
+//   k_fill_neighbors   A1  warp-per-spin collection + bitonic sort -> row-major ELL, ascending
+//   k_weights          A2  w_ij = alpha g_ij and its transpose                (Eq. 3)
+//   k_gather<G>        A3  h_dip,i = sum_k s_j w_ij, G lanes cooperate per row
+//   k_scan             A4-A7 total field + Philox thermal + astroid + margin + leaf-block arg-max
+//                                                                             (Eqs. 2,5,6)
+//   k_scan_finalize    A7  top-level arg-max + switchable count (fs_scan)
+//   k_relax            A7-A9 persistent single-CTA-per-replica relax loop with incremental updates
+//                                                                             (Eq. 3 linear in s_j)
+//   k_fields_out       fs_get_fields
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "flatspin.h"
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// host-side helpers
+// ------------------------------------------------------------------------------------------------
+thread_local char g_err[512] = "";
+std::atomic<long long> g_launches{0};
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof(g_err), fmt, ap); va_end(ap);
+    return code;
+}
+#define CUDA_TRY(expr)                                                                             \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess)                                                                    \
+            return fail(FS_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #expr, cudaGetErrorString(e__)); \
+    } while (0)
+#define LAUNCHED() (g_launches.fetch_add(1, std::memory_order_relaxed))
+
+constexpr int RELAX_THREADS = 512;
+constexpr int MAX_LEAF_BLOCKS = 8192;   // leaf-block maxima kept in the relax CTA's shared memory
+constexpr int MAX_K = 8192;             // maximum degree supported by the warp bitonic sort
+constexpr int SCAN_THREADS = 256;
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Counters {            // one per replica, device resident
+    long long total_flips;
+    long long last_flips;
+    long long n_switchable;
+    long long best_index;
+    double best_L;
+    int status;              // 1 = stopped by max_flips
+    int pad;
+};
+
+// ------------------------------------------------------------------------------------------------
+// device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool better(double va, int ia, double vb, int ib) {
+    // arg-max key: value descending, index ascending (lowest index wins exact ties; reading C-7)
+    return (va > vb) || (va == vb && ia < ib);
+}
+
+__device__ __forceinline__ void warp_argmax(double& v, int& i) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        double ov = __shfl_xor_sync(0xffffffffu, v, o);
+        int oi = __shfl_xor_sync(0xffffffffu, i, o);
+        if (better(ov, oi, v, i)) { v = ov; i = oi; }
+    }
+}
+
+// Philox4x32-10 (Salmon et al. SC'11), restated for the device.  counter = (spin, step, 0, 0),
+// key = (seed_lo, seed_hi)  (reading C-11).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// thermal field of spin i at `step` in global x,y: sigma * (z0, z1), Box-Muller on two 52-bit uniforms
+// (reading C-11)
+__device__ __forceinline__ double2 thermal_xy(double sigma, uint64_t seed, uint32_t step, uint32_t i) {
+    uint32_t x[4];
+    philox4x32_10(i, step, 0u, 0u, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), x);
+    uint64_t a = (((uint64_t)x[0] << 32) | x[1]) >> 12;
+    uint64_t b = (((uint64_t)x[2] << 32) | x[3]) >> 12;
+    const double two_m52 = 1.0 / 4503599627370496.0;
+    double u1 = ((double)a + 0.5) * two_m52;
+    double u2 = ((double)b + 0.5) * two_m52;
+    double r = sqrt(-2.0 * log(u1));
+    double sn, cs;
+    sincos(2.0 * CUDART_PI * u2, &sn, &cs);
+    return make_double2(sigma * r * cs, sigma * r * sn);
+}
+
+struct Astroid { double inv_b, inv_c, e_par, e_perp; };   // 1/b, 1/c, 2/gamma, 2/beta
+
+// switching margin M_i (Eq. 5 left-hand side if Eq. 6 holds, else -inf): PAPER.md:103, :112
+__device__ __forceinline__ double margin(double hpar, double hperp, double s, double hc, const Astroid& a) {
+    if (!(s * hpar < 0.0)) return -CUDART_INF;
+    double ihc = 1.0 / hc;
+    double x = fabs(hpar) * a.inv_b * ihc;
+    double y = fabs(hperp) * a.inv_c * ihc;
+    return pow(x, a.e_par) + pow(y, a.e_perp);
+}
+
+// ------------------------------------------------------------------------------------------------
+// A0: frame tables + hc validation
+// ------------------------------------------------------------------------------------------------
+__global__ void k_frame(int64_t N, int R, const double* __restrict__ angle, const double* __restrict__ hc,
+                        double2* __restrict__ cs, int* __restrict__ flags) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double sn, c;
+    sincos(angle[i], &sn, &c);
+    cs[i] = make_double2(c, sn);
+    bool bad = !isfinite(angle[i]);
+    for (int r = 0; r < R; ++r) {
+        double h = hc[(int64_t)r * N + i];
+        bad |= !(h > 0.0) || !isfinite(h);
+    }
+    if (bad) atomicOr(&flags[0], 1);
+}
+
+// ------------------------------------------------------------------------------------------------
+// A1: cell grid
+// ------------------------------------------------------------------------------------------------
+__global__ void k_bbox(int64_t N, const double2* __restrict__ pos, double* __restrict__ bbox /*xmin,ymin,xmax,ymax*/) {
+    __shared__ double sm[4][32];
+    double xmin = CUDART_INF, ymin = CUDART_INF, xmax = -CUDART_INF, ymax = -CUDART_INF;
+    bool bad = false;
+    for (int64_t i = threadIdx.x; i < N; i += blockDim.x) {
+        double2 p = pos[i];
+        bad |= !isfinite(p.x) || !isfinite(p.y);
+        xmin = fmin(xmin, p.x); xmax = fmax(xmax, p.x);
+        ymin = fmin(ymin, p.y); ymax = fmax(ymax, p.y);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        xmin = fmin(xmin, __shfl_xor_sync(0xffffffffu, xmin, o));
+        ymin = fmin(ymin, __shfl_xor_sync(0xffffffffu, ymin, o));
+        xmax = fmax(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
+        ymax = fmax(ymax, __shfl_xor_sync(0xffffffffu, ymax, o));
+    }
+    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) { sm[0][w] = xmin; sm[1][w] = ymin; sm[2][w] = xmax; sm[3][w] = ymax; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int nw = blockDim.x >> 5;
+        for (int k = 1; k < nw; ++k) {
+            xmin = fmin(xmin, sm[0][k]); ymin = fmin(ymin, sm[1][k]);
+            xmax = fmax(xmax, sm[2][k]); ymax = fmax(ymax, sm[3][k]);
+        }
+        bbox[0] = xmin; bbox[1] = ymin; bbox[2] = xmax; bbox[3] = ymax;
+    }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) bbox[0] = CUDART_NAN;
+}
+
+struct Grid { double x0, y0, inv_cell; int ncx, ncy; };
+
+__device__ __forceinline__ void cell_xy(const Grid& g, double2 p, int& cx, int& cy) {
+    cx = min(g.ncx - 1, max(0, (int)floor((p.x - g.x0) * g.inv_cell)));
+    cy = min(g.ncy - 1, max(0, (int)floor((p.y - g.y0) * g.inv_cell)));
+}
+
+__global__ void k_cell_count(int64_t N, Grid g, const double2* __restrict__ pos, int* __restrict__ cell_of,
+                             int* __restrict__ cell_cnt) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int cx, cy; cell_xy(g, pos[i], cx, cy);
+    int c = cy * g.ncx + cx;
+    cell_of[i] = c;
+    atomicAdd(&cell_cnt[c], 1);
+}
+
+// single-CTA exclusive scan: cell_start[c] = sum_{c'<c} cnt[c'];  cell_start[ncells] = N
+__global__ void k_cell_scan(int ncells, const int* __restrict__ cnt, int* __restrict__ start, int* __restrict__ fill) {
+    __shared__ int wsum[32];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int base = 0; base < ncells; base += blockDim.x) {
+        int c = base + threadIdx.x;
+        int v = (c < ncells) ? cnt[c] : 0;
+        int incl = v;
+        for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+        if (lane == 31) wsum[w] = incl;
+        __syncthreads();
+        if (w == 0) {
+            int t = (lane < nw) ? wsum[lane] : 0, inc2 = t;
+            for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, inc2, o); if (lane >= o) inc2 += u; }
+            wsum[lane] = inc2 - t;   // exclusive offsets of the warps
+        }
+        __syncthreads();
+        int excl = carry + wsum[w] + incl - v;
+        if (c < ncells) { start[c] = excl; fill[c] = excl; }
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry = excl + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) start[ncells] = carry;
+}
+
+__global__ void k_cell_scatter(int64_t N, const int* __restrict__ cell_of, int* __restrict__ fill, int* __restrict__ items) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int slot = atomicAdd(&fill[cell_of[i]], 1);
+    items[slot] = (int)i;      // order inside a cell is arbitrary; every ELL row is sorted afterwards
+}
+
+// degree of every spin; flags bit 1 = coincident pair.  One thread per spin over the 3x3 cells.
+__global__ void k_count_neighbors(int64_t N, Grid g, double cut2, const double2* __restrict__ pos,
+                                  const int* __restrict__ cell_start, const int* __restrict__ items,
+                                  int* __restrict__ deg, int* __restrict__ flags, int* __restrict__ kmax,
+                                  unsigned long long* __restrict__ total) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int d = 0;
+    if (i < N) {
+        double2 p = pos[i];
+        int cx, cy; cell_xy(g, p, cx, cy);
+        for (int yy = max(0, cy - 1); yy <= min(g.ncy - 1, cy + 1); ++yy)
+            for (int xx = max(0, cx - 1); xx <= min(g.ncx - 1, cx + 1); ++xx) {
+                int c = yy * g.ncx + xx;
+                for (int q = cell_start[c]; q < cell_start[c + 1]; ++q) {
+                    int j = items[q];
+                    if (j == (int)i) continue;
+                    double2 pj = pos[j];
+                    double dx = p.x - pj.x, dy = p.y - pj.y;
+                    double d2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+                    if (d2 == 0.0) atomicOr(&flags[0], 2);
+                    else if (d2 <= cut2) ++d;
+                }
+            }
+        deg[i] = d;
+    }
+    int m = d;
+    unsigned long long sum = d;
+    for (int o = 16; o > 0; o >>= 1) {
+        m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+        sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicMax(kmax, m); atomicAdd(total, sum); }
+}
+
+// warp per spin: collect neighbours into shared memory, bitonic sort ascending, write the ELL row.
+__global__ void k_fill_neighbors(int64_t N, Grid g, double cut2, int Kp, int Kp2,
+                                 const double2* __restrict__ pos, const int* __restrict__ cell_start,
+                                 const int* __restrict__ items, int* __restrict__ nbr) {
+    extern __shared__ int sm_i[];
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    int* buf = sm_i + (size_t)w * Kp2;
+    for (int64_t i = blockIdx.x * (int64_t)nw + w; i < N; i += (int64_t)gridDim.x * nw) {
+        double2 p = pos[i];
+        int cx, cy; cell_xy(g, p, cx, cy);
+        int n = 0;
+        for (int yy = max(0, cy - 1); yy <= min(g.ncy - 1, cy + 1); ++yy)
+            for (int xx = max(0, cx - 1); xx <= min(g.ncx - 1, cx + 1); ++xx) {
+                int c = yy * g.ncx + xx;
+                int q0 = cell_start[c], q1 = cell_start[c + 1];
+                for (int q = q0 + lane; q - lane < q1; q += 32) {
+                    bool ok = false; int j = -1;
+                    if (q < q1) {
+                        j = items[q];
+                        if (j != (int)i) {
+                            double2 pj = pos[j];
+                            double dx = p.x - pj.x, dy = p.y - pj.y;
+                            double d2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+                            ok = (d2 != 0.0) && (d2 <= cut2);
+                        }
+                    }
+                    unsigned m = __ballot_sync(0xffffffffu, ok);
+                    if (ok) buf[n + __popc(m & ((1u << lane) - 1u))] = j;
+                    n += __popc(m);
+                }
+            }
+        for (int k = n + lane; k < Kp2; k += 32) buf[k] = 0x7fffffff;
+        __syncwarp();
+        for (int size = 2; size <= Kp2; size <<= 1)
+            for (int stride = size >> 1; stride > 0; stride >>= 1) {
+                for (int t = lane; t < (Kp2 >> 1); t += 32) {
+                    int lo = 2 * t - (t & (stride - 1));       // index with bit `stride` cleared
+                    int hi = lo + stride;
+                    bool up = ((lo & size) == 0);
+                    int a = buf[lo], b = buf[hi];
+                    if ((a > b) == up) { buf[lo] = b; buf[hi] = a; }
+                }
+                __syncwarp();
+            }
+        int* row = nbr + i * (int64_t)Kp;
+        for (int k = lane; k < Kp; k += 32) row[k] = (k < n) ? buf[k] : -1;
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A2: couplings.  Field at a from a unit moment at b, in a's fixed frame, times alpha (Eq. 3):
+//     H = 3 r (m_b . r)/|r|^5 - m_b/|r|^3,  r = r_a - r_b;  (par, perp) = (H . m^_a, H . m^_a_perp)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double2 coupling(double2 pa, double2 ca, double2 pb, double2 cb, double alpha) {
+    double dx = pa.x - pb.x, dy = pa.y - pb.y;
+    double d2 = dx * dx + dy * dy;
+    double inv = 1.0 / sqrt(d2);
+    double inv3 = inv * inv * inv, inv5 = inv3 * inv * inv;
+    double dot = cb.x * dx + cb.y * dy;
+    double Hx = 3.0 * dx * dot * inv5 - cb.x * inv3;
+    double Hy = 3.0 * dy * dot * inv5 - cb.y * inv3;
+    return make_double2(alpha * (Hx * ca.x + Hy * ca.y), alpha * (-Hx * ca.y + Hy * ca.x));
+}
+
+__global__ void k_weights(int64_t N, int Kp, double alpha, const double2* __restrict__ pos,
+                          const double2* __restrict__ cs, const int* __restrict__ nbr,
+                          double2* __restrict__ w, double2* __restrict__ wT) {
+    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t >= N * Kp) return;
+    int64_t i = t / Kp;
+    int j = nbr[t];
+    double2 a = make_double2(0.0, 0.0), b = a;
+    if (j >= 0) {
+        a = coupling(pos[i], cs[i], pos[j], cs[j], alpha);   // field at i from j
+        b = coupling(pos[j], cs[j], pos[i], cs[i], alpha);   // field at j from i
+    }
+    w[t] = a;
+    wT[t] = b;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A3: full gather.  G lanes cooperate on one ELL row; each lane takes 4 consecutive slots per step
+// (one 16-byte index load + four 16-byte weight loads), partial sums folded with warp shuffles in a
+// fixed order (deterministic).  blockIdx.y = replica.
+// ------------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(256) k_gather(int64_t N, int Kp, const int* __restrict__ nbr,
+                                                const double2* __restrict__ w, const int8_t* __restrict__ s_all,
+                                                double2* __restrict__ hdip_all) {
+    const int8_t* __restrict__ s = s_all + (int64_t)blockIdx.y * N;
+    double2* __restrict__ hdip = hdip_all + (int64_t)blockIdx.y * N;
+    int64_t tid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int g = (int)(tid % G);
+    const int64_t ngroups = (int64_t)gridDim.x * blockDim.x / G;
+    const int64_t warp_first = (tid - (threadIdx.x & 31)) / G;      // group of lane 0: warp-uniform loop bound
+    for (int64_t base = 0; warp_first + base < N; base += ngroups) {
+        const int64_t i = tid / G + base;
+        double ax = 0.0, ay = 0.0, bx = 0.0, by = 0.0;
+        if (i < N) {
+            const int4* rowi = reinterpret_cast<const int4*>(nbr + i * (int64_t)Kp);
+            const double2* roww = w + i * (int64_t)Kp;
+#pragma unroll 2
+            for (int k4 = g; k4 < (Kp >> 2); k4 += G) {
+                int4 j = __ldg(rowi + k4);
+                const double2* ww = roww + 4 * k4;
+                if (j.x >= 0) { double2 v = __ldg(ww + 0); double sj = (double)s[j.x]; ax = fma(sj, v.x, ax); ay = fma(sj, v.y, ay); }
+                if (j.y >= 0) { double2 v = __ldg(ww + 1); double sj = (double)s[j.y]; bx = fma(sj, v.x, bx); by = fma(sj, v.y, by); }
+                if (j.z >= 0) { double2 v = __ldg(ww + 2); double sj = (double)s[j.z]; ax = fma(sj, v.x, ax); ay = fma(sj, v.y, ay); }
+                if (j.w >= 0) { double2 v = __ldg(ww + 3); double sj = (double)s[j.w]; bx = fma(sj, v.x, bx); by = fma(sj, v.y, by); }
+            }
+        }
+        ax += bx; ay += by;
+#pragma unroll
+        for (int o = G >> 1; o > 0; o >>= 1) {
+            ax += __shfl_xor_sync(0xffffffffu, ax, o);
+            ay += __shfl_xor_sync(0xffffffffu, ay, o);
+        }
+        if (g == 0 && i < N) hdip[i] = make_double2(ax, ay);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A4-A7: fused scan.  One thread per spin; writes hfix = rot(h_ext + h_th), the margin M and the
+// arg-max of every leaf block of LB spins.  blockIdx.y = replica.
+// ------------------------------------------------------------------------------------------------
+struct FieldSpec { double sigma; uint64_t seed; uint32_t step; };
+
+__global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs,
+                                               const double2* __restrict__ hext_all /*[R] (hx,hy)*/,
+                                               const double2* __restrict__ cs, const double* __restrict__ hc_all,
+                                               const int8_t* __restrict__ s_all, const double2* __restrict__ hdip_all,
+                                               double2* __restrict__ hfix_all, double* __restrict__ M_all,
+                                               double* __restrict__ bval_all, int* __restrict__ bidx_all, int nblk,
+                                               Counters* __restrict__ ctr) {
+    __shared__ double wv[32];
+    __shared__ int wi[32];
+    int r = blockIdx.y;
+    int64_t off = (int64_t)r * N;
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    double m = -CUDART_INF; int mi = 0x7fffffff;
+    if (i < N) {
+        double2 c = cs[i];
+        double2 he = hext_all[r];
+        double ex = he.x, ey = he.y;
+        if (fs.sigma != 0.0) {
+            double2 t = thermal_xy(fs.sigma, fs.seed + (uint64_t)r, fs.step, (uint32_t)i);
+            // (ext + th) rotated together would round differently from the paper's sum of three fields;
+            // rotate separately and add (Eq. 2)
+            double tp = t.x * c.x + t.y * c.y, tq = -t.x * c.y + t.y * c.x;
+            double ep = ex * c.x + ey * c.y, eq = -ex * c.y + ey * c.x;
+            hfix_all[off + i] = make_double2(ep + tp, eq + tq);
+        } else {
+            hfix_all[off + i] = make_double2(ex * c.x + ey * c.y, -ex * c.y + ey * c.x);
+        }
+        double2 hf = hfix_all[off + i];
+        double2 hd = hdip_all[off + i];
+        m = margin(hd.x + hf.x, hd.y + hf.y, (double)s_all[off + i], hc_all[off + i], ast);
+        M_all[off + i] = m;
+        mi = (int)i;
+    }
+    unsigned long long nsw = __popcll(__ballot_sync(0xffffffffu, m > 1.0));
+    warp_argmax(m, mi);
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (LB == 32) {
+        int blk = (int)(blockIdx.x * (int64_t)(blockDim.x >> 5) + w);
+        if (lane == 0 && blk < nblk) { bval_all[(int64_t)r * nblk + blk] = m; bidx_all[(int64_t)r * nblk + blk] = mi; }
+    } else {
+        if (lane == 0) { wv[w] = m; wi[w] = mi; }
+        __syncthreads();
+        int wpl = LB >> 5;                               // warps per leaf block
+        if (lane == 0 && (w % wpl) == 0) {
+            double bv = wv[w]; int bi = wi[w];
+            for (int k = 1; k < wpl; ++k) if (better(wv[w + k], wi[w + k], bv, bi)) { bv = wv[w + k]; bi = wi[w + k]; }
+            int blk = (int)((blockIdx.x * (int64_t)blockDim.x + threadIdx.x) / LB);
+            if (blk < nblk) { bval_all[(int64_t)r * nblk + blk] = bv; bidx_all[(int64_t)r * nblk + blk] = bi; }
+        }
+    }
+    if (lane == 0 && nsw) atomicAdd((unsigned long long*)&ctr[r].n_switchable, nsw);
+}
+
+__global__ void k_scan_finalize(int nblk, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
+                                Counters* __restrict__ ctr) {
+    __shared__ double wv[32];
+    __shared__ int wi[32];
+    int r = blockIdx.x;
+    const double* bval = bval_all + (int64_t)r * nblk;
+    const int* bidx = bidx_all + (int64_t)r * nblk;
+    double v = -CUDART_INF; int bi = 0x7fffffff;
+    for (int t = threadIdx.x; t < nblk; t += blockDim.x)
+        if (better(bval[t], bidx[t], v, bi)) { v = bval[t]; bi = bidx[t]; }
+    warp_argmax(v, bi);
+    if ((threadIdx.x & 31) == 0) { wv[threadIdx.x >> 5] = v; wi[threadIdx.x >> 5] = bi; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < (int)(blockDim.x >> 5); ++k) if (better(wv[k], wi[k], v, bi)) { v = wv[k]; bi = wi[k]; }
+        bool any = v > 1.0;
+        ctr[r].best_index = any ? bi : -1;
+        ctr[r].best_L = any ? v : -CUDART_INF;
+    }
+}
+
+__global__ void k_reset_scan_counters(int R, Counters* ctr) {
+    int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < R) { ctr[r].n_switchable = 0; ctr[r].best_index = -1; ctr[r].best_L = -CUDART_INF; }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A7-A9: relax loop.  One persistent CTA per replica; leaf-block maxima live in shared memory; per
+// flip: top arg-max (shared memory) -> row k of the transposed ELL -> neighbours' h_dip -= 2 s_k w_ik
+// (Eq. 3 is linear in s_k) -> margins of nbr(k) U {k} -> repair the touched leaf blocks.
+// No host round trip and no grid-wide barrier per flip.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(RELAX_THREADS, 1)
+k_relax(int64_t N, int Kp, int LB, int nblk, Astroid ast, long long max_flips, long long log_cap,
+        const int* __restrict__ nbr, const double2* __restrict__ wT, const double* __restrict__ hc_all,
+        int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, const double2* __restrict__ hfix_all,
+        double* __restrict__ M_all, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
+        int* __restrict__ log_all, Counters* __restrict__ ctr) {
+    extern __shared__ unsigned char smem_raw[];
+    double* bval = reinterpret_cast<double*>(smem_raw);
+    int* bidx = reinterpret_cast<int*>(bval + nblk);
+    int* touched = bidx + nblk;                       // [Kp + 1] leaf blocks touched by this flip
+    __shared__ double wv[RELAX_THREADS / 32];
+    __shared__ int wi[RELAX_THREADS / 32];
+
+    const int r = blockIdx.x;
+    const int64_t off = (int64_t)r * N;
+    const double* hc = hc_all + off;
+    int8_t* s = s_all + off;
+    double2* hdip = hdip_all + off;
+    const double2* hfix = hfix_all + off;
+    double* M = M_all + off;
+    int* flog = log_all + (int64_t)r * log_cap;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = RELAX_THREADS / 32;
+
+    for (int t = tid; t < nblk; t += RELAX_THREADS) {
+        bval[t] = bval_all[(int64_t)r * nblk + t];
+        bidx[t] = bidx_all[(int64_t)r * nblk + t];
+    }
+    __syncthreads();
+
+    long long nflips = 0;
+    int status = 0;
+    for (;;) {
+        // ---- A7: top-level arg-max over the leaf-block maxima
+        double v = -CUDART_INF; int k = 0x7fffffff;
+        for (int t = tid; t < nblk; t += RELAX_THREADS)
+            if (better(bval[t], bidx[t], v, k)) { v = bval[t]; k = bidx[t]; }
+        warp_argmax(v, k);
+        if (lane == 0) { wv[warp] = v; wi[warp] = k; }
+        __syncthreads();
+        v = (lane < NW) ? wv[lane] : -CUDART_INF;
+        k = (lane < NW) ? wi[lane] : 0x7fffffff;
+        warp_argmax(v, k);                              // every warp reduces the NW partials redundantly
+        if (!(v > 1.0)) break;                          // no switchable spin left
+        if (max_flips > 0 && nflips >= max_flips) { status = 1; break; }
+
+        // ---- A8: flip k, update its neighbours incrementally, recompute their margins
+        const int8_t s_old = s[k];                      // s[k] is rewritten only after the barrier below
+        const int* rowk = nbr + (int64_t)k * Kp;
+        const double2* wTk = wT + (int64_t)k * Kp;
+        int ntouch = 0;
+        for (int t = tid; t <= Kp; t += RELAX_THREADS) {
+            int blk = -1;
+            if (t == Kp) {                              // the flipped spin itself
+                double2 hd = hdip[k], hf = hfix[k];
+                M[k] = margin(hd.x + hf.x, hd.y + hf.y, -(double)s_old, hc[k], ast);
+                blk = k / LB;
+            } else {
+                int i = rowk[t];
+                if (i >= 0) {
+                    double2 wt = wTk[t];
+                    double2 hd = hdip[i], hf = hfix[i];
+                    double two_s = 2.0 * (double)s_old;
+                    hd.x -= two_s * wt.x;               // h_i -= 2 s_k,old alpha g_ik
+                    hd.y -= two_s * wt.y;
+                    hdip[i] = hd;
+                    M[i] = margin(hd.x + hf.x, hd.y + hf.y, (double)s[i], hc[i], ast);
+                    blk = i / LB;
+                }
+            }
+            touched[t] = blk;
+        }
+        (void)ntouch;
+        __syncthreads();
+        if (tid == 0) {
+            s[k] = (int8_t)(-s_old);
+            if (nflips < log_cap) flog[nflips] = k;
+        }
+        // ---- A7 repair: recompute the maxima of the touched leaf blocks (one warp per block)
+        for (int t = warp; t <= Kp; t += NW) {
+            int blk = touched[t];
+            if (blk < 0) continue;
+            bool dup = false;                           // skip if an earlier entry names the same block
+            for (int u = lane; u < t; u += 32) dup |= (touched[u] == blk);
+            if (__any_sync(0xffffffffu, dup)) continue;
+            double bv = -CUDART_INF; int bi = 0x7fffffff;
+            int64_t base = (int64_t)blk * LB;
+            for (int q = lane; q < LB; q += 32) {
+                int64_t i = base + q;
+                if (i < N) { double m = M[i]; if (better(m, (int)i, bv, bi)) { bv = m; bi = (int)i; } }
+            }
+            warp_argmax(bv, bi);
+            if (lane == 0) { bval[blk] = bv; bidx[blk] = bi; }
+        }
+        ++nflips;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        ctr[r].total_flips += nflips;
+        ctr[r].last_flips = nflips;
+        ctr[r].status = status;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// fs_get_fields
+// ------------------------------------------------------------------------------------------------
+__global__ void k_fields_out(int64_t N, int which, FieldSpec fs, const double2* __restrict__ hext_all,
+                             const double2* __restrict__ cs, const double2* __restrict__ hdip_all,
+                             double2* __restrict__ out_all) {
+    int r = blockIdx.y;
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double2 c = cs[i];
+    double2 he = hext_all[r];
+    double2 d = hdip_all[(int64_t)r * N + i];
+    double2 e = make_double2(he.x * c.x + he.y * c.y, -he.x * c.y + he.y * c.x);
+    double2 t = make_double2(0.0, 0.0);
+    if (fs.sigma != 0.0 && (which == FS_FIELD_TOTAL || which == FS_FIELD_THERMAL)) {
+        double2 g = thermal_xy(fs.sigma, fs.seed + (uint64_t)r, fs.step, (uint32_t)i);
+        t = make_double2(g.x * c.x + g.y * c.y, -g.x * c.y + g.y * c.x);
+    }
+    double2 o;
+    if (which == FS_FIELD_DIP) o = d;
+    else if (which == FS_FIELD_EXT) o = e;
+    else if (which == FS_FIELD_THERMAL) o = t;
+    else o = make_double2(d.x + e.x + t.x, d.y + e.y + t.y);
+    out_all[(int64_t)r * N + i] = o;
+}
+
+__global__ void k_set_field(int R, double hx, double hy, double2* hext) {
+    int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < R) hext[r] = make_double2(hx, hy);
+}
+
+__global__ void k_fill_i8(int64_t n, int8_t v, int8_t* p) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
+}  // namespace
+
+// ================================================================================================
+// host side
+// ================================================================================================
+struct fs_sim {
+    int64_t N = 0; int R = 1; int K = 0, Kp = 4, LB = 32, nblk = 0, ncells = 0;
+    int64_t n_inter = 0, log_cap = 0;
+    fs_params p{};
+    Astroid ast{};
+    Grid grid{};
+    cudaStream_t stream = nullptr;
+    int sm_count = 148;
+    // geometry
+    double2 *pos = nullptr, *cs = nullptr, *w = nullptr, *wT = nullptr;
+    int *nbr = nullptr, *deg = nullptr;
+    // per replica
+    double* hc = nullptr; int8_t* s = nullptr; double2 *hdip = nullptr, *hfix = nullptr; double* M = nullptr;
+    double* bval = nullptr; int* bidx = nullptr; int* flog = nullptr; Counters* ctr = nullptr;
+    double2* hext = nullptr;     // [R] device copy of the global field
+    // state
+    bool fields_dirty = true;
+    double sigma = 0.0; uint64_t seed = 0; uint32_t step = 0;
+    double2* hext_host = nullptr;   // pinned staging [R]
+    Counters* ctr_host = nullptr;   // pinned staging [R]
+    int gather_variant = FS_GATHER_AUTO;
+    size_t relax_smem = 0;
+};
+
+namespace {
+
+struct GridPlan {
+    Grid g; int ncells; double cut2;
+};
+
+struct Layout {
+    // grid-phase buffers (depend on N, ncells only)
+    size_t scratch, cell_of, cell_cnt, cell_start, cell_fill, items, deg;
+    size_t grid_end;
+    // K-dependent
+    size_t pos, cs, nbr, w, wT, hc, s, hdip, hfix, M, bval, bidx, flog, ctr, hext, total;
+};
+
+int choose_leaf(int64_t N, int* LB, int* nblk) {
+    for (int lb = 32; lb <= 1024; lb <<= 1) {
+        int64_t nb = (N + lb - 1) / lb;
+        if (nb <= MAX_LEAF_BLOCKS) { *LB = lb; *nblk = (int)nb; return 0; }
+    }
+    return -1;
+}
+
+void layout_grid(Layout& L, int64_t N, int ncells) {
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    L.scratch = take(256);
+    L.cell_of = take(sizeof(int) * N);
+    L.cell_cnt = take(sizeof(int) * (size_t)(ncells + 1));
+    L.cell_start = take(sizeof(int) * (size_t)(ncells + 1));
+    L.cell_fill = take(sizeof(int) * (size_t)(ncells + 1));
+    L.items = take(sizeof(int) * N);
+    L.deg = take(sizeof(int) * N);
+    L.grid_end = o;
+}
+
+void layout_rest(Layout& L, int64_t N, int R, int Kp, int nblk, int64_t log_cap) {
+    size_t o = L.grid_end;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    size_t NK = (size_t)N * Kp, RN = (size_t)R * N;
+    L.pos = take(16 * (size_t)N);
+    L.cs = take(16 * (size_t)N);
+    L.nbr = take(4 * NK);
+    L.w = take(16 * NK);
+    L.wT = take(16 * NK);
+    L.hc = take(8 * RN);
+    L.s = take(RN);
+    L.hdip = take(16 * RN);
+    L.hfix = take(16 * RN);
+    L.M = take(8 * RN);
+    L.bval = take(8 * (size_t)R * nblk);
+    L.bidx = take(4 * (size_t)R * nblk);
+    L.flog = take(4 * (size_t)R * log_cap);
+    L.ctr = take(sizeof(Counters) * (size_t)R);
+    L.hext = take(16 * (size_t)R);
+    L.total = o;
+}
+
+int check_params(int64_t N, int R, const fs_params* p) {
+    if (!p) return fail(FS_ERR_ARG, "params is NULL");
+    if (N <= 0 || N > 0x7ffffff0LL) return fail(FS_ERR_ARG, "N=%lld out of range", (long long)N);
+    if (R <= 0) return fail(FS_ERR_ARG, "R=%d must be positive", R);
+    if (!(p->b > 0) || !(p->c > 0) || !(p->beta > 0) || !(p->gamma > 0) || !(p->neighbor_distance > 0) ||
+        !std::isfinite(p->alpha) || !std::isfinite(p->neighbor_distance))
+        return fail(FS_ERR_ARG, "b, c, beta, gamma, neighbor_distance must be > 0 and alpha finite");
+    return FS_OK;
+}
+
+// bounding box -> cell grid plan.  `bbox_dev` = 4 doubles of device scratch.  Synchronises.
+int plan_grid(int64_t N, const double* pos_dev, const fs_params* p, double* bbox_dev, cudaStream_t st, GridPlan* out) {
+    k_bbox<<<1, 1024, 0, st>>>(N, reinterpret_cast<const double2*>(pos_dev), bbox_dev); LAUNCHED();
+    double bb[4];
+    CUDA_TRY(cudaMemcpyAsync(bb, bbox_dev, sizeof(bb), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (!(bb[0] == bb[0])) return fail(FS_ERR_ARG, "non-finite position");
+    double cell = p->neighbor_distance * (1.0 + 1e-6);
+    double ex = bb[2] - bb[0], ey = bb[3] - bb[1];
+    // cap the number of cells at ~4N (sparse point sets / tiny cutoffs): larger cells stay correct
+    for (;;) {
+        double nx = std::floor(ex / cell) + 1.0, ny = std::floor(ey / cell) + 1.0;
+        if (nx * ny <= 4.0 * (double)N + 1024.0) break;
+        cell *= 1.5;
+    }
+    out->g.x0 = bb[0]; out->g.y0 = bb[1]; out->g.inv_cell = 1.0 / cell;
+    out->g.ncx = (int)(std::floor(ex / cell) + 1.0);
+    out->g.ncy = (int)(std::floor(ey / cell) + 1.0);
+    out->ncells = out->g.ncx * out->g.ncy;
+    out->cut2 = p->neighbor_distance * p->neighbor_distance * (1.0 + 1e-9);
+    return FS_OK;
+}
+
+// cell grid + degree count inside `base` laid out by layout_grid.  Synchronises; returns K, I, flags.
+int build_grid_and_count(int64_t N, const double* pos_dev, const GridPlan& gp, unsigned char* base, const Layout& L,
+                         cudaStream_t st, int* K, long long* I, int* flags) {
+    int* cell_of = (int*)(base + L.cell_of); int* cell_cnt = (int*)(base + L.cell_cnt);
+    int* cell_start = (int*)(base + L.cell_start); int* cell_fill = (int*)(base + L.cell_fill);
+    int* items = (int*)(base + L.items); int* deg = (int*)(base + L.deg);
+    int* scr = (int*)(base + L.scratch);                 // [8]=flags, [9]=kmax, [10..11]=total (after 4 bbox doubles)
+    const double2* pos = reinterpret_cast<const double2*>(pos_dev);
+    CUDA_TRY(cudaMemsetAsync(cell_cnt, 0, sizeof(int) * (size_t)(gp.ncells + 1), st));
+    CUDA_TRY(cudaMemsetAsync(scr + 9, 0, 3 * sizeof(int), st));    // kmax + total (flags keep k_frame's bits)
+    int nb = (int)((N + 255) / 256);
+    k_cell_count<<<nb, 256, 0, st>>>(N, gp.g, pos, cell_of, cell_cnt); LAUNCHED();
+    k_cell_scan<<<1, 1024, 0, st>>>(gp.ncells, cell_cnt, cell_start, cell_fill); LAUNCHED();
+    k_cell_scatter<<<nb, 256, 0, st>>>(N, cell_of, cell_fill, items); LAUNCHED();
+    k_count_neighbors<<<nb, 256, 0, st>>>(N, gp.g, gp.cut2, pos, cell_start, items, deg, scr + 8, scr + 9,
+                                          (unsigned long long*)(scr + 10)); LAUNCHED();
+    int host[4];
+    CUDA_TRY(cudaMemcpyAsync(host, scr + 8, sizeof(host), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaGetLastError());
+    *flags = host[0]; *K = host[1];
+    unsigned long long tot; std::memcpy(&tot, host + 2, 8); *I = (long long)tot;
+    return FS_OK;
+}
+
+int pad_k(int K) { int kp = (K + 3) / 4 * 4; return kp < 4 ? 4 : kp; }
+
+template <int G>
+void launch_gather_g(fs_sim* sim) {
+    int occ = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_gather<G>, 256, 0);
+    if (occ < 1) occ = 1;
+    int64_t groups_per_block = 256 / G;
+    int64_t need = (sim->N + groups_per_block - 1) / groups_per_block;
+    int64_t blocks = std::min<int64_t>(need, (int64_t)sim->sm_count * occ * 4);
+    dim3 grid((unsigned)blocks, (unsigned)sim->R);
+    k_gather<G><<<grid, 256, 0, sim->stream>>>(sim->N, sim->Kp, sim->nbr, sim->w, sim->s, sim->hdip);
+    LAUNCHED();
+}
+
+int do_gather(fs_sim* sim) {
+    int q = sim->Kp / 4;
+    if (q <= 1) launch_gather_g<1>(sim);
+    else if (q <= 2) launch_gather_g<2>(sim);
+    else if (q <= 4) launch_gather_g<4>(sim);
+    else if (q <= 8) launch_gather_g<8>(sim);
+    else if (q <= 16) launch_gather_g<16>(sim);
+    else launch_gather_g<32>(sim);
+    CUDA_TRY(cudaGetLastError());
+    sim->fields_dirty = false;
+    return FS_OK;
+}
+
+int ensure_fields(fs_sim* sim) { return sim->fields_dirty ? do_gather(sim) : FS_OK; }
+
+int do_scan(fs_sim* sim, bool count) {
+    int rc = ensure_fields(sim);
+    if (rc) return rc;
+    if (count) { k_reset_scan_counters<<<(sim->R + 127) / 128, 128, 0, sim->stream>>>(sim->R, sim->ctr); LAUNCHED(); }
+    int threads = sim->LB > SCAN_THREADS ? sim->LB : SCAN_THREADS;
+    dim3 grid((unsigned)((sim->N + threads - 1) / threads), (unsigned)sim->R);
+    FieldSpec fsp{sim->sigma, sim->seed, sim->step};
+    k_scan<<<grid, threads, 0, sim->stream>>>(sim->N, sim->LB, sim->ast, fsp, sim->hext, sim->cs, sim->hc, sim->s,
+                                               sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->ctr);
+    LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    return FS_OK;
+}
+
+int push_field(fs_sim* sim) {
+    CUDA_TRY(cudaMemcpyAsync(sim->hext, sim->hext_host, sizeof(double2) * sim->R, cudaMemcpyHostToDevice, sim->stream));
+    return FS_OK;
+}
+
+int fetch_counters(fs_sim* sim) {
+    CUDA_TRY(cudaMemcpyAsync(sim->ctr_host, sim->ctr, sizeof(Counters) * sim->R, cudaMemcpyDeviceToHost, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    return FS_OK;
+}
+
+int do_relax(fs_sim* sim, int64_t max_flips) {
+    int rc = do_scan(sim, false);
+    if (rc) return rc;
+    k_relax<<<sim->R, RELAX_THREADS, sim->relax_smem, sim->stream>>>(
+        sim->N, sim->Kp, sim->LB, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr,
+        sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr);
+    LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    return FS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* fs_last_error(void) { return g_err; }
+int64_t fs_kernel_launches(void) { return (int64_t)g_launches.load(); }
+
+int fs_workspace_bytes(int64_t N, int32_t R, const double* pos_dev, const fs_params* p, size_t* bytes_out, void* stream) {
+    int rc = check_params(N, R, p);
+    if (rc) return rc;
+    if (!pos_dev || !bytes_out) return fail(FS_ERR_ARG, "null pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    double* bbox = nullptr;
+    CUDA_TRY(cudaMalloc(&bbox, 256));
+    GridPlan gp;
+    rc = plan_grid(N, pos_dev, p, bbox, st, &gp);
+    cudaFree(bbox);
+    if (rc) return rc;
+    Layout L{};
+    layout_grid(L, N, gp.ncells);
+    unsigned char* tmp = nullptr;
+    CUDA_TRY(cudaMalloc(&tmp, L.grid_end));
+    cudaMemsetAsync(tmp, 0, 256, st);
+    int K = 0, flags = 0; long long I = 0;
+    rc = build_grid_and_count(N, pos_dev, gp, tmp, L, st, &K, &I, &flags);
+    cudaFree(tmp);
+    if (rc) return rc;
+    if (flags & 2) return fail(FS_ERR_COINCIDENT, "two spins share a position");
+    if (K > MAX_K) return fail(FS_ERR_ARG, "max degree %d exceeds %d", K, MAX_K);
+    int LB, nblk;
+    if (choose_leaf(N, &LB, &nblk)) return fail(FS_ERR_ARG, "N too large for the relax hierarchy");
+    layout_rest(L, N, R, pad_k(K), nblk, 4 * N + 1024);
+    *bytes_out = L.total;
+    return FS_OK;
+}
+
+int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev, const double* angle_dev,
+                       const double* hc_dev, const fs_params* p, void* workspace_dev, size_t workspace_bytes,
+                       void* stream) {
+    int rc = check_params(N, R, p);
+    if (rc) return rc;
+    if (!out || !pos_dev || !angle_dev || !hc_dev || !workspace_dev) return fail(FS_ERR_ARG, "null pointer");
+    if (((uintptr_t)workspace_dev & 255u) != 0) return fail(FS_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char* base = (unsigned char*)workspace_dev;
+    if (workspace_bytes < 256) return fail(FS_ERR_WORKSPACE, "workspace too small");
+    CUDA_TRY(cudaMemsetAsync(base, 0, 256, st));
+
+    GridPlan gp;
+    rc = plan_grid(N, pos_dev, p, (double*)base, st, &gp);
+    if (rc) return rc;
+    Layout L{};
+    layout_grid(L, N, gp.ncells);
+    if (workspace_bytes < L.grid_end) return fail(FS_ERR_WORKSPACE, "workspace too small (%zu < %zu)", workspace_bytes, L.grid_end);
+    int K = 0, flags = 0; long long I = 0;
+    rc = build_grid_and_count(N, pos_dev, gp, base, L, st, &K, &I, &flags);
+    if (rc) return rc;
+    if (flags & 2) return fail(FS_ERR_COINCIDENT, "two spins share a position");
+    if (K > MAX_K) return fail(FS_ERR_ARG, "max degree %d exceeds %d", K, MAX_K);
+    int LB, nblk;
+    if (choose_leaf(N, &LB, &nblk)) return fail(FS_ERR_ARG, "N too large for the relax hierarchy");
+    int Kp = pad_k(K);
+    int64_t log_cap = 4 * N + 1024;
+    layout_rest(L, N, R, Kp, nblk, log_cap);
+    if (workspace_bytes < L.total) return fail(FS_ERR_WORKSPACE, "workspace too small (%zu < %zu)", workspace_bytes, L.total);
+
+    fs_sim* sim = new (std::nothrow) fs_sim();
+    if (!sim) return fail(FS_ERR_ARG, "out of host memory");
+    sim->N = N; sim->R = R; sim->K = K; sim->Kp = Kp; sim->LB = LB; sim->nblk = nblk; sim->ncells = gp.ncells;
+    sim->n_inter = I; sim->log_cap = log_cap; sim->p = *p; sim->grid = gp.g; sim->stream = st;
+    sim->ast = Astroid{1.0 / p->b, 1.0 / p->c, 2.0 / p->gamma, 2.0 / p->beta};
+    int dev = 0; cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sim->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    sim->pos = (double2*)(base + L.pos); sim->cs = (double2*)(base + L.cs);
+    sim->nbr = (int*)(base + L.nbr); sim->w = (double2*)(base + L.w); sim->wT = (double2*)(base + L.wT);
+    sim->deg = (int*)(base + L.deg);
+    sim->hc = (double*)(base + L.hc); sim->s = (int8_t*)(base + L.s);
+    sim->hdip = (double2*)(base + L.hdip); sim->hfix = (double2*)(base + L.hfix); sim->M = (double*)(base + L.M);
+    sim->bval = (double*)(base + L.bval); sim->bidx = (int*)(base + L.bidx); sim->flog = (int*)(base + L.flog);
+    sim->ctr = (Counters*)(base + L.ctr); sim->hext = (double2*)(base + L.hext);
+
+#define CREATE_TRY(expr)                                                                           \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            fs_destroy(sim);                                                                       \
+            return fail(FS_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #expr, cudaGetErrorString(e__)); \
+        }                                                                                          \
+    } while (0)
+    CREATE_TRY(cudaMallocHost(&sim->hext_host, sizeof(double2) * R));
+    CREATE_TRY(cudaMallocHost(&sim->ctr_host, sizeof(Counters) * R));
+    for (int r = 0; r < R; ++r) sim->hext_host[r] = make_double2(0.0, 0.0);
+
+    CREATE_TRY(cudaMemcpyAsync(sim->pos, pos_dev, 16 * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    CREATE_TRY(cudaMemcpyAsync(sim->hc, hc_dev, 8 * (size_t)R * N, cudaMemcpyDeviceToDevice, st));
+    CREATE_TRY(cudaMemsetAsync(sim->ctr, 0, sizeof(Counters) * R, st));
+    CREATE_TRY(cudaMemsetAsync(sim->hdip, 0, 16 * (size_t)R * N, st));
+    CREATE_TRY(cudaMemcpyAsync(sim->hext, sim->hext_host, sizeof(double2) * R, cudaMemcpyHostToDevice, st));
+    int nb = (int)((N + 255) / 256);
+    int* scr = (int*)(base + L.scratch);
+    k_frame<<<nb, 256, 0, st>>>(N, R, angle_dev, sim->hc, sim->cs, scr + 8); LAUNCHED();
+    {
+        int64_t rn = (int64_t)R * N;
+        k_fill_i8<<<(unsigned)((rn + 255) / 256), 256, 0, st>>>(rn, (int8_t)1, sim->s); LAUNCHED();
+    }
+    // A1 fill + sort
+    int Kp2 = 2; while (Kp2 < Kp) Kp2 <<= 1;
+    {
+        int warps = 4;
+        size_t smem = (size_t)warps * Kp2 * sizeof(int);
+        CREATE_TRY(cudaFuncSetAttribute(k_fill_neighbors, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int64_t blocks = std::min<int64_t>((N + warps - 1) / warps, (int64_t)sim->sm_count * 16);
+        k_fill_neighbors<<<(unsigned)blocks, warps * 32, smem, st>>>(N, gp.g, gp.cut2, Kp, Kp2, sim->pos,
+                                                                      (int*)(base + L.cell_start), (int*)(base + L.items), sim->nbr);
+        LAUNCHED();
+    }
+    // A2 weights
+    {
+        int64_t tot = N * (int64_t)Kp;
+        k_weights<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(N, Kp, p->alpha, sim->pos, sim->cs, sim->nbr, sim->w, sim->wT);
+        LAUNCHED();
+    }
+    sim->relax_smem = (size_t)nblk * 12 + (size_t)(Kp + 1) * 4 + 16;
+    CREATE_TRY(cudaFuncSetAttribute(k_relax, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
+    int hflags = 0;
+    CREATE_TRY(cudaMemcpyAsync(&hflags, scr + 8, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CREATE_TRY(cudaStreamSynchronize(st));
+    CREATE_TRY(cudaGetLastError());
+#undef CREATE_TRY
+    if (hflags & 1) { fs_destroy(sim); return fail(FS_ERR_ARG, "hc must be finite and > 0, angle finite"); }
+    sim->fields_dirty = true;
+    *out = sim;
+    return FS_OK;
+}
+
+int fs_create(fs_sim** out, int64_t N, const double* pos_dev, const double* angle_dev, const double* hc_dev,
+              const fs_params* p, void* workspace_dev, size_t workspace_bytes, void* stream) {
+    return fs_create_ensemble(out, N, 1, pos_dev, angle_dev, hc_dev, p, workspace_dev, workspace_bytes, stream);
+}
+
+int fs_destroy(fs_sim* sim) {
+    if (!sim) return FS_OK;
+    if (sim->hext_host) cudaFreeHost(sim->hext_host);
+    if (sim->ctr_host) cudaFreeHost(sim->ctr_host);
+    delete sim;
+    return FS_OK;
+}
+
+int fs_get_info(const fs_sim* sim, int64_t* N, int32_t* R, int32_t* K, int64_t* n_interactions) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (N) *N = sim->N;
+    if (R) *R = sim->R;
+    if (K) *K = sim->K;
+    if (n_interactions) *n_interactions = sim->n_inter;
+    return FS_OK;
+}
+
+int fs_set_spins(fs_sim* sim, const int8_t* s_dev) {
+    if (!sim || !s_dev) return fail(FS_ERR_ARG, "null pointer");
+    CUDA_TRY(cudaMemcpyAsync(sim->s, s_dev, (size_t)sim->R * sim->N, cudaMemcpyDeviceToDevice, sim->stream));
+    sim->fields_dirty = true;
+    return FS_OK;
+}
+
+int fs_get_spins(fs_sim* sim, int8_t* s_dev_out) {
+    if (!sim || !s_dev_out) return fail(FS_ERR_ARG, "null pointer");
+    CUDA_TRY(cudaMemcpyAsync(s_dev_out, sim->s, (size_t)sim->R * sim->N, cudaMemcpyDeviceToDevice, sim->stream));
+    return FS_OK;
+}
+
+int fs_set_thermal(fs_sim* sim, double sigma_th, uint64_t seed) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (!(sigma_th >= 0.0)) return fail(FS_ERR_ARG, "sigma_th must be >= 0");
+    sim->sigma = sigma_th; sim->seed = seed;
+    return FS_OK;
+}
+
+int fs_set_field(fs_sim* sim, double hx, double hy, uint32_t step) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    sim->step = step;
+    k_set_field<<<(sim->R + 127) / 128, 128, 0, sim->stream>>>(sim->R, hx, hy, sim->hext); LAUNCHED();   // by value: no host sync
+    CUDA_TRY(cudaGetLastError());
+    return FS_OK;
+}
+
+int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step) {
+    if (!sim || !h_host) return fail(FS_ERR_ARG, "null pointer");
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    for (int r = 0; r < sim->R; ++r) sim->hext_host[r] = make_double2(h_host[2 * r], h_host[2 * r + 1]);
+    sim->step = step;
+    return push_field(sim);
+}
+
+int fs_set_gather_variant(fs_sim* sim, int variant) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (variant < 0 || variant > 2) return fail(FS_ERR_ARG, "unknown gather variant %d", variant);
+    sim->gather_variant = variant;
+    return FS_OK;
+}
+
+int fs_update_fields(fs_sim* sim) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    return do_gather(sim);
+}
+
+int fs_scan_ensemble(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, double* best_L) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    int rc = do_scan(sim, true);
+    if (rc) return rc;
+    k_scan_finalize<<<sim->R, 256, 0, sim->stream>>>(sim->nblk, sim->bval, sim->bidx, sim->ctr); LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    if (!n_switchable && !best_index && !best_L) return FS_OK;
+    rc = fetch_counters(sim);
+    if (rc) return rc;
+    for (int r = 0; r < sim->R; ++r) {
+        if (n_switchable) n_switchable[r] = sim->ctr_host[r].n_switchable;
+        if (best_index) best_index[r] = sim->ctr_host[r].best_index;
+        if (best_L) best_L[r] = sim->ctr_host[r].best_L;
+    }
+    return FS_OK;
+}
+
+int fs_scan(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, double* best_L) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (sim->R == 1) return fs_scan_ensemble(sim, n_switchable, best_index, best_L);
+    int rc = fs_scan_ensemble(sim, nullptr, nullptr, nullptr);
+    if (rc) return rc;
+    if (!n_switchable && !best_index && !best_L) return FS_OK;
+    rc = fetch_counters(sim);
+    if (rc) return rc;
+    if (n_switchable) *n_switchable = sim->ctr_host[0].n_switchable;
+    if (best_index) *best_index = sim->ctr_host[0].best_index;
+    if (best_L) *best_L = sim->ctr_host[0].best_L;
+    return FS_OK;
+}
+
+int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    int rc = do_relax(sim, max_flips);
+    if (rc) return rc;
+    if (!n_flips_out) return FS_OK;
+    rc = fetch_counters(sim);
+    if (rc) return rc;
+    int capped = 0;
+    for (int r = 0; r < sim->R; ++r) { n_flips_out[r] = sim->ctr_host[r].last_flips; capped |= sim->ctr_host[r].status; }
+    return capped ? fail(FS_ERR_MAXFLIPS, "relax stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
+}
+
+int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    int rc = do_relax(sim, max_flips);
+    if (rc) return rc;
+    if (!n_flips_out) return FS_OK;
+    rc = fetch_counters(sim);
+    if (rc) return rc;
+    int64_t tot = 0; int capped = 0;
+    for (int r = 0; r < sim->R; ++r) { tot += sim->ctr_host[r].last_flips; capped |= sim->ctr_host[r].status; }
+    *n_flips_out = tot;
+    return capped ? fail(FS_ERR_MAXFLIPS, "relax stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
+}
+
+int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    int rc = fetch_counters(sim);
+    if (rc) return rc;
+    for (int r = 0; r < sim->R; ++r) {
+        if (total_flips) total_flips[r] = sim->ctr_host[r].total_flips;
+        if (last_relax_flips) last_relax_flips[r] = sim->ctr_host[r].last_flips;
+    }
+    if (reset) CUDA_TRY(cudaMemsetAsync(sim->ctr, 0, sizeof(Counters) * sim->R, sim->stream));
+    return FS_OK;
+}
+
+int fs_get_fields(fs_sim* sim, int which, double* h_dev_out) {
+    if (!sim || !h_dev_out) return fail(FS_ERR_ARG, "null pointer");
+    if (which < 0 || which > 3) return fail(FS_ERR_ARG, "unknown field selector %d", which);
+    if (which == FS_FIELD_TOTAL || which == FS_FIELD_DIP) { int rc = ensure_fields(sim); if (rc) return rc; }
+    dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
+    FieldSpec fsp{sim->sigma, sim->seed, sim->step};
+    k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, which, fsp, sim->hext, sim->cs, sim->hdip, (double2*)h_dev_out);
+    LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    return FS_OK;
+}
+
+int fs_get_flip_log(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out) {
+    if (!sim || !n_out) return fail(FS_ERR_ARG, "null pointer");
+    if (replica < 0 || replica >= sim->R) return fail(FS_ERR_ARG, "replica out of range");
+    int rc = fetch_counters(sim);
+    if (rc) return rc;
+    int64_t n = sim->ctr_host[replica].last_flips;
+    *n_out = n;
+    int64_t ncopy = std::min(std::min(n, cap), sim->log_cap);
+    if (ncopy > 0) {
+        if (!idx_dev_out) return fail(FS_ERR_ARG, "null output buffer");
+        CUDA_TRY(cudaMemcpyAsync(idx_dev_out, sim->flog + (int64_t)replica * sim->log_cap, 4 * (size_t)ncopy,
+                                 cudaMemcpyDeviceToDevice, sim->stream));
+    }
+    return FS_OK;
+}
+
+int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (K_out) *K_out = sim->K;
+    if (idx_dev_out && sim->K > 0)
+        CUDA_TRY(cudaMemcpy2DAsync(idx_dev_out, 4 * (size_t)sim->K, sim->nbr, 4 * (size_t)sim->Kp, 4 * (size_t)sim->K,
+                                   (size_t)sim->N, cudaMemcpyDeviceToDevice, sim->stream));
+    return FS_OK;
+}
+
+int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t* n_switchable, int64_t* best_index,
+                 double* best_L) {
+    if (!sim || !s_host || !h_host_out) return fail(FS_ERR_ARG, "null pointer");
+    size_t rn = (size_t)sim->R * sim->N;
+    CUDA_TRY(cudaMemcpyAsync(sim->s, s_host, rn, cudaMemcpyHostToDevice, sim->stream));
+    sim->fields_dirty = true;
+    int rc = do_gather(sim);
+    if (rc) return rc;
+    rc = fs_scan_ensemble(sim, nullptr, nullptr, nullptr);
+    if (rc) return rc;
+    // total field into hfix's sibling buffer M is not large enough; reuse hfix (rewritten by the next scan)
+    dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
+    FieldSpec fsp{sim->sigma, sim->seed, sim->step};
+    k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, FS_FIELD_TOTAL, fsp, sim->hext, sim->cs, sim->hdip, sim->hfix);
+    LAUNCHED();
+    CUDA_TRY(cudaMemcpyAsync(h_host_out, sim->hfix, 16 * rn, cudaMemcpyDeviceToHost, sim->stream));
+    rc = fetch_counters(sim);
+    if (rc) return rc;
+    if (n_switchable) *n_switchable = sim->ctr_host[0].n_switchable;
+    if (best_index) *best_index = sim->ctr_host[0].best_index;
+    if (best_L) *best_L = sim->ctr_host[0].best_L;
+    return FS_OK;
+}
+
+int fs_relax_host(fs_sim* sim, double hx, double hy, uint32_t step, int8_t* s_host_out, int64_t* n_flips_out) {
+    if (!sim || !s_host_out) return fail(FS_ERR_ARG, "null pointer");
+    int rc = fs_set_field(sim, hx, hy, step);
+    if (rc) return rc;
+    rc = do_relax(sim, 0);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(s_host_out, sim->s, (size_t)sim->R * sim->N, cudaMemcpyDeviceToHost, sim->stream));
+    rc = fetch_counters(sim);
+    if (rc) return rc;
+    if (n_flips_out) {
+        int64_t tot = 0;
+        for (int r = 0; r < sim->R; ++r) tot += sim->ctr_host[r].last_flips;
+        *n_flips_out = tot;
+    }
+    return FS_OK;
+}
+
+}  // extern "C"

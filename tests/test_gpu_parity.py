@@ -1,0 +1,243 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Bars (BASELINE.json north_star): spins / flip order / flip counts / neighbour tables
+bit-exact; fp64 fields within 1e-12 relative to max|h|."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2002_11401_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FIELD_TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2002_11401_b200 import binding
+    return binding
+
+
+def mk(B, w, spins=None):
+    from oracle import Oracle
+    sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+    orc = Oracle(w.pos, w.angle, w.hc, w.params, spins=w.spins if spins is None else spins)
+    sim.set_spins(w.spins if spins is None else spins)
+    if w.sigma_th:
+        sim.set_thermal(w.sigma_th, w.thermal_seed); orc.set_thermal(w.sigma_th, w.thermal_seed)
+    return sim, orc
+
+
+def field_err(hg, ho):
+    return np.abs(hg - ho).max() / max(np.abs(ho).max(), 1e-300)
+
+
+def run_parity(B, w, stride=1, tier="B", check_fields_every=0):
+    sim, orc = mk(B, w)
+    total = 0
+    steps = list(enumerate(w.fields))[::stride]
+    for n_done, (t, (hx, hy)) in enumerate(steps):
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        n = sim.relax()
+        no, log = getattr(orc, "relax_" + tier)()
+        assert n == no, (t, n, no)
+        if n:
+            glog = sim.get_flip_log().cpu().numpy()
+            assert np.array_equal(glog, log), f"flip order differs at step {t}"
+        total += n
+        if check_fields_every and n_done % check_fields_every == 0:
+            assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    assert field_err(sim.get_fields(1).cpu().numpy(), orc.fields(1)) < FIELD_TOL
+    ev, gap, thr = orc.monitor()
+    assert ev == 0, "oracle recorded a near-tie: flip order not well posed on this input"
+    assert sim.scan()[0] == 0 and orc.scan()[0] == 0
+    return total, sim, orc
+
+
+# ------------------------------------------------------------------ A1/A2: neighbour tables, couplings
+@pytest.mark.parametrize("which,scale", [("1", None), ("2", 12), ("3", 14), ("5", 24)])
+def test_neighbor_tables_bit_exact(B, which, scale):
+    from oracle import Oracle
+    w = W.config(which, scale=scale)
+    sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+    orc = Oracle(w.pos, w.angle, w.hc, w.params)
+    ref = orc.neighbors()
+    got = sim.get_neighbors().cpu().numpy()
+    assert sim.K == ref.shape[1] and sim.n_interactions == orc.num_interactions
+    assert np.array_equal(got, ref)
+
+
+def test_config2_full_neighbor_count(B):
+    w = W.config("2")
+    sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+    assert (sim.N, sim.K, sim.n_interactions) == (7699, 14, 105476)
+
+
+# ------------------------------------------------------------------ A3: full gather
+@pytest.mark.parametrize("which,scale", [("1", None), ("2", 20), ("3", 30), ("4", 40), ("5", 40)])
+def test_full_gather_fields(B, which, scale):
+    w = W.config(which, scale=scale)
+    spins = W.random_spins(w.N, seed=11)
+    sim, orc = mk(B, w, spins=spins)
+    hx, hy = w.fields[len(w.fields) // 3]
+    sim.set_field(hx, hy, 3); orc.set_field(hx, hy, 3)
+    sim.update_fields()
+    for which_f in (0, 1, 2, 3):
+        hg = sim.get_fields(which_f).cpu().numpy(); ho = orc.fields(which_f)
+        scale_ref = max(np.abs(ho).max(), 1e-300)
+        assert np.abs(hg - ho).max() / scale_ref < FIELD_TOL if np.abs(ho).max() > 0 else np.abs(hg).max() == 0
+
+
+# ------------------------------------------------------------------ A6/A7: scan
+@pytest.mark.parametrize("which,scale", [("1", None), ("3", 20), ("4", 30), ("5", 30)])
+def test_scan_candidates_and_argmax(B, which, scale):
+    w = W.config(which, scale=scale)
+    spins = W.random_spins(w.N, seed=5)
+    sim, orc = mk(B, w, spins=spins)
+    for t in (0, len(w.fields) // 4, len(w.fields) // 2):
+        t = min(t, len(w.fields) - 1)
+        hx, hy = w.fields[t]
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        n, best, L = sim.scan()
+        no, besto, Lo = orc.scan()
+        assert (n, best) == (no, besto)
+        if no:
+            assert abs(L - Lo) <= 1e-12 * abs(Lo)
+
+
+# ------------------------------------------------------------------ A7-A9: relaxation, flip order bit-exact
+def test_config1_full_protocol_bit_exact(B):
+    w = W.config("1")
+    total, sim, orc = run_parity(B, w, tier="A", check_fields_every=100)
+    assert total == 2 * w.N
+
+
+def test_config2_kagome_protocol(B):
+    w = W.config("2", scale=16)
+    total, _, _ = run_parity(B, w, stride=4)
+    assert total > w.N
+
+
+def test_config3_pinwheel_protocol(B):
+    w = W.config("3", scale=24)
+    total, _, _ = run_parity(B, w, stride=8)
+    assert total > w.N // 2
+
+
+def test_config4_thermal_protocol(B):
+    w = W.config("4", scale=60)           # 7320 spins: several leaf blocks and a ragged tail
+    total, _, _ = run_parity(B, w, stride=2)
+    assert total >= w.N
+
+
+def test_exact_ties_lowest_index(B):
+    pos, ang = W.ising(40, 1)
+    p = dict(alpha=0.0, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    sim = B.Sim(pos, ang, np.full(40, 0.1), p)
+    sim.set_field(-0.2, 0.05, 0)
+    assert sim.relax() == 40
+    assert list(sim.get_flip_log().cpu().numpy()) == list(range(40))
+
+
+def test_max_flips_cap_and_resume(B):
+    w = W.config("1")
+    sim, orc = mk(B, w)
+    hx, hy = w.fields[250]
+    sim.set_field(hx, hy, 0); orc.set_field(hx, hy, 0)
+    n1 = sim.relax(max_flips=7)
+    l1 = sim.get_flip_log().cpu().numpy().copy()
+    n2 = sim.relax()
+    l2 = sim.get_flip_log().cpu().numpy()
+    no, log = orc.relax_B()
+    assert n1 == 7 and n1 + n2 == no and np.array_equal(np.concatenate([l1, l2]), log)
+
+
+def test_run_to_run_determinism(B):
+    w = W.config("4", scale=30)
+    outs = []
+    for _ in range(2):
+        sim, _ = mk(B, w)
+        logs = []
+        for t, (hx, hy) in enumerate(w.fields[::4]):
+            sim.set_field(hx, hy, t); sim.relax()
+            logs.append(sim.get_flip_log().cpu().numpy().copy())
+        outs.append((np.concatenate(logs), sim.get_fields(0).cpu().numpy()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+# ------------------------------------------------------------------ A10: ensembles
+def test_ensemble_matches_independent_oracles(B):
+    from oracle import Oracle
+    w = W.config("1")
+    R = 5
+    hc = W.coercive_fields(w.N, seed=100, replicas=R)
+    sim = B.Sim(w.pos, w.angle, hc, w.params)
+    sim.set_thermal(0.005, 42)
+    orcs = [Oracle(w.pos, w.angle, hc[r], w.params, spins=w.spins) for r in range(R)]
+    for r, o in enumerate(orcs):
+        o.set_thermal(0.005, 42 + r)
+    for t, (hx, hy) in enumerate(w.fields[::25]):
+        sim.set_field(hx, hy, t)
+        n = sim.relax_ensemble()
+        for r, o in enumerate(orcs):
+            o.set_field(hx, hy, t)
+            no, log = o.relax_B()
+            assert n[r] == no
+            assert np.array_equal(sim.get_flip_log(replica=r).cpu().numpy(), log)
+    s = sim.get_spins().cpu().numpy()
+    h = sim.get_fields(0).cpu().numpy()
+    for r, o in enumerate(orcs):
+        assert np.array_equal(s[r], o.spins())
+        assert field_err(h[r], o.fields(0)) < FIELD_TOL
+
+
+# ------------------------------------------------------------------ edge cases / errors
+def test_single_spin_and_no_neighbors(B):
+    p = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    sim = B.Sim(np.array([[0.0, 0.0]]), np.array([0.0]), np.array([0.2]), p)
+    assert sim.K == 0 and sim.n_interactions == 0
+    sim.set_field(-0.3, 0.0, 0)
+    assert sim.relax() == 1 and sim.get_spins().cpu().numpy()[0] == -1
+    assert sim.relax() == 0
+    # well separated spins: no neighbours at all
+    pos = np.stack([np.arange(10) * 5.0, np.zeros(10)], 1)
+    sim = B.Sim(pos, np.zeros(10), np.full(10, 0.2), p)
+    assert sim.K == 0
+    assert np.abs(sim.get_fields(1).cpu().numpy()).max() == 0
+
+
+def test_errors(B):
+    p = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    pos = np.array([[0.0, 0.0], [0.0, 0.0]])
+    with pytest.raises(B.FlatspinError) as e:
+        B.Sim(pos, np.zeros(2), np.full(2, 0.2), p)
+    assert e.value.code == B.FS_ERR_COINCIDENT
+    with pytest.raises(B.FlatspinError) as e:
+        B.Sim(np.array([[0.0, 0.0], [1.0, 0.0]]), np.zeros(2), np.array([0.2, -0.1]), p)
+    assert e.value.code == B.FS_ERR_ARG
+
+
+def test_host_buffer_entry_points(B):
+    import torch
+    w = W.config("5", scale=20)
+    sim, orc = mk(B, w)
+    hx, hy = w.fields[0]
+    sim.set_field(hx, hy, 0); orc.set_field(hx, hy, 0)
+    s_host = torch.as_tensor(w.spins).pin_memory()
+    h_host = torch.empty((w.N, 2), dtype=torch.float64).pin_memory()
+    n, best, L = sim.step_host(s_host, h_host)
+    assert (n, best) == orc.scan()[:2]
+    assert field_err(h_host.numpy(), orc.fields(0)) < FIELD_TOL
+    w1 = W.config("1")
+    sim, orc = mk(B, w1)
+    s_out = torch.empty(w1.N, dtype=torch.int8).pin_memory()
+    hx, hy = w1.fields[250]
+    orc.set_field(hx, hy, 250)
+    assert sim.relax_host(hx, hy, 250, s_out) == orc.relax_B()[0]
+    assert np.array_equal(s_out.numpy(), orc.spins())
