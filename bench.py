@@ -197,38 +197,51 @@ def run_ours(args, rank, world, local_rank):
     t0 = time.perf_counter()
     sim = B.Sim(w.pos, w.angle, w.hc, w.params, device=dev)
     torch.cuda.synchronize(); t_create = time.perf_counter() - t0
+    lat = sim.lattice()
     sim.set_gather_variant(args.gather)
+    use_stencil = lat["active"] and args.gather != B.GATHER_ELL_F64
     sim.set_spins(w.spins)
     hx, hy = w.fields[0]
     sim.set_field(hx, hy, 0)
     I, N, K = sim.n_interactions, sim.N, sim.K
-    bytes_per_inter = 20.0 if args.gather != B.GATHER_ELL_DICT else 6.0
-    alg_bytes = I * bytes_per_inter + N * 17.0      # idx+weights per interaction; s read + h_dip written per spin
+    ell_bytes = I * 20.0 + N * 17.0     # idx + weight pair per interaction; s read + h_dip written per spin
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > L2 (126 MB)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
+    def timed_steps(n):
+        """n steps of (gather, scan); L2 flushed (untimed) before every step.  Returns per-step ms of the
+        whole step and of the gather kernel, from CUDA events on the launching stream."""
+        e = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n)]
+        for k in range(n):
+            flush.fill_(k & 0xff)
+            e[k][0].record(); sim.update_fields(); e[k][1].record(); sim.scan_async(); e[k][2].record()
+        barrier()
+        return (np.array([a.elapsed_time(c) for a, b, c in e]), np.array([a.elapsed_time(b) for a, b, c in e]))
+
     for _ in range(max(args.warmup, 3)):
         sim.update_fields(); sim.scan_async()
     barrier()
     sampler = ClockSampler(local_rank); sampler.start()
-    g0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    g1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = B.kernel_launches()
-    e0.record()
-    for k in range(args.steps):
-        g0[k].record(); sim.update_fields(); g1[k].record()
-        sim.scan_async()
-    e1.record()
-    barrier()
+    step_ms, g_ms = timed_steps(args.steps)
     clocks = sampler.stop()
     launches = B.kernel_launches() - l0
-    ms = e0.elapsed_time(e1)
-    gather_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(g0, g1)]))
+    ms = float(step_ms.sum())
+    gather_ms = float(g_ms.mean())
     n_sw, best, bestL = sim.scan()
+    ell = None
+    if use_stencil and not args.no_ell:
+        # the general-geometry ELL gather on the same workload, for the HBM roofline (inputs 6.2 GB > L2)
+        sim.set_gather_variant(B.GATHER_ELL_F64)
+        for _ in range(3):
+            sim.update_fields()
+        _, eg = timed_steps(min(args.steps, 10))
+        sim.set_gather_variant(args.gather)
+        ell = float(eg.mean())
 
     # end to end through the host-buffer C-ABI call: H2D spins + gather + scan + D2H fields every step
     s_host = torch.as_tensor(w.spins).pin_memory()
@@ -250,27 +263,45 @@ def run_ours(args, rank, world, local_rank):
     e2e_value = world * I * args.steps / (e2e_ms * 1e-3)
 
     peak, peak_src = measured_peaks()
-    achieved = alg_bytes / (gather_ms * 1e-3) / 1e9
+    if use_stencil:
+        dfma_peak = B.measure_fp64_peak()                     # DFMA/s, measured in this run
+        achieved = 2.0 * 2.0 * I / (gather_ms * 1e-3) / 1e12    # 2 DFMA (4 flop) per interaction
+        roofline = {"bound": "alu", "kernel": "k_gather_stencil", "achieved": achieved, "peak": 2.0 * dfma_peak / 1e12,
+                    "unit": "TFLOP/s", "frac": achieved / (2.0 * dfma_peak / 1e12), "traffic": None,
+                    "peak_source": "fp64 DFMA-chain kernel (fs_measure_fp64_peak) measured in this run; "
+                                   "nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2 TFLOP/s",
+                    "algorithmic_flops_per_launch": 4.0 * I, "kernel_ms": gather_ms,
+                    "share_of_step": gather_ms / (ms / args.steps)}
+    else:
+        achieved = ell_bytes / (gather_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "k_gather", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": ell_bytes, "kernel_ms": gather_ms,
+                    "share_of_step": gather_ms / (ms / args.steps)}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "N": N, "K": K, "interactions": I, "neighbor_distance": w.params["neighbor_distance"],
-                   "step": "fs_update_fields + fs_scan", "gather_variant": int(args.gather),
-                   "l2": "inputs larger than L2 (ELL tables %.1f GB per step), no flush" % (alg_bytes / 1e9),
+                   "step": "fs_update_fields + fs_scan", "gather": "lattice stencil" if use_stencil else "ELL fp64",
+                   "lattice": lat,
+                   "l2": "flushed before every timed step (256 MiB fill, untimed); step time = sum of per-step CUDA-event intervals",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "create_s": t_create,
                    "n_switchable": n_sw, "best_index": best},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(N), "d2h_bytes_per_step": int(16 * N + 24),
                 "ms_per_step": e2e_ms / args.steps, "call": "fs_step_host (pinned host spins in, host total fields out)"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": "k_gather", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": gather_ms,
-                     "share_of_step": gather_ms / (ms / args.steps)},
+        "roofline": roofline,
         "paper_context": {"v100_field_calcs_per_s": 1e8, "v100_interactions_per_s": 8e8,
                           "source": "PAPER.md:274-282, Tesla V100, 8-neighbourhood; other hardware, context only"},
     }
+    if ell is not None:
+        a = ell_bytes / (ell * 1e-3) / 1e9
+        line["roofline_ell"] = {"bound": "hbm", "kernel": "k_gather (general-geometry ELL path, same workload)",
+                                "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak, "traffic": None,
+                                "peak_source": peak_src, "algorithmic_bytes_per_launch": ell_bytes, "kernel_ms": ell,
+                                "interactions_per_s": I / (ell * 1e-3)}
     sim.close()
     if rank == 0 and not args.no_cpu:
         v, n_sp, n_int, dt = oracle_field_sample(w, budget_s=args.cpu_budget)
@@ -296,7 +327,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--gather", type=int, default=0, help="FS_GATHER_* variant (0 auto, 1 fp64 ELL, 2 dictionary ELL)")
+    ap.add_argument("--gather", type=int, default=0, help="FS_GATHER_* variant (0 auto, 1 ELL fp64, 2 lattice stencil)")
+    ap.add_argument("--no-ell", action="store_true", help="skip the side measurement of the ELL gather")
     ap.add_argument("--scale", type=int, default=None, help="debug: lattice size override for config 5")
     ap.add_argument("--relax-scale", type=int, default=None, help="debug: lattice size override for config 4")
     ap.add_argument("--no-relax", action="store_true")

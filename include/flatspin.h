@@ -12,6 +12,8 @@
  *   - Every DEVICE pointer is caller-owned CUDA global memory (a torch tensor's data_ptr()).  Inputs
  *     of fs_create* are consumed during the call and may be freed afterwards.  The workspace is
  *     caller-owned and must outlive the handle.  Outputs are written to caller-owned buffers.
+ *     The only library-owned device memory is the lattice-stencil table set (index grids of <= 8N
+ *     cells + a few KB of couplings), allocated by fs_create and freed by fs_destroy.
  *   - HOST pointers to scalars (n_flips_out ...) are written after a stream synchronise; passing NULL
  *     skips the synchronise (the call is then fully asynchronous on `stream`).
  *   - All work is enqueued on the stream given at creation (a cudaStream_t passed as void*; NULL =
@@ -58,10 +60,25 @@ enum {
 enum { FS_FIELD_TOTAL = 0, FS_FIELD_DIP = 1, FS_FIELD_EXT = 2, FS_FIELD_THERMAL = 3 };
 
 /* Gather kernel variants for fs_update_fields:
- *   0 = auto, 1 = ELL with fp64 weight pairs streamed from HBM (20 B / interaction),
- *   2 = ELL with 16-bit ids into a shared-memory table of unique weight pairs, the per-sublattice
- *       stencil table (6 B / interaction); falls back to 1 if the geometry has > 65535 unique pairs. */
-enum { FS_GATHER_AUTO = 0, FS_GATHER_ELL_F64 = 1, FS_GATHER_ELL_DICT = 2 };
+ *   0 = auto: the lattice stencil when the geometry was detected to be a regular lattice, else ELL;
+ *   1 = ELL: neighbour indices + fp64 coupling pairs streamed from HBM (20 B / interaction; HBM-bound);
+ *   2 = lattice stencil: dense per-sublattice spin grids correlated with the table
+ *       T[sub_i][sub_j][du][dv] = alpha*g_ij held in shared memory (no per-interaction HBM traffic;
+ *       FP64-pipe bound).  FS_ERR_ARG if the geometry is not a verified regular lattice. */
+enum { FS_GATHER_AUTO = 0, FS_GATHER_ELL_F64 = 1, FS_GATHER_STENCIL = 2 };
+
+/* Why the stencil is not available (fs_get_lattice info[1]); 0 = it is. */
+enum {
+    FS_LATTICE_OK = 0,
+    FS_LATTICE_NO_NEIGHBORS = 1,          /* K == 0: nothing to gather */
+    FS_LATTICE_NO_BASIS = 2,              /* no two lattice vectors found around the reference spin */
+    FS_LATTICE_TOO_MANY_SUBLATTICES = 3,  /* more than 8 */
+    FS_LATTICE_NOT_PERIODIC = 4,          /* spins off the lattice, or two spins in one cell */
+    FS_LATTICE_STENCIL_TOO_WIDE = 5,      /* half-extent > 40 cells or shared memory exceeded */
+    FS_LATTICE_TOO_SPARSE = 6,            /* dense grids would exceed 8N + 2^20 cells */
+    FS_LATTICE_REACH_MISMATCH = 7,        /* stencil would reach a different set of pairs than the ELL */
+    FS_LATTICE_WEIGHT_MISMATCH = 8        /* couplings of equal offsets differ by more than 2e-13/K relative */
+};
 
 /* Bytes of workspace fs_create[_ensemble] needs for this geometry (runs the cell-grid neighbour count,
  * PAPER.md:57, to find the maximum degree K).  pos_dev: DEVICE [N,2] row-major fp64.
@@ -103,6 +120,17 @@ int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step);
 
 /* Choose the gather kernel variant (FS_GATHER_*).  Default auto. */
 int fs_set_gather_variant(fs_sim* sim, int variant);
+
+/* Result of the regular-lattice detection run by fs_create (flatspin geometries are
+ * lattices with 1-3 sublattices, :146).  info HOST [10] int32: {stencil active, FS_LATTICE_* reason,
+ * sublattices, U, V (cells along the two lattice vectors), Ru, Rv (stencil half-extents), stencil
+ * slots present, warps per CTA, shared-memory bytes per CTA}.  dinfo HOST [2]: {max |w_ELL - T| over
+ * all interactions, max |w|}.  Either may be NULL.  No synchronise. */
+int fs_get_lattice(const fs_sim* sim, int32_t* info, double* dinfo);
+
+/* Calibration for the FP64 roofline: runs a chain of dependent-free DFMAs on every SM and
+ * returns the best of 4 timed launches in DFMA/s (HOST).  Synchronises `stream`. */
+int fs_measure_fp64_peak(double* dfma_per_s, void* stream);
 
 /* Full dipolar-field gather h_dip,i = sum_k s[nbr[i][k]] * w[i][k] for every spin (Eq. 3 over the
  * neighbourhood).  Asynchronous. */

@@ -16,14 +16,14 @@ from . import build as _build
 
 FS_OK, FS_ERR_ARG, FS_ERR_COINCIDENT, FS_ERR_WORKSPACE, FS_ERR_CUDA, FS_ERR_MAXFLIPS = 0, -1, -2, -3, -4, -5
 FIELD_TOTAL, FIELD_DIP, FIELD_EXT, FIELD_THERMAL = 0, 1, 2, 3
-GATHER_AUTO, GATHER_ELL_F64, GATHER_ELL_DICT = 0, 1, 2
+GATHER_AUTO, GATHER_ELL_F64, GATHER_STENCIL = 0, 1, 2
 
 EXPORTS = [
     "fs_workspace_bytes", "fs_create", "fs_create_ensemble", "fs_destroy", "fs_get_info", "fs_set_spins",
     "fs_get_spins", "fs_set_thermal", "fs_set_field", "fs_set_field_ensemble", "fs_set_gather_variant",
     "fs_update_fields", "fs_scan", "fs_scan_ensemble", "fs_relax", "fs_relax_ensemble", "fs_get_counters",
     "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
-    "fs_kernel_launches", "fs_last_error",
+    "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak",
 ]
 
 
@@ -74,6 +74,8 @@ def load_library(path: str | None = None):
         "fs_relax_host": [vp, dbl, dbl, C.c_uint32, vp, P(i64)],
         "fs_kernel_launches": [],
         "fs_last_error": [],
+        "fs_get_lattice": [vp, vp, vp],
+        "fs_measure_fp64_peak": [P(dbl), vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -94,6 +96,15 @@ def _check(L, rc, allow=()):
 
 def kernel_launches() -> int:
     return int(load_library().fs_kernel_launches())
+
+
+def measure_fp64_peak(stream=None) -> float:
+    """DFMA/s of the DFMA-chain calibration kernel (the FP64 roofline denominator)."""
+    L = load_library()
+    v = C.c_double()
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    _check(L, L.fs_measure_fp64_peak(C.byref(v), sp))
+    return float(v.value)
 
 
 class Sim:
@@ -170,6 +181,14 @@ class Sim:
 
     def set_gather_variant(self, v):
         _check(self.L, self.L.fs_set_gather_variant(self.h, int(v)))
+
+    def lattice(self) -> dict:
+        info = np.zeros(10, np.int32); d = np.zeros(2, np.float64)
+        _check(self.L, self.L.fs_get_lattice(self.h, info.ctypes.data, d.ctypes.data))
+        keys = ("active", "reason", "nsub", "U", "V", "Ru", "Rv", "slots", "warps_per_cta", "smem_bytes")
+        out = {k: int(v) for k, v in zip(keys, info)}
+        out["active"] = bool(out["active"]); out["max_dev"] = float(d[0]); out["w_max"] = float(d[1])
+        return out
 
     # ---- compute
     def update_fields(self):

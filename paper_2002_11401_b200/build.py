@@ -22,7 +22,8 @@ def nvcc_path() -> str:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    newest = max(os.path.getmtime(SRC), os.path.getmtime(HDR))
+    deps = [HDR] + [os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc"))]
+    newest = max(os.path.getmtime(f) for f in deps)
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
         cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
               ["-I", os.path.join(ROOT, "include"), SRC, "-o", LIB]

@@ -12,10 +12,11 @@
 //   k_gather<G>        A3  h_dip,i = sum_k s_j w_ij, G lanes cooperate per row
 //   k_scan             A4-A7 total field + Philox thermal + astroid + margin + leaf-block arg-max
 //                                                                             (Eqs. 2,5,6)
-//   k_scan_finalize    A7  top-level arg-max + switchable count (fs_scan)
+//                      (+ top-level arg-max and switchable count by the last CTA to finish, for fs_scan)
 //   k_relax            A7-A9 persistent single-CTA-per-replica relax loop with incremental updates
 //                                                                             (Eq. 3 linear in s_j)
 //   k_fields_out       fs_get_fields
+//   lattice.cuh        lattice detection + stencil tables + k_gather_stencil (A3, FP64-bound variant)
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
@@ -26,6 +27,8 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <algorithm>
+#include <vector>
 
 #include "flatspin.h"
 
@@ -63,7 +66,8 @@ struct Counters {            // one per replica, device resident
     long long best_index;
     double best_L;
     int status;              // 1 = stopped by max_flips
-    int pad;
+    unsigned int ticket;     // k_scan: CTAs of this replica that have finished (last one finalises)
+    unsigned long long acc_switch;   // k_scan: running count of switchable spins
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -124,6 +128,8 @@ __device__ __forceinline__ double margin(double hpar, double hperp, double s, do
     double y = fabs(hperp) * a.inv_c * ihc;
     return pow(x, a.e_par) + pow(y, a.e_perp);
 }
+
+#include "lattice.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // A0: frame tables + hc validation
@@ -391,7 +397,7 @@ __global__ void __launch_bounds__(256) k_gather(int64_t N, int Kp, const int* __
 // ------------------------------------------------------------------------------------------------
 struct FieldSpec { double sigma; uint64_t seed; uint32_t step; };
 
-__global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs,
+__global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs, int finalize,
                                                const double2* __restrict__ hext_all /*[R] (hx,hy)*/,
                                                const double2* __restrict__ cs, const double* __restrict__ hc_all,
                                                const int8_t* __restrict__ s_all, const double2* __restrict__ hdip_all,
@@ -400,6 +406,7 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
                                                Counters* __restrict__ ctr) {
     __shared__ double wv[32];
     __shared__ int wi[32];
+    __shared__ int is_last;
     int r = blockIdx.y;
     int64_t off = (int64_t)r * N;
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -408,17 +415,18 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
         double2 c = cs[i];
         double2 he = hext_all[r];
         double ex = he.x, ey = he.y;
+        double2 hf;
         if (fs.sigma != 0.0) {
             double2 t = thermal_xy(fs.sigma, fs.seed + (uint64_t)r, fs.step, (uint32_t)i);
             // (ext + th) rotated together would round differently from the paper's sum of three fields;
             // rotate separately and add (Eq. 2)
             double tp = t.x * c.x + t.y * c.y, tq = -t.x * c.y + t.y * c.x;
             double ep = ex * c.x + ey * c.y, eq = -ex * c.y + ey * c.x;
-            hfix_all[off + i] = make_double2(ep + tp, eq + tq);
+            hf = make_double2(ep + tp, eq + tq);
         } else {
-            hfix_all[off + i] = make_double2(ex * c.x + ey * c.y, -ex * c.y + ey * c.x);
+            hf = make_double2(ex * c.x + ey * c.y, -ex * c.y + ey * c.x);
         }
-        double2 hf = hfix_all[off + i];
+        hfix_all[off + i] = hf;
         double2 hd = hdip_all[off + i];
         m = margin(hd.x + hf.x, hd.y + hf.y, (double)s_all[off + i], hc_all[off + i], ast);
         M_all[off + i] = m;
@@ -441,33 +449,34 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
             if (blk < nblk) { bval_all[(int64_t)r * nblk + blk] = bv; bidx_all[(int64_t)r * nblk + blk] = bi; }
         }
     }
-    if (lane == 0 && nsw) atomicAdd((unsigned long long*)&ctr[r].n_switchable, nsw);
-}
-
-__global__ void k_scan_finalize(int nblk, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
-                                Counters* __restrict__ ctr) {
-    __shared__ double wv[32];
-    __shared__ int wi[32];
-    int r = blockIdx.x;
-    const double* bval = bval_all + (int64_t)r * nblk;
-    const int* bidx = bidx_all + (int64_t)r * nblk;
+    if (!finalize) return;
+    // A7 top level (fs_scan only): the last CTA of this replica to finish reduces the leaf maxima
+    if (lane == 0 && nsw) atomicAdd(&ctr[r].acc_switch, nsw);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) is_last = (atomicAdd(&ctr[r].ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    const volatile double* bval = bval_all + (int64_t)r * nblk;
+    const volatile int* bidx = bidx_all + (int64_t)r * nblk;
     double v = -CUDART_INF; int bi = 0x7fffffff;
-    for (int t = threadIdx.x; t < nblk; t += blockDim.x)
-        if (better(bval[t], bidx[t], v, bi)) { v = bval[t]; bi = bidx[t]; }
+    for (int t = threadIdx.x; t < nblk; t += blockDim.x) {
+        double tv = bval[t]; int ti = bidx[t];
+        if (better(tv, ti, v, bi)) { v = tv; bi = ti; }
+    }
     warp_argmax(v, bi);
-    if ((threadIdx.x & 31) == 0) { wv[threadIdx.x >> 5] = v; wi[threadIdx.x >> 5] = bi; }
+    __syncthreads();                                     // wv/wi are reused
+    if (lane == 0) { wv[w] = v; wi[w] = bi; }
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int k = 1; k < (int)(blockDim.x >> 5); ++k) if (better(wv[k], wi[k], v, bi)) { v = wv[k]; bi = wi[k]; }
         bool any = v > 1.0;
         ctr[r].best_index = any ? bi : -1;
         ctr[r].best_L = any ? v : -CUDART_INF;
+        ctr[r].n_switchable = (long long)atomicExch(&ctr[r].acc_switch, 0ull);
+        ctr[r].ticket = 0u;
     }
-}
-
-__global__ void k_reset_scan_counters(int R, Counters* ctr) {
-    int r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r < R) { ctr[r].n_switchable = 0; ctr[r].best_index = -1; ctr[r].best_L = -CUDART_INF; }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -643,6 +652,19 @@ struct fs_sim {
     Counters* ctr_host = nullptr;   // pinned staging [R]
     int gather_variant = FS_GATHER_AUTO;
     size_t relax_smem = 0;
+    // regular-lattice stencil (lattice.cuh); library-owned device memory, freed by fs_destroy
+    bool stencil_ok = false;
+    int stencil_reason = 0;         // why not (FS_LATTICE_* code), 0 = active
+    LatFrame lframe{};
+    LatGrid lg{};
+    void* lat_mem = nullptr;        // sub | cu | cv
+    void* st_mem = nullptr;         // gidx | T | owner | rowtab | scratch
+    uint8_t* lat_sub = nullptr; int *lat_cu = nullptr, *lat_cv = nullptr;
+    int8_t* sgrid = nullptr;
+    int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
+    int st_nw = 4; size_t st_smem = 0;
+    double st_maxdev = 0.0, st_wmax = 0.0;
+    long long st_slots = 0;         // stencil slots present (sum over sublattice pairs)
 };
 
 namespace {
@@ -775,7 +797,24 @@ void launch_gather_g(fs_sim* sim) {
     LAUNCHED();
 }
 
+int do_gather_stencil(fs_sim* sim) {
+    const LatGrid& g = sim->lg;
+    int TV = ST_OV * sim->st_nw;
+    dim3 grid((unsigned)((g.U + ST_TU - 1) / ST_TU), (unsigned)((g.V + TV - 1) / TV), (unsigned)(g.nsub * sim->R));
+    int64_t cells = (int64_t)g.nsub * g.Vp * g.Up;
+    k_spin_grid<<<(unsigned)((cells + 255) / 256), 256, 0, sim->stream>>>(sim->N, g, sim->R, sim->gidx, sim->s, sim->sgrid);
+    LAUNCHED();
+    k_gather_stencil<<<grid, 32 * sim->st_nw, sim->st_smem, sim->stream>>>(sim->N, g, sim->gidx, sim->sgrid, sim->T,
+                                                                            sim->rowtab, sim->hdip);
+    LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    sim->fields_dirty = false;
+    return FS_OK;
+}
+
 int do_gather(fs_sim* sim) {
+    bool stencil = sim->stencil_ok && sim->gather_variant != FS_GATHER_ELL_F64;
+    if (stencil) return do_gather_stencil(sim);
     int q = sim->Kp / 4;
     if (q <= 1) launch_gather_g<1>(sim);
     else if (q <= 2) launch_gather_g<2>(sim);
@@ -788,17 +827,202 @@ int do_gather(fs_sim* sim) {
     return FS_OK;
 }
 
+// ---- lattice detection (host logic + lattice.cuh kernels).  Never fails the creation: any problem
+// leaves sim->stencil_ok = false with a reason code and the ELL gather in charge.
+struct PickRow { double px, py, cx, cy; };
+
+__global__ void k_lat_pick(int i0, int Kp, const int* __restrict__ nbr, const double2* __restrict__ pos,
+                           const double2* __restrict__ cs, PickRow* __restrict__ out) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t > Kp) return;
+    int j = (t == Kp) ? i0 : nbr[(int64_t)i0 * Kp + t];
+    PickRow r{0, 0, 2, 2};                               // (2,2) marks padding
+    if (j >= 0) { double2 p = pos[j], c = cs[j]; r = PickRow{p.x, p.y, c.x, c.y}; }
+    out[t] = r;
+}
+
+int lattice_fail(fs_sim* sim, int reason) {
+    sim->stencil_ok = false; sim->stencil_reason = reason;
+    if (sim->st_mem) { cudaFree(sim->st_mem); sim->st_mem = nullptr; }
+    if (sim->lat_mem) { cudaFree(sim->lat_mem); sim->lat_mem = nullptr; }
+    cudaGetLastError();
+    return FS_OK;
+}
+
+int detect_lattice(fs_sim* sim) {
+    const int64_t N = sim->N; const int Kp = sim->Kp; cudaStream_t st = sim->stream;
+    if (sim->K <= 0) return lattice_fail(sim, FS_LATTICE_NO_NEIGHBORS);
+    // reference spin: lowest index among the spins of maximum degree (an interior spin)
+    std::vector<int> deg((size_t)N);
+    CUDA_TRY(cudaMemcpyAsync(deg.data(), sim->deg, 4 * (size_t)N, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    int i0 = 0;
+    for (int64_t i = 1; i < N; ++i) if (deg[i] > deg[i0]) i0 = (int)i;
+    // its neighbours' positions and orientations
+    PickRow* pick_dev = nullptr;
+    CUDA_TRY(cudaMalloc(&pick_dev, sizeof(PickRow) * (size_t)(Kp + 1)));
+    k_lat_pick<<<(Kp + 1 + 127) / 128, 128, 0, st>>>(i0, Kp, sim->nbr, sim->pos, sim->cs, pick_dev); LAUNCHED();
+    std::vector<PickRow> pick((size_t)Kp + 1);
+    cudaError_t e = cudaMemcpyAsync(pick.data(), pick_dev, sizeof(PickRow) * (size_t)(Kp + 1), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(pick_dev);
+    if (e != cudaSuccess) return fail(FS_ERR_CUDA, "lattice pick: %s", cudaGetErrorString(e));
+    const PickRow me = pick[Kp];
+    struct Nb { double dx, dy, cx, cy, len; };
+    std::vector<Nb> nb;
+    for (int t = 0; t < Kp; ++t)
+        if (pick[t].cx <= 1.5) {
+            double dx = pick[t].px - me.px, dy = pick[t].py - me.py;
+            nb.push_back(Nb{dx, dy, pick[t].cx, pick[t].cy, std::sqrt(dx * dx + dy * dy)});
+        }
+    std::sort(nb.begin(), nb.end(), [](const Nb& a, const Nb& b) { return a.len < b.len; });
+    // candidate lattice vectors: displacements to same-orientation neighbours, and differences of
+    // displacements between neighbours that share an orientation (nearest 64 only)
+    auto same = [](double ax, double ay, double bx, double by) { return std::fabs(ax - bx) < 1e-9 && std::fabs(ay - by) < 1e-9; };
+    struct Vec { double x, y, len, ang; };
+    std::vector<Vec> cand;
+    auto push = [&](double x, double y) {
+        double len = std::sqrt(x * x + y * y);
+        if (!(len > 1e-9)) return;
+        if (x < -1e-12 * len || (std::fabs(x) <= 1e-12 * len && y < 0)) { x = -x; y = -y; }   // half plane
+        cand.push_back(Vec{x, y, len, std::atan2(y, x)});
+    };
+    for (const Nb& a : nb) if (same(a.cx, a.cy, me.cx, me.cy)) push(a.dx, a.dy);
+    size_t near = std::min<size_t>(nb.size(), 64);
+    for (size_t a = 0; a < near; ++a)
+        for (size_t b = a + 1; b < near; ++b)
+            if (same(nb[a].cx, nb[a].cy, nb[b].cx, nb[b].cy)) push(nb[a].dx - nb[b].dx, nb[a].dy - nb[b].dy);
+    if (cand.empty()) return lattice_fail(sim, FS_LATTICE_NO_BASIS);
+    std::sort(cand.begin(), cand.end(), [](const Vec& a, const Vec& b) {
+        if (std::fabs(a.len - b.len) > 1e-9 * std::max(a.len, b.len)) return a.len < b.len;
+        return std::fabs(a.ang) < std::fabs(b.ang);     // among equals: closest to the +x axis (spin index order)
+    });
+    const Vec a1 = cand[0];
+    Vec a2{-a1.y, a1.x, a1.len, 0.0};                    // 1-D chains: any perpendicular
+    for (const Vec& c : cand) {
+        double cr = a1.x * c.y - a1.y * c.x;
+        if (std::fabs(cr) > 1e-6 * a1.len * c.len) { a2 = c; if (cr < 0) { a2.x = -c.x; a2.y = -c.y; } break; }
+    }
+    double det = a1.x * a2.y - a1.y * a2.x;
+    if (!(std::fabs(det) > 1e-12)) return lattice_fail(sim, FS_LATTICE_NO_BASIS);
+    sim->lframe = LatFrame{me.px, me.py, a2.y / det, -a2.x / det, -a1.y / det, a1.x / det};
+
+    // sublattices: one pass per sublattice
+    CUDA_TRY(cudaMalloc(&sim->lat_mem, align_up((size_t)N) + 2 * align_up(4 * (size_t)N) + 256));
+    unsigned char* lb = (unsigned char*)sim->lat_mem;
+    sim->lat_sub = lb; sim->lat_cu = (int*)(lb + align_up((size_t)N)); sim->lat_cv = (int*)(lb + align_up((size_t)N) + align_up(4 * (size_t)N));
+    int* scr = (int*)(lb + align_up((size_t)N) + 2 * align_up(4 * (size_t)N));      // 64 ints of scratch
+    CUDA_TRY(cudaMemsetAsync(sim->lat_sub, 0xff, (size_t)N, st));
+    const int nb256 = (int)((N + 255) / 256);
+    int nsub = 0, rep = i0;
+    for (;;) {
+        if (nsub == NSUB_MAX) return lattice_fail(sim, FS_LATTICE_TOO_MANY_SUBLATTICES);
+        int init[2] = {0x7fffffff, 0};
+        CUDA_TRY(cudaMemcpyAsync(scr, init, sizeof(init), cudaMemcpyHostToDevice, st));
+        k_lat_assign<<<nb256, 256, 0, st>>>(N, sim->lframe, rep, nsub, sim->pos, sim->cs, sim->lat_sub, sim->lat_cu,
+                                            sim->lat_cv, scr); LAUNCHED();
+        int res[2];
+        CUDA_TRY(cudaMemcpyAsync(res, scr, sizeof(res), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        ++nsub;
+        if (res[1] == 0) return lattice_fail(sim, FS_LATTICE_NOT_PERIODIC);       // representative did not match itself
+        if (res[0] == 0x7fffffff) break;
+        rep = res[0];
+    }
+    // extents
+    int ext_init[8] = {0x7fffffff, 0x7fffffff, (int)0x80000000, (int)0x80000000, 0, 0, 0, 0};
+    CUDA_TRY(cudaMemcpyAsync(scr, ext_init, sizeof(ext_init), cudaMemcpyHostToDevice, st));
+    unsigned long long* scr64 = (unsigned long long*)(scr + 8);                   // [0] wmax, [1] dev, [2] count
+    CUDA_TRY(cudaMemsetAsync(scr64, 0, 32, st));
+    const int64_t NK = N * (int64_t)Kp;
+    const unsigned nbk = (unsigned)((NK + 255) / 256);
+    k_lat_extent<<<nbk, 256, 0, st>>>(N, Kp, sim->nbr, sim->w, sim->lat_cu, sim->lat_cv, scr, scr64); LAUNCHED();
+    int ext[8]; unsigned long long wbits = 0;
+    CUDA_TRY(cudaMemcpyAsync(ext, scr, sizeof(ext), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(&wbits, scr64, 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    LatGrid g{};
+    g.nsub = nsub; g.u0 = ext[0]; g.v0 = ext[1];
+    int64_t U = (int64_t)ext[2] - ext[0] + 1, V = (int64_t)ext[3] - ext[1] + 1;
+    g.Ru = ext[4]; g.Rv = ext[5];
+    if (g.Ru > STENCIL_RMAX || g.Rv > STENCIL_RMAX) return lattice_fail(sim, FS_LATTICE_STENCIL_TOO_WIDE);
+    int64_t Up = U + 2 * g.Ru, Vp = V + 2 * g.Rv;
+    int64_t cells = (int64_t)nsub * Up * Vp;
+    if (U <= 0 || V <= 0 || cells > 8 * N + (1 << 20) || Up > (1 << 30) || Vp > (1 << 30))
+        return lattice_fail(sim, FS_LATTICE_TOO_SPARSE);
+    g.U = (int)U; g.V = (int)V; g.Up = (int)Up; g.Vp = (int)Vp; g.W = 2 * g.Ru + 1; g.H = 2 * g.Rv + 1;
+    std::memcpy(&sim->st_wmax, &wbits, 8);
+    // kernel shape: few warps per CTA when the stencil is wide (compute-bound: small tiles balance the
+    // SMs), many when it is narrow (staging-bound: large tiles amortise the halo)
+    int wh = g.W * g.H;
+    sim->st_nw = wh >= 100 ? 2 : (wh >= 25 ? 4 : 8);
+    const int pitch = ((ST_TU + 2 * g.Ru + 15) / 16) * 16;
+    for (;;) {
+        int TV = ST_OV * sim->st_nw;
+        sim->st_smem = 8 * (size_t)(TV + 2 * g.Rv) * pitch + 16 * (size_t)(wh + 1) + 8 * (size_t)g.W;
+        if (sim->st_smem <= 200 * 1024 || sim->st_nw == 1) break;
+        sim->st_nw >>= 1;
+    }
+    if (sim->st_smem > 200 * 1024) return lattice_fail(sim, FS_LATTICE_STENCIL_TOO_WIDE);
+    {
+        int TV = ST_OV * sim->st_nw;
+        g.Upa = (g.U + ST_TU - 1) / ST_TU * ST_TU - ST_TU + pitch;      // last tile's row of chunks stays in bounds
+        g.Vpa = (g.V + TV - 1) / TV * TV + 2 * g.Rv;
+    }
+    const size_t sg_bytes = (size_t)sim->R * nsub * g.Vpa * g.Upa;
+    // tables
+    size_t slots = (size_t)nsub * nsub * wh;
+    size_t o_gidx = 0, o_T = align_up(4 * (size_t)cells), o_owner = o_T + align_up(16 * slots),
+           o_rows = o_owner + align_up(8 * slots), o_sg = o_rows + align_up(8 * (size_t)nsub * nsub * g.W),
+           o_end = o_sg + align_up(sg_bytes);
+    CUDA_TRY(cudaMalloc(&sim->st_mem, o_end));
+    unsigned char* sb = (unsigned char*)sim->st_mem;
+    sim->gidx = (int*)(sb + o_gidx); sim->T = (double2*)(sb + o_T); sim->owner = (unsigned long long*)(sb + o_owner);
+    sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (int8_t*)(sb + o_sg);
+    CUDA_TRY(cudaMemsetAsync(sim->sgrid, 0, sg_bytes, st));
+    CUDA_TRY(cudaMemsetAsync(sim->gidx, 0xff, 4 * (size_t)cells, st));
+    CUDA_TRY(cudaMemsetAsync(sim->T, 0, 16 * slots, st));
+    CUDA_TRY(cudaMemsetAsync(sim->owner, 0xff, 8 * slots, st));
+    CUDA_TRY(cudaMemsetAsync(scr, 0, 4, st));                                      // flags
+    k_lat_scatter<<<nb256, 256, 0, st>>>(N, g, sim->lat_sub, sim->lat_cu, sim->lat_cv, sim->gidx, scr); LAUNCHED();
+    for (int mode = 0; mode < 3; ++mode) {
+        k_stencil_build<<<nbk, 256, 0, st>>>(mode, N, Kp, g, sim->nbr, sim->w, sim->lat_sub, sim->lat_cu, sim->lat_cv,
+                                             sim->owner, sim->T, scr64 + 1); LAUNCHED();
+    }
+    k_stencil_rows<<<(nsub * nsub * g.W + 127) / 128, 128, 0, st>>>(g, sim->owner, sim->rowtab); LAUNCHED();
+    k_stencil_count<<<nb256, 256, 0, st>>>(N, g, sim->lat_sub, sim->lat_cu, sim->lat_cv, sim->gidx, sim->owner, scr64 + 2); LAUNCHED();
+    int flags = 0; unsigned long long res64[3];
+    CUDA_TRY(cudaMemcpyAsync(&flags, scr, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(res64, scr64, 24, cudaMemcpyDeviceToHost, st));
+    std::vector<unsigned long long> own(slots);
+    CUDA_TRY(cudaMemcpyAsync(own.data(), sim->owner, 8 * slots, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaGetLastError());
+    std::memcpy(&sim->st_maxdev, &res64[1], 8);
+    sim->st_slots = 0;
+    for (unsigned long long o : own) sim->st_slots += (o != ~0ull);
+    if (flags & 4) return lattice_fail(sim, FS_LATTICE_NOT_PERIODIC);
+    if ((long long)res64[2] != (long long)sim->n_inter) return lattice_fail(sim, FS_LATTICE_REACH_MISMATCH);
+    if (!(sim->st_maxdev * (double)sim->K <= 2e-13 * sim->st_wmax)) return lattice_fail(sim, FS_LATTICE_WEIGHT_MISMATCH);
+    if (sim->st_smem > 48 * 1024)
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->st_smem));
+    sim->lg = g;
+    sim->stencil_ok = true; sim->stencil_reason = 0;
+    // the build-only arrays (sub, cu, cv) are no longer needed
+    cudaFree(sim->lat_mem); sim->lat_mem = nullptr; sim->lat_sub = nullptr; sim->lat_cu = sim->lat_cv = nullptr;
+    return FS_OK;
+}
+
 int ensure_fields(fs_sim* sim) { return sim->fields_dirty ? do_gather(sim) : FS_OK; }
 
-int do_scan(fs_sim* sim, bool count) {
+int do_scan(fs_sim* sim, bool finalize) {
     int rc = ensure_fields(sim);
     if (rc) return rc;
-    if (count) { k_reset_scan_counters<<<(sim->R + 127) / 128, 128, 0, sim->stream>>>(sim->R, sim->ctr); LAUNCHED(); }
     int threads = sim->LB > SCAN_THREADS ? sim->LB : SCAN_THREADS;
     dim3 grid((unsigned)((sim->N + threads - 1) / threads), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
-    k_scan<<<grid, threads, 0, sim->stream>>>(sim->N, sim->LB, sim->ast, fsp, sim->hext, sim->cs, sim->hc, sim->s,
-                                               sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->ctr);
+    k_scan<<<grid, threads, 0, sim->stream>>>(sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc,
+                                               sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->ctr);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -956,6 +1180,8 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     CREATE_TRY(cudaGetLastError());
 #undef CREATE_TRY
     if (hflags & 1) { fs_destroy(sim); return fail(FS_ERR_ARG, "hc must be finite and > 0, angle finite"); }
+    rc = detect_lattice(sim);
+    if (rc) { fs_destroy(sim); return rc; }
     sim->fields_dirty = true;
     *out = sim;
     return FS_OK;
@@ -970,6 +1196,8 @@ int fs_destroy(fs_sim* sim) {
     if (!sim) return FS_OK;
     if (sim->hext_host) cudaFreeHost(sim->hext_host);
     if (sim->ctr_host) cudaFreeHost(sim->ctr_host);
+    if (sim->lat_mem) cudaFree(sim->lat_mem);
+    if (sim->st_mem) cudaFree(sim->st_mem);
     delete sim;
     return FS_OK;
 }
@@ -1022,7 +1250,48 @@ int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step) {
 int fs_set_gather_variant(fs_sim* sim, int variant) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
     if (variant < 0 || variant > 2) return fail(FS_ERR_ARG, "unknown gather variant %d", variant);
+    if (variant == FS_GATHER_STENCIL && !sim->stencil_ok)
+        return fail(FS_ERR_ARG, "stencil gather unavailable for this geometry (FS_LATTICE reason %d)", sim->stencil_reason);
     sim->gather_variant = variant;
+    return FS_OK;
+}
+
+int fs_get_lattice(const fs_sim* sim, int32_t* info, double* dinfo) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (info) {
+        const LatGrid& g = sim->lg;
+        int32_t v[10] = {sim->stencil_ok ? 1 : 0, sim->stencil_reason, g.nsub, g.U, g.V, g.Ru, g.Rv,
+                         (int32_t)sim->st_slots, sim->st_nw, (int32_t)sim->st_smem};
+        for (int k = 0; k < 10; ++k) info[k] = v[k];
+    }
+    if (dinfo) { dinfo[0] = sim->st_maxdev; dinfo[1] = sim->st_wmax; }
+    return FS_OK;
+}
+
+int fs_measure_fp64_peak(double* dfma_per_s, void* stream) {
+    if (!dfma_per_s) return fail(FS_ERR_ARG, "null pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* sink = nullptr;
+    CUDA_TRY(cudaMalloc(&sink, 8));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 1 << 14, blocks = sms * 8, threads = 256;
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, st);
+        k_dfma_peak<<<blocks, threads, 0, st>>>(iters, 1.0 + rep, sink); LAUNCHED();
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+        double rate = 8.0 * iters * (double)blocks * threads / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    CUDA_TRY(cudaGetLastError());
+    *dfma_per_s = best;
     return FS_OK;
 }
 
@@ -1035,8 +1304,6 @@ int fs_scan_ensemble(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, do
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
     int rc = do_scan(sim, true);
     if (rc) return rc;
-    k_scan_finalize<<<sim->R, 256, 0, sim->stream>>>(sim->nblk, sim->bval, sim->bidx, sim->ctr); LAUNCHED();
-    CUDA_TRY(cudaGetLastError());
     if (!n_switchable && !best_index && !best_L) return FS_OK;
     rc = fetch_counters(sim);
     if (rc) return rc;
