@@ -25,7 +25,9 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <algorithm>
 #include <vector>
@@ -39,6 +41,11 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 thread_local char g_err[512] = "";
 std::atomic<long long> g_launches{0};
+// ownership of the constant-memory coupling table (lattice.cuh c_T)
+std::mutex g_ct_mutex;
+unsigned long long g_ct_owner = 0;
+std::atomic<unsigned long long> g_ct_next_id{0};
+cudaEvent_t g_ct_event = nullptr;
 
 int fail(int code, const char* fmt, ...) {
     va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof(g_err), fmt, ap); va_end(ap);
@@ -58,6 +65,12 @@ constexpr int MAX_K = 8192;             // maximum degree supported by the warp 
 constexpr int SCAN_THREADS = 256;
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// tuning overrides for experiments (unset in normal use)
+int env_int(const char* name, int dflt) {
+    const char* v = std::getenv(name);
+    return v && *v ? std::atoi(v) : dflt;
+}
 
 struct Counters {            // one per replica, device resident
     long long total_flips;
@@ -660,9 +673,10 @@ struct fs_sim {
     void* lat_mem = nullptr;        // sub | cu | cv
     void* st_mem = nullptr;         // gidx | T | owner | rowtab | scratch
     uint8_t* lat_sub = nullptr; int *lat_cu = nullptr, *lat_cv = nullptr;
-    int8_t* sgrid = nullptr;
+    uint16_t* sgrid = nullptr;
     int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
-    int st_nw = 4; size_t st_smem = 0;
+    int st_nw = 4, st_rs = 1, st_pv = 0; size_t st_smem = 0; bool st_ct = false;
+    unsigned long long st_id = 0;   // identity for the ownership of the constant-memory table
     double st_maxdev = 0.0, st_wmax = 0.0;
     long long st_slots = 0;         // stencil slots present (sum over sublattice pairs)
 };
@@ -800,16 +814,81 @@ void launch_gather_g(fs_sim* sim) {
 int do_gather_stencil(fs_sim* sim) {
     const LatGrid& g = sim->lg;
     int TV = ST_OV * sim->st_nw;
-    dim3 grid((unsigned)((g.U + ST_TU - 1) / ST_TU), (unsigned)((g.V + TV - 1) / TV), (unsigned)(g.nsub * sim->R));
-    int64_t cells = (int64_t)g.nsub * g.Vp * g.Up;
-    k_spin_grid<<<(unsigned)((cells + 255) / 256), 256, 0, sim->stream>>>(sim->N, g, sim->R, sim->gidx, sim->s, sim->sgrid);
+    dim3 sgrid((unsigned)((g.Up + 31) / 32), (unsigned)((g.Vp + 31) / 32), (unsigned)g.nsub);
+    k_spin_grid<<<sgrid, 256, 0, sim->stream>>>(sim->N, g, sim->R, sim->gidx, sim->s, sim->sgrid);
     LAUNCHED();
-    k_gather_stencil<<<grid, 32 * sim->st_nw, sim->st_smem, sim->stream>>>(sim->N, g, sim->gidx, sim->sgrid, sim->T,
-                                                                            sim->rowtab, sim->hdip);
+    dim3 grid((unsigned)((g.U + ST_TU - 1) / ST_TU), (unsigned)((g.V + TV - 1) / TV), (unsigned)(g.nsub * sim->R));
+    int threads = 32 * sim->st_nw * sim->st_rs;
+#define FS_LAUNCH_STENCIL(MAXT, MINB, CTV)                                                          \
+    k_gather_stencil<MAXT, MINB, CTV><<<grid, threads, sim->st_smem, sim->stream>>>(                \
+        sim->N, g, sim->st_nw, sim->st_pv, sim->gidx, sim->sgrid, sim->T, sim->rowtab, sim->hdip)
+    if (sim->st_ct) {
+        // the constant-memory table is shared by all simulations of the process: take it over if needed
+        std::lock_guard<std::mutex> lock(g_ct_mutex);
+        if (g_ct_owner != sim->st_id) {
+            if (g_ct_event) CUDA_TRY(cudaStreamWaitEvent(sim->stream, g_ct_event, 0));   // previous owner's kernels first
+            CUDA_TRY(cudaMemcpyToSymbolAsync(c_T, sim->T, 16 * (size_t)g.nsub * g.nsub * g.W * g.H, 0,
+                                             cudaMemcpyDeviceToDevice, sim->stream));
+            CUDA_TRY(cudaMemcpyToSymbolAsync(c_rows, sim->rowtab, 8 * (size_t)g.nsub * g.nsub * g.W, 0,
+                                             cudaMemcpyDeviceToDevice, sim->stream));
+            g_ct_owner = sim->st_id;
+        }
+        if (threads <= 128) FS_LAUNCH_STENCIL(128, 7, true); else FS_LAUNCH_STENCIL(256, 3, true);
+        if (!g_ct_event) CUDA_TRY(cudaEventCreateWithFlags(&g_ct_event, cudaEventDisableTiming));
+        CUDA_TRY(cudaEventRecord(g_ct_event, sim->stream));
+    } else {
+        if (threads <= 128) FS_LAUNCH_STENCIL(128, 7, false); else FS_LAUNCH_STENCIL(256, 3, false);
+    }
+#undef FS_LAUNCH_STENCIL
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     sim->fields_dirty = false;
     return FS_OK;
+}
+
+// Shape of the stencil kernel for this lattice: NW v-slabs x RS row groups per CTA.  Small model: every
+// CTA does work ~ NW; an SM runs ceil(ctas / SMs) of them (one wave if they fit) and needs >= 20
+// resident warps to keep its FP64 pipe busy.  Ties go to the larger tile (less halo), then fewer groups.
+struct StencilShape { int nw, rs, pv; size_t smem; };
+
+bool stencil_ct(const LatGrid& g) {
+    return (int64_t)g.nsub * g.nsub * g.W * g.H <= CT_MAX && g.nsub * g.nsub * g.W <= CR_MAX &&
+           env_int("FS_STENCIL_NO_CT", 0) == 0;
+}
+
+size_t stencil_smem(const LatGrid& g, int nw, int rs, int* pv_out) {
+    int TV = ST_OV * nw, SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv;
+    int pv = SH + 2; while ((pv & 3) != 2) ++pv;                     // row pitch = 2 mod 4 cells: lanes -> distinct banks
+    size_t tsm = stencil_ct(g) ? 0 : 16 * (size_t)g.nsub * g.W * g.H;
+    size_t tables = (tsm + 8 * (size_t)g.nsub * g.W + 128 * (size_t)TV + 15) & ~(size_t)15;
+    size_t tiles = 2 * (size_t)g.nsub * SU * pv, red = (size_t)(rs - 1) * nw * 4096;
+    if (pv_out) *pv_out = pv;
+    return tables + std::max(tiles, red);
+}
+
+bool plan_stencil(const fs_sim* sim, const LatGrid& g, StencilShape* out) {
+    double best = 1e300; bool found = false;
+    for (int nw = 8; nw >= 1; nw >>= 1)
+        for (int rs = 1; rs <= 4 && nw * rs <= 8; rs <<= 1) {
+            if (rs > g.W) continue;
+            int pv; size_t smem = stencil_smem(g, nw, rs, &pv);
+            if (smem > 200 * 1024) continue;
+            int threads = 32 * nw * rs, TV = ST_OV * nw;
+            int64_t ctas = (int64_t)((g.U + ST_TU - 1) / ST_TU) * ((g.V + TV - 1) / TV) * g.nsub * sim->R;
+            int regs = threads <= 128 ? 72 : 80;
+            int64_t resident = std::min<int64_t>(std::min<int64_t>(65536 / (regs * threads), (227 * 1024) / (int64_t)(smem + 1024)),
+                                                 std::min<int64_t>(2048 / threads, 32));
+            if (resident < 1) continue;
+            int64_t per_sm = (ctas + sim->sm_count - 1) / sim->sm_count;
+            int64_t waves = (per_sm + resident - 1) / resident;
+            double warps = (double)std::min(per_sm, resident) * nw * rs;
+            double eff = std::min(1.0, warps / 20.0);
+            // multi-wave launches pay for a partly filled last wave
+            double cost = (waves == 1 ? (double)per_sm : (double)waves * resident) * nw / eff;
+            cost *= 1.0 + 0.02 * (rs - 1) + 0.16 / nw;               // reduction epilogue; halo staging per output
+            if (cost < best - 1e-9) { best = cost; *out = StencilShape{nw, rs, pv, smem}; found = true; }
+        }
+    return found;
 }
 
 int do_gather(fs_sim* sim) {
@@ -952,24 +1031,22 @@ int detect_lattice(fs_sim* sim) {
         return lattice_fail(sim, FS_LATTICE_TOO_SPARSE);
     g.U = (int)U; g.V = (int)V; g.Up = (int)Up; g.Vp = (int)Vp; g.W = 2 * g.Ru + 1; g.H = 2 * g.Rv + 1;
     std::memcpy(&sim->st_wmax, &wbits, 8);
-    // kernel shape: few warps per CTA when the stencil is wide (compute-bound: small tiles balance the
-    // SMs), many when it is narrow (staging-bound: large tiles amortise the halo)
     int wh = g.W * g.H;
-    sim->st_nw = wh >= 100 ? 2 : (wh >= 25 ? 4 : 8);
-    const int pitch = ((ST_TU + 2 * g.Ru + 15) / 16) * 16;
-    for (;;) {
-        int TV = ST_OV * sim->st_nw;
-        sim->st_smem = 8 * (size_t)(TV + 2 * g.Rv) * pitch + 16 * (size_t)(wh + 1) + 8 * (size_t)g.W;
-        if (sim->st_smem <= 200 * 1024 || sim->st_nw == 1) break;
-        sim->st_nw >>= 1;
+    StencilShape shp{};
+    if (!plan_stencil(sim, g, &shp)) return lattice_fail(sim, FS_LATTICE_STENCIL_TOO_WIDE);
+    if (env_int("FS_STENCIL_NW", 0) > 0) {                           // tuning override
+        shp.nw = env_int("FS_STENCIL_NW", 0); shp.rs = std::max(1, env_int("FS_STENCIL_RS", 1));
+        shp.smem = stencil_smem(g, shp.nw, shp.rs, &shp.pv);
     }
-    if (sim->st_smem > 200 * 1024) return lattice_fail(sim, FS_LATTICE_STENCIL_TOO_WIDE);
+    sim->st_nw = shp.nw; sim->st_rs = shp.rs; sim->st_pv = shp.pv; sim->st_smem = shp.smem;
+    sim->st_ct = stencil_ct(g);
+    sim->st_id = ++g_ct_next_id;
     {
         int TV = ST_OV * sim->st_nw;
-        g.Upa = (g.U + ST_TU - 1) / ST_TU * ST_TU - ST_TU + pitch;      // last tile's row of chunks stays in bounds
+        g.Upa = (g.U + ST_TU - 1) / ST_TU * ST_TU + 2 * g.Ru;           // whole tiles + halo: the prologue needs no bounds tests
         g.Vpa = (g.V + TV - 1) / TV * TV + 2 * g.Rv;
     }
-    const size_t sg_bytes = (size_t)sim->R * nsub * g.Vpa * g.Upa;
+    const size_t sg_bytes = 2 * (size_t)sim->R * nsub * g.Vpa * g.Upa;
     // tables
     size_t slots = (size_t)nsub * nsub * wh;
     size_t o_gidx = 0, o_T = align_up(4 * (size_t)cells), o_owner = o_T + align_up(16 * slots),
@@ -978,7 +1055,7 @@ int detect_lattice(fs_sim* sim) {
     CUDA_TRY(cudaMalloc(&sim->st_mem, o_end));
     unsigned char* sb = (unsigned char*)sim->st_mem;
     sim->gidx = (int*)(sb + o_gidx); sim->T = (double2*)(sb + o_T); sim->owner = (unsigned long long*)(sb + o_owner);
-    sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (int8_t*)(sb + o_sg);
+    sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (uint16_t*)(sb + o_sg);
     CUDA_TRY(cudaMemsetAsync(sim->sgrid, 0, sg_bytes, st));
     CUDA_TRY(cudaMemsetAsync(sim->gidx, 0xff, 4 * (size_t)cells, st));
     CUDA_TRY(cudaMemsetAsync(sim->T, 0, 16 * slots, st));
@@ -1004,8 +1081,13 @@ int detect_lattice(fs_sim* sim) {
     if (flags & 4) return lattice_fail(sim, FS_LATTICE_NOT_PERIODIC);
     if ((long long)res64[2] != (long long)sim->n_inter) return lattice_fail(sim, FS_LATTICE_REACH_MISMATCH);
     if (!(sim->st_maxdev * (double)sim->K <= 2e-13 * sim->st_wmax)) return lattice_fail(sim, FS_LATTICE_WEIGHT_MISMATCH);
-    if (sim->st_smem > 48 * 1024)
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->st_smem));
+    if (sim->st_smem > 48 * 1024) {
+        int b = (int)sim->st_smem;
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+    }
     sim->lg = g;
     sim->stencil_ok = true; sim->stencil_reason = 0;
     // the build-only arrays (sub, cu, cv) are no longer needed
@@ -1261,7 +1343,7 @@ int fs_get_lattice(const fs_sim* sim, int32_t* info, double* dinfo) {
     if (info) {
         const LatGrid& g = sim->lg;
         int32_t v[10] = {sim->stencil_ok ? 1 : 0, sim->stencil_reason, g.nsub, g.U, g.V, g.Ru, g.Rv,
-                         (int32_t)sim->st_slots, sim->st_nw, (int32_t)sim->st_smem};
+                         (int32_t)sim->st_slots, sim->st_nw * sim->st_rs, (int32_t)sim->st_smem};
         for (int k = 0; k < 10; ++k) info[k] = v[k];
     }
     if (dinfo) { dinfo[0] = sim->st_maxdev; dinfo[1] = sim->st_wmax; }

@@ -31,7 +31,7 @@ struct LatFrame { double ox, oy, i11, i12, i21, i22; };   // (u, v) = Ainv (r - 
 
 struct LatGrid {
     int nsub, u0, v0, U, V, Ru, Rv, Up, Vp, W, H;         // W = 2Ru+1, H = 2Rv+1, Up = U+2Ru, Vp = V+2Rv
-    int Upa, Vpa;                                         // spin-grid allocation: whole tiles + halo, Upa % 16 == 0
+    int Upa, Vpa;                                         // spin-grid allocation [Upa][Vpa]: whole tiles + halo, Vpa even
 };
 
 __device__ __forceinline__ void lat_uv(const LatFrame& f, double2 p, double& u, double& v) {
@@ -174,122 +174,204 @@ __global__ void k_stencil_count(int64_t N, LatGrid g, const uint8_t* __restrict_
     if ((threadIdx.x & 31) == 0 && n) atomicAdd(total, n);
 }
 
-// dense spin grids sg[rep][sub][Vpa][Upa] (int8; 0 = no magnet) from the spin array, once per gather
+// dense spin grids sg[rep][sub][Upa][Vpa] (v fastest), one 16-bit cell per lattice site = the upper 16
+// bits of the spin as a double (+1.0 -> 0x3ff0, -1.0 -> 0xbff0, no magnet -> 0), rebuilt from s once
+// per gather.  32 x 32 tiles are transposed through shared memory: gidx is read along u, sg written
+// along v, both coalesced.
 __global__ void k_spin_grid(int64_t N, LatGrid g, int R, const int* __restrict__ gidx, const int8_t* __restrict__ s_all,
-                            int8_t* __restrict__ sg) {
-    int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    int64_t cells = (int64_t)g.nsub * g.Vp * g.Up;
-    if (t >= cells) return;
-    int gu = (int)(t % g.Up);
-    int64_t q = t / g.Up;                                // sub * Vp + gv
-    int gv = (int)(q % g.Vp), sub = (int)(q / g.Vp);
-    int idx = gidx[t];
-    for (int r = 0; r < R; ++r)
-        sg[(((int64_t)r * g.nsub + sub) * g.Vpa + gv) * g.Upa + gu] = idx >= 0 ? s_all[(int64_t)r * N + idx] : (int8_t)0;
-}
-
-// ------------------------------------------------------------------------------------------------
-// A3, stencil variant.  CTA = NW warps; tile = 32 cells along u (one per lane) x 8*NW cells along v
-// (8 consecutive outputs per thread).  Per source sublattice: the spin tile + halo is staged in shared
-// memory as doubles (0.0 = no magnet) with 16-byte loads of the int8 grid, then for each stencil row
-// du the thread slides an 8-wide register window along v: per stencil slot one 8-byte shared load +
-// one broadcast 16-byte weight load (prefetched one slot ahead) feed 16 DFMA.
-// blockIdx.z = replica * nsub + target sublattice.
-// ------------------------------------------------------------------------------------------------
-#define FS_ST_STEP(TA, TB, X0, X1, X2, X3, X4, X5, X6, X7)                             \
-    {                                                                                  \
-        TB = *tp++;                                                                    \
-        a0x = fma(X0, TA.x, a0x); a0y = fma(X0, TA.y, a0y);                            \
-        a1x = fma(X1, TA.x, a1x); a1y = fma(X1, TA.y, a1y);                            \
-        a2x = fma(X2, TA.x, a2x); a2y = fma(X2, TA.y, a2y);                            \
-        a3x = fma(X3, TA.x, a3x); a3y = fma(X3, TA.y, a3y);                            \
-        a4x = fma(X4, TA.x, a4x); a4y = fma(X4, TA.y, a4y);                            \
-        a5x = fma(X5, TA.x, a5x); a5y = fma(X5, TA.y, a5y);                            \
-        a6x = fma(X6, TA.x, a6x); a6y = fma(X6, TA.y, a6y);                            \
-        a7x = fma(X7, TA.x, a7x); a7y = fma(X7, TA.y, a7y);                            \
-        if (--n == 0) break;                                                           \
-        X0 = *sp; sp += P;                                                             \
+                            uint16_t* __restrict__ sg) {
+    __shared__ int tile[32][33];
+    const int sub = blockIdx.z, gu0 = blockIdx.x * 32, gv0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;           // 32 x 8 threads
+    for (int k = ty; k < 32; k += 8) {
+        int gu = gu0 + tx, gv = gv0 + k;
+        tile[k][tx] = (gu < g.Up && gv < g.Vp) ? gidx[((int64_t)sub * g.Vp + gv) * g.Up + gu] : -1;
     }
-
-__device__ __forceinline__ double spin_as_double(unsigned b) {     // int8 {-1, 0, +1} -> double, integer ops only
-    unsigned hi = (b & 0xffu) ? (0x3ff00000u | ((b & 0x80u) << 24)) : 0u;
-    return __hiloint2double((int)hi, 0);
+    __syncthreads();
+    for (int k = ty; k < 32; k += 8) {
+        int gu = gu0 + k, gv = gv0 + tx;
+        if (gu >= g.Up || gv >= g.Vp) continue;
+        int idx = tile[tx][k];
+        for (int r = 0; r < R; ++r) {
+            int sv = idx >= 0 ? (int)s_all[(int64_t)r * N + idx] : 0;
+            sg[(((int64_t)r * g.nsub + sub) * g.Upa + gu) * g.Vpa + gv] = (uint16_t)(sv > 0 ? 0x3ff0 : (sv < 0 ? 0xbff0 : 0));
+        }
+    }
 }
 
-__global__ void __launch_bounds__(256) k_gather_stencil(int64_t N, LatGrid g, const int* __restrict__ gidx,
-                                                        const int8_t* __restrict__ sg, const double2* __restrict__ T,
-                                                        const int2* __restrict__ rowtab, double2* __restrict__ hdip_all) {
-    extern __shared__ double st_sm[];
-    const int NW = blockDim.x >> 5, TV = ST_OV * NW;
-    const int chunks = (ST_TU + 2 * g.Ru + 15) >> 4;   // 16-cell chunks per tile row
-    const int P = chunks << 4;                         // shared row pitch (u fastest)
-    const int SH = TV + 2 * g.Rv;
-    double* S = st_sm;                                 // [SH][P]
-    double2* Tsm = reinterpret_cast<double2*>(S + (size_t)SH * P);   // [W][H] + 1
-    int2* rows = reinterpret_cast<int2*>(Tsm + (size_t)g.W * g.H + 1);   // [W]
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src));
+}
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(gmem_src));
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// ------------------------------------------------------------------------------------------------
+// A3, stencil variant.  CTA = NW x RS warps; tile = 32 cells along u (one per lane) x 8*NW cells
+// along v (8 consecutive outputs per thread).  Prologue: the 16-bit spin tiles (+ halo) of every
+// source sublattice, the coupling tables T[si][*], their row intervals and the spin index of every
+// output go to shared memory with cp.async in one shot (one global round trip per CTA, no staging
+// through registers).  Main loop: for each stencil row du the thread slides an 8-wide register window
+// along v, which is the contiguous direction of its shared-memory row (immediate offsets, row pitch
+// = 2 mod 4 cells so the 32 lanes hit 32 banks); per stencil slot one 2-byte shared load (shifted
+// into the high word of a double whose low word is a register that stays zero) + one broadcast
+// 16-byte weight load feed 16 DFMA.  The stencil rows are dealt round-robin to RS warp groups that
+// share the tile (RS times the warps for the same shared-memory traffic: the FP64 pipe wants >= 4
+// warps per scheduler); their partial sums are added through shared memory in a fixed order.
+// blockIdx.z = replica * nsub + target sublattice.  blockDim = 32 * NW * RS.
+// ------------------------------------------------------------------------------------------------
+#define FS_ST_LD(K, Z) __hiloint2double((int)((unsigned)sp[K] << 16), Z)
+#define FS_ST_FMA(X0, X1, X2, X3, X4, X5, X6, X7, K)                                   \
+        const double2 t##K = CT ? c_T[tofs + K] : tp[K];                               \
+        a0x = fma(X0, t##K.x, a0x); a0y = fma(X0, t##K.y, a0y);                        \
+        a1x = fma(X1, t##K.x, a1x); a1y = fma(X1, t##K.y, a1y);                        \
+        a2x = fma(X2, t##K.x, a2x); a2y = fma(X2, t##K.y, a2y);                        \
+        a3x = fma(X3, t##K.x, a3x); a3y = fma(X3, t##K.y, a3y);                        \
+        a4x = fma(X4, t##K.x, a4x); a4y = fma(X4, t##K.y, a4y);                        \
+        a5x = fma(X5, t##K.x, a5x); a5y = fma(X5, t##K.y, a5y);                        \
+        a6x = fma(X6, t##K.x, a6x); a6y = fma(X6, t##K.y, a6y);                        \
+        a7x = fma(X7, t##K.x, a7x); a7y = fma(X7, t##K.y, a7y);
+// one slot of a full group of 8 (no exit test); slot K consumes the window and refills its oldest cell
+#define FS_ST_FULL(X0, X1, X2, X3, X4, X5, X6, X7, Z, K)                               \
+    { FS_ST_FMA(X0, X1, X2, X3, X4, X5, X6, X7, K) X0 = FS_ST_LD(8 + K, Z); }
+// one slot of the ragged tail
+#define FS_ST_TAIL(X0, X1, X2, X3, X4, X5, X6, X7, Z, K)                               \
+    { FS_ST_FMA(X0, X1, X2, X3, X4, X5, X6, X7, K) if (--n == 0) break; X0 = FS_ST_LD(8 + K, Z); }
+
+// Coupling tables of the lattice that used the stencil last (all sublattice pairs), for the CT variant of
+// k_gather_stencil: a warp-uniform weight read through the constant cache lands in a uniform register,
+// and DFMA R, R, UR, R reads only two vector-register pairs: 62 DFMA/clk/SM measured against 51 with
+// the weight in a vector register.  Re-uploaded when another simulation takes over.
+constexpr int CT_MAX = 3584;           // double2 entries (56 KB of the 64 KB constant bank)
+constexpr int CR_MAX = 960;            // row intervals (7.5 KB)
+__constant__ double2 c_T[CT_MAX];
+__constant__ int2 c_rows[CR_MAX];
+
+template <int MAXT, int MINB, bool CT>
+__global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGrid g, int NW, int Pv,
+                                                               const int* __restrict__ gidx, const uint16_t* __restrict__ sg,
+                                                               const double2* __restrict__ T, const int2* __restrict__ rowtab,
+                                                               double2* __restrict__ hdip_all) {
+    extern __shared__ __align__(16) unsigned char st_raw[];
+    const int RS = (blockDim.x >> 5) / NW, TV = ST_OV * NW;
+    const int SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv, WH = g.W * g.H;
+    double2* Tsm = reinterpret_cast<double2*>(st_raw);                      // [nsub][WH]
+    const size_t tsm_n = CT ? 0 : (size_t)g.nsub * WH;                      // no shared copy of T in the CT variant
+    int2* rows = reinterpret_cast<int2*>(Tsm + tsm_n);                      // [nsub][W]
+    int* oidx = reinterpret_cast<int*>(rows + (size_t)g.nsub * g.W);        // [TV][32] spin index of every output
+    uint16_t* S = reinterpret_cast<uint16_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 15) & ~(size_t)15));   // [nsub][SU][Pv]
     const int si = blockIdx.z % g.nsub, rep = blockIdx.z / g.nsub;
     const int tu0 = blockIdx.x * ST_TU, tv0 = blockIdx.y * TV;       // tile origin, interior coordinates
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // the warp index via a shuffle from lane 0: the compiler then knows everything derived from it is
+    // warp-uniform and keeps row intervals / weight offsets / weights in uniform registers
+    const int wid_u = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31, warp = wid_u % NW, rs = wid_u / NW;
+
+    // ---- prologue: everything this CTA reads, in flight at once
+    {
+        const int HP = SH >> 1;                        // SH is even: 2-cell (4-byte) pieces per row
+        const uint16_t* src = sg + (((int64_t)rep * g.nsub * g.Upa + tu0) * g.Vpa + tv0);
+        const int nwarps = blockDim.x >> 5, wid = threadIdx.x >> 5;
+        for (int sj = 0; sj < g.nsub; ++sj)
+            for (int ul = wid; ul < SU; ul += nwarps) {            // one tile row per warp: no index divisions
+                uint16_t* drow = S + ((size_t)sj * SU + ul) * Pv;
+                const uint16_t* srow = src + ((int64_t)sj * g.Upa + ul) * g.Vpa;
+                for (int c = lane; c < HP; c += 32) cp_async4(drow + 2 * c, srow + 2 * c);
+            }
+    }
+    if (!CT)
+        for (int t = threadIdx.x; t < g.nsub * WH; t += blockDim.x) cp_async16(Tsm + t, T + (int64_t)si * g.nsub * WH + t);
+    for (int t = threadIdx.x; t < g.nsub * g.W; t += blockDim.x) rows[t] = __ldg(rowtab + si * g.nsub * g.W + t);
+    for (int t = threadIdx.x; t < TV * 32; t += blockDim.x) {
+        int gu = tu0 + (t & 31) + g.Ru, gv = tv0 + (t >> 5) + g.Rv;
+        if (gu < g.Up && gv < g.Vp) cp_async4(oidx + t, gidx + ((int64_t)si * g.Vp + gv) * g.Up + gu);
+        else oidx[t] = -1;
+    }
+    cp_async_wait_all();
+    __syncthreads();
 
     double a0x = 0, a0y = 0, a1x = 0, a1y = 0, a2x = 0, a2y = 0, a3x = 0, a3y = 0;
     double a4x = 0, a4y = 0, a5x = 0, a5y = 0, a6x = 0, a6y = 0, a7x = 0, a7y = 0;
+    int z0, z1, z2, z3, z4, z5, z6, z7;                // eight zeros the compiler cannot merge: the low words of x0..x7
+    asm volatile("mov.u32 %0, 0; mov.u32 %1, 0; mov.u32 %2, 0; mov.u32 %3, 0; mov.u32 %4, 0; mov.u32 %5, 0; mov.u32 %6, 0; mov.u32 %7, 0;"
+                 : "=r"(z0), "=r"(z1), "=r"(z2), "=r"(z3), "=r"(z4), "=r"(z5), "=r"(z6), "=r"(z7));
 
     for (int sj = 0; sj < g.nsub; ++sj) {
-        const int pair = si * g.nsub + sj;
-        __syncthreads();                               // the previous pass is done with S/Tsm/rows
-        const int8_t* src = sg + (((int64_t)rep * g.nsub + sj) * g.Vpa + tv0) * g.Upa + tu0;
-        for (int t = threadIdx.x; t < SH * chunks; t += blockDim.x) {
-            int vl = t / chunks, c = t - vl * chunks;
-            const uint4 raw = __ldg(reinterpret_cast<const uint4*>(src + (int64_t)vl * g.Upa + 16 * c));
-            double2* dst = reinterpret_cast<double2*>(S + (size_t)vl * P + 16 * c);
-            const unsigned wds[4] = {raw.x, raw.y, raw.z, raw.w};
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                dst[2 * k] = make_double2(spin_as_double(wds[k]), spin_as_double(wds[k] >> 8));
-                dst[2 * k + 1] = make_double2(spin_as_double(wds[k] >> 16), spin_as_double(wds[k] >> 24));
-            }
-        }
-        for (int t = threadIdx.x; t < g.W * g.H; t += blockDim.x) Tsm[t] = __ldg(T + (int64_t)pair * g.W * g.H + t);
-        if (threadIdx.x == 0) Tsm[g.W * g.H] = make_double2(0.0, 0.0);       // read (never used) by the last prefetch
-        for (int t = threadIdx.x; t < g.W; t += blockDim.x) rows[t] = __ldg(rowtab + pair * g.W + t);
-        __syncthreads();
-        for (int r = 0; r < g.W; ++r) {                // r = du + Ru
-            const int2 rt = rows[r];
+        const uint16_t* Sj = S + ((size_t)sj * SU + lane) * Pv + warp * ST_OV + g.Rv;
+        const double2* Tj = Tsm + (CT ? 0 : (size_t)sj * WH + g.Rv);
+        const int tj = (si * g.nsub + sj) * WH + g.Rv;
+        for (int r = 0; r < g.W; ++r) {                // r = du + Ru: a uniform counter, so that the row interval
+            if (r % RS != rs) continue;                // and the weight offsets below live in uniform registers
+            const int2 rt = CT ? c_rows[(si * g.nsub + sj) * g.W + r] : rows[sj * g.W + r];
             int n = rt.y - rt.x + 1;
             if (n <= 0) continue;
-            // output (lane, warp*8+q) reads S[(warp*8 + q + dv + Rv)][lane + du + Ru]
-            const double* sp = S + (size_t)(warp * ST_OV + rt.x + g.Rv) * P + (lane + r);
-            const double2* tp = Tsm + r * g.H + (rt.x + g.Rv);
-            double x0 = sp[0], x1 = sp[P], x2 = sp[2 * P], x3 = sp[3 * P];
-            double x4 = sp[4 * P], x5 = sp[5 * P], x6 = sp[6 * P], x7 = sp[7 * P];
-            sp += 8 * P;
-            double2 ta = *tp++, tb;
-            for (;;) {
-                FS_ST_STEP(ta, tb, x0, x1, x2, x3, x4, x5, x6, x7)
-                FS_ST_STEP(tb, ta, x1, x2, x3, x4, x5, x6, x7, x0)
-                FS_ST_STEP(ta, tb, x2, x3, x4, x5, x6, x7, x0, x1)
-                FS_ST_STEP(tb, ta, x3, x4, x5, x6, x7, x0, x1, x2)
-                FS_ST_STEP(ta, tb, x4, x5, x6, x7, x0, x1, x2, x3)
-                FS_ST_STEP(tb, ta, x5, x6, x7, x0, x1, x2, x3, x4)
-                FS_ST_STEP(ta, tb, x6, x7, x0, x1, x2, x3, x4, x5)
-                FS_ST_STEP(tb, ta, x7, x0, x1, x2, x3, x4, x5, x6)
+            // output (lane, warp*8+q) at slot (du, dv) reads S[sj][lane + du + Ru][warp*8 + q + dv + Rv]
+            const uint16_t* sp = Sj + (size_t)r * Pv + rt.x;
+            const double2* tp = Tj + (CT ? 0 : r * g.H + rt.x);
+            int tofs = tj + r * g.H + rt.x;
+            double x0 = FS_ST_LD(0, z0), x1 = FS_ST_LD(1, z1), x2 = FS_ST_LD(2, z2), x3 = FS_ST_LD(3, z3);
+            double x4 = FS_ST_LD(4, z4), x5 = FS_ST_LD(5, z5), x6 = FS_ST_LD(6, z6), x7 = FS_ST_LD(7, z7);
+            for (; n >= 8; n -= 8, sp += 8, tp += 8, tofs += 8) {
+                FS_ST_FULL(x0, x1, x2, x3, x4, x5, x6, x7, z0, 0)
+                FS_ST_FULL(x1, x2, x3, x4, x5, x6, x7, x0, z1, 1)
+                FS_ST_FULL(x2, x3, x4, x5, x6, x7, x0, x1, z2, 2)
+                FS_ST_FULL(x3, x4, x5, x6, x7, x0, x1, x2, z3, 3)
+                FS_ST_FULL(x4, x5, x6, x7, x0, x1, x2, x3, z4, 4)
+                FS_ST_FULL(x5, x6, x7, x0, x1, x2, x3, x4, z5, 5)
+                FS_ST_FULL(x6, x7, x0, x1, x2, x3, x4, x5, z6, 6)
+                FS_ST_FULL(x7, x0, x1, x2, x3, x4, x5, x6, z7, 7)
             }
+            if (n > 0) do {
+                FS_ST_TAIL(x0, x1, x2, x3, x4, x5, x6, x7, z0, 0)
+                FS_ST_TAIL(x1, x2, x3, x4, x5, x6, x7, x0, z1, 1)
+                FS_ST_TAIL(x2, x3, x4, x5, x6, x7, x0, x1, z2, 2)
+                FS_ST_TAIL(x3, x4, x5, x6, x7, x0, x1, x2, z3, 3)
+                FS_ST_TAIL(x4, x5, x6, x7, x0, x1, x2, x3, z4, 4)
+                FS_ST_TAIL(x5, x6, x7, x0, x1, x2, x3, x4, z5, 5)
+                FS_ST_TAIL(x6, x7, x0, x1, x2, x3, x4, x5, z6, 6)
+            } while (0);
         }
     }
-    // epilogue: scatter the 8 outputs of this thread to their spins
-    double2* __restrict__ hdip = hdip_all + (int64_t)rep * N;
-    const int gu = tu0 + lane + g.Ru;
-    if (gu < g.Up) {
-        const int gv0 = tv0 + warp * ST_OV + g.Rv;
-        const int* gi = gidx + ((int64_t)si * g.Vp + gv0) * g.Up + gu;
-#define FS_ST_OUT(q, AX, AY)                                                           \
-        if (gv0 + q < g.Vp) { int idx = __ldg(gi + (int64_t)q * g.Up); if (idx >= 0) hdip[idx] = make_double2(AX, AY); }
-        FS_ST_OUT(0, a0x, a0y) FS_ST_OUT(1, a1x, a1y) FS_ST_OUT(2, a2x, a2y) FS_ST_OUT(3, a3x, a3y)
-        FS_ST_OUT(4, a4x, a4y) FS_ST_OUT(5, a5x, a5y) FS_ST_OUT(6, a6x, a6y) FS_ST_OUT(7, a7x, a7y)
-#undef FS_ST_OUT
+    // ---- epilogue: add the row groups' partial sums (fixed order), scatter the 8 outputs to their spins
+    if (RS > 1) {
+        __syncthreads();                               // everyone is done with the tiles
+        double* red_base = reinterpret_cast<double*>(S);
+        double* red = red_base + ((size_t)((rs - 1) * NW + warp) * 16) * 32 + lane;
+        if (rs > 0) {
+            red[0 * 32] = a0x; red[1 * 32] = a0y; red[2 * 32] = a1x; red[3 * 32] = a1y;
+            red[4 * 32] = a2x; red[5 * 32] = a2y; red[6 * 32] = a3x; red[7 * 32] = a3y;
+            red[8 * 32] = a4x; red[9 * 32] = a4y; red[10 * 32] = a5x; red[11 * 32] = a5y;
+            red[12 * 32] = a6x; red[13 * 32] = a6y; red[14 * 32] = a7x; red[15 * 32] = a7y;
+        }
+        __syncthreads();
+        if (rs > 0) return;
+        for (int k = 1; k < RS; ++k) {
+            const double* rd = red_base + ((size_t)((k - 1) * NW + warp) * 16) * 32 + lane;
+            a0x += rd[0 * 32]; a0y += rd[1 * 32]; a1x += rd[2 * 32]; a1y += rd[3 * 32];
+            a2x += rd[4 * 32]; a2y += rd[5 * 32]; a3x += rd[6 * 32]; a3y += rd[7 * 32];
+            a4x += rd[8 * 32]; a4y += rd[9 * 32]; a5x += rd[10 * 32]; a5y += rd[11 * 32];
+            a6x += rd[12 * 32]; a6y += rd[13 * 32]; a7x += rd[14 * 32]; a7y += rd[15 * 32];
+        }
     }
+    double2* __restrict__ hdip = hdip_all + (int64_t)rep * N;
+    const int* oi = oidx + (warp * ST_OV) * 32 + lane;
+    int i;
+    if ((i = oi[0 * 32]) >= 0) hdip[i] = make_double2(a0x, a0y);
+    if ((i = oi[1 * 32]) >= 0) hdip[i] = make_double2(a1x, a1y);
+    if ((i = oi[2 * 32]) >= 0) hdip[i] = make_double2(a2x, a2y);
+    if ((i = oi[3 * 32]) >= 0) hdip[i] = make_double2(a3x, a3y);
+    if ((i = oi[4 * 32]) >= 0) hdip[i] = make_double2(a4x, a4y);
+    if ((i = oi[5 * 32]) >= 0) hdip[i] = make_double2(a5x, a5y);
+    if ((i = oi[6 * 32]) >= 0) hdip[i] = make_double2(a6x, a6y);
+    if ((i = oi[7 * 32]) >= 0) hdip[i] = make_double2(a7x, a7y);
 }
-#undef FS_ST_STEP
+#undef FS_ST_FULL
+#undef FS_ST_TAIL
+#undef FS_ST_FMA
+#undef FS_ST_LD
 
 // DFMA-chain calibration: every thread runs 8 independent chains of `iters` DFMAs.
 __global__ void k_dfma_peak(int iters, double seed, double* __restrict__ sink) {
