@@ -131,15 +131,41 @@ __device__ __forceinline__ double2 thermal_xy(double sigma, uint64_t seed, uint3
     return make_double2(sigma * r * cs, sigma * r * sn);
 }
 
-struct Astroid { double inv_b, inv_c, e_par, e_perp; };   // 1/b, 1/c, 2/gamma, 2/beta
+struct Astroid { double inv_b, inv_c, e_par, e_perp; int k_par, k_perp; };   // 1/b, 1/c, 2/gamma, 2/beta, power kinds
 
-// switching margin M_i (Eq. 5 left-hand side if Eq. 6 holds, else -inf): PAPER.md:103, :112
-__device__ __forceinline__ double margin(double hpar, double hperp, double s, double hc, const Astroid& a) {
+// x^e for x >= 0, e > 0.  kind 1: e = 2/3 (gamma or beta = 3, the classical astroid, Eq. 4)
+// -> cbrt(x^2); kind 2: e = 1; kind 3: e = 2; else exp(e log x).  On this path (one warp, a dependent
+// chain per flip) CUDA's pow costs ~770 cycles, exp(log) ~450, cbrt ~310 (measured); all are within a
+// few ulp of the exact power, far inside the 1e-12 parity bar and the >= 1e-10 decision gaps (D-3).
+__device__ __forceinline__ double pow_kind(double x, double e, int kind) {
+    if (kind == 1) return cbrt(x * x);
+    if (kind == 2) return x;
+    if (kind == 3) return x * x;
+    return x > 0.0 ? exp(e * log(x)) : 0.0;
+}
+
+// switching margin M_i (Eq. 5 left-hand side if Eq. 6 holds, else -inf): PAPER.md:103, :112.
+// ihc = 1 / h_c^(i), precomputed once (k_frame).
+__device__ __forceinline__ double margin(double hpar, double hperp, double s, double ihc, const Astroid& a) {
     if (!(s * hpar < 0.0)) return -CUDART_INF;
-    double ihc = 1.0 / hc;
-    double x = fabs(hpar) * a.inv_b * ihc;
-    double y = fabs(hperp) * a.inv_c * ihc;
-    return pow(x, a.e_par) + pow(y, a.e_perp);
+    double x = fabs(hpar) * (a.inv_b * ihc);
+    double y = fabs(hperp) * (a.inv_c * ihc);
+    return pow_kind(x, a.e_par, a.k_par) + pow_kind(y, a.e_perp, a.k_perp);
+}
+
+// arg-max over a warp with key (value descending, index ascending).  Values are margins: either -inf
+// or >= 0, so their bit patterns order like unsigned integers (-inf and 0 both map to key 0: neither
+// can win, only margins > 1 matter).  Three REDUX reductions (~100 cycles) instead of five rounds of
+// three shuffles and a double compare (~350 cycles, measured).
+__device__ __forceinline__ void warp_argmax_margin(double& v, int& i) {
+    unsigned long long key = v > 0.0 ? (unsigned long long)__double_as_longlong(v) : 0ull;
+    unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
+    unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
+    unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
+    unsigned mi = __reduce_min_sync(0xffffffffu, (hi == mhi && lo == mlo) ? (unsigned)i : 0xffffffffu);
+    key = ((unsigned long long)mhi << 32) | mlo;
+    v = key ? __longlong_as_double((long long)key) : -CUDART_INF;
+    i = (int)mi;
 }
 
 #include "lattice.cuh"
@@ -147,7 +173,7 @@ __device__ __forceinline__ double margin(double hpar, double hperp, double s, do
 // ------------------------------------------------------------------------------------------------
 // A0: frame tables + hc validation
 // ------------------------------------------------------------------------------------------------
-__global__ void k_frame(int64_t N, int R, const double* __restrict__ angle, const double* __restrict__ hc,
+__global__ void k_frame(int64_t N, int R, const double* __restrict__ angle, double* __restrict__ hc /* in: h_c, out: 1/h_c */,
                         double2* __restrict__ cs, int* __restrict__ flags) {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -158,6 +184,7 @@ __global__ void k_frame(int64_t N, int R, const double* __restrict__ angle, cons
     for (int r = 0; r < R; ++r) {
         double h = hc[(int64_t)r * N + i];
         bad |= !(h > 0.0) || !isfinite(h);
+        hc[(int64_t)r * N + i] = 1.0 / h;
     }
     if (bad) atomicOr(&flags[0], 1);
 }
@@ -446,7 +473,7 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
         mi = (int)i;
     }
     unsigned long long nsw = __popcll(__ballot_sync(0xffffffffu, m > 1.0));
-    warp_argmax(m, mi);
+    warp_argmax_margin(m, mi);
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     if (LB == 32) {
         int blk = (int)(blockIdx.x * (int64_t)(blockDim.x >> 5) + w);
@@ -498,22 +525,59 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
 // (Eq. 3 is linear in s_k) -> margins of nbr(k) U {k} -> repair the touched leaf blocks.
 // No host round trip and no grid-wide barrier per flip.
 // ------------------------------------------------------------------------------------------------
+#ifdef FS_RELAX_PROFILE
+__device__ long long g_relax_prof[8];                  // cycles in: groups+top, update, barrier 1, leaf repair, barrier 2; flips
+#define FS_PROF_T(var) long long var = clock64()
+#define FS_PROF_ADD(slot, a, b) prof[slot] += (b) - (a)
+#else
+#define FS_PROF_T(var)
+#define FS_PROF_ADD(slot, a, b)
+#endif
+
+// The arg-max hierarchy of the relax loop works on integer keys: key(M) = bit pattern of M if M > 0,
+// else 0 (margins are -inf or >= 0, so keys order like the margins; only keys > key(1.0) can win).
+typedef unsigned long long mkey_t;
+__device__ __forceinline__ mkey_t margin_key(double m) { return m > 0.0 ? (mkey_t)__double_as_longlong(m) : 0ull; }
+constexpr mkey_t KEY_ONE = 0x3ff0000000000000ull;      // key(1.0): "L > 1" (Eq. 5) <=> key > KEY_ONE
+
+__device__ __forceinline__ void warp_argmax_key(mkey_t& key, int& i) {
+    unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
+    unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
+    unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
+    unsigned mi = __reduce_min_sync(0xffffffffu, (hi == mhi && lo == mlo) ? (unsigned)i : 0xffffffffu);
+    key = ((mkey_t)mhi << 32) | mlo;
+    i = (int)mi;
+}
+
+// arg-max of 32 consecutive leaf maxima -> group maximum (one warp)
+__device__ __forceinline__ void repair_group(int grp, int nblk, const mkey_t* bkey, const int* bidx, mkey_t* gkey, int* gidx_) {
+    int t = grp * 32 + (threadIdx.x & 31);
+    mkey_t v = t < nblk ? bkey[t] : 0ull;
+    int i = t < nblk ? bidx[t] : 0x7fffffff;
+    warp_argmax_key(v, i);
+    if ((threadIdx.x & 31) == 0) { gkey[grp] = v; gidx_[grp] = i; }
+}
+
 __global__ void __launch_bounds__(RELAX_THREADS, 1)
-k_relax(int64_t N, int Kp, int LB, int nblk, Astroid ast, long long max_flips, long long log_cap,
-        const int* __restrict__ nbr, const double2* __restrict__ wT, const double* __restrict__ hc_all,
+k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_flips, long long log_cap,
+        const int* __restrict__ nbr, const double2* __restrict__ wT, const double* __restrict__ ihc_all,
         int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, const double2* __restrict__ hfix_all,
         double* __restrict__ M_all, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
         int* __restrict__ log_all, Counters* __restrict__ ctr) {
+    // three-level arg-max hierarchy in shared memory: spins -> leaves (LB spins) -> groups (32 leaves) -> top
     extern __shared__ unsigned char smem_raw[];
-    double* bval = reinterpret_cast<double*>(smem_raw);
-    int* bidx = reinterpret_cast<int*>(bval + nblk);
-    int* touched = bidx + nblk;                       // [Kp + 1] leaf blocks touched by this flip
-    __shared__ double wv[RELAX_THREADS / 32];
-    __shared__ int wi[RELAX_THREADS / 32];
+    const int ngrp = (nblk + 31) >> 5, LB = 1 << LBshift;
+    mkey_t* bkey = reinterpret_cast<mkey_t*>(smem_raw);           // [nblk]
+    mkey_t* gkey = bkey + nblk;                                   // [ngrp]
+    int* bidx = reinterpret_cast<int*>(gkey + ngrp);              // [nblk]
+    int* gidx_ = bidx + nblk;                                     // [ngrp]
+    int* touched = gidx_ + ngrp;                                  // [Kp + 1] distinct leaf blocks touched by this flip
+    int* dirty = touched + (Kp + 1);                              // [Kp + 1] groups of the leaves repaired last
+    __shared__ int sh_k, sh_sold, sh_stop, sh_ntouched, sh_ndirty;
 
     const int r = blockIdx.x;
     const int64_t off = (int64_t)r * N;
-    const double* hc = hc_all + off;
+    const double* ihc = ihc_all + off;
     int8_t* s = s_all + off;
     double2* hdip = hdip_all + off;
     const double2* hfix = hfix_all + off;
@@ -521,84 +585,142 @@ k_relax(int64_t N, int Kp, int LB, int nblk, Astroid ast, long long max_flips, l
     int* flog = log_all + (int64_t)r * log_cap;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = RELAX_THREADS / 32;
+    const bool one_warp = (Kp + 1 <= 32);               // the whole update fits one warp: no broadcast of k needed
 
     for (int t = tid; t < nblk; t += RELAX_THREADS) {
-        bval[t] = bval_all[(int64_t)r * nblk + t];
+        bkey[t] = margin_key(bval_all[(int64_t)r * nblk + t]);
         bidx[t] = bidx_all[(int64_t)r * nblk + t];
     }
+    __syncthreads();
+    for (int g = warp; g < ngrp; g += NW) repair_group(g, nblk, bkey, bidx, gkey, gidx_);
+    if (tid == 0) { sh_stop = 0; sh_ntouched = 0; sh_ndirty = 0; }
     __syncthreads();
 
     long long nflips = 0;
     int status = 0;
+#ifdef FS_RELAX_PROFILE
+    long long prof[6] = {0, 0, 0, 0, 0, 0};
+#endif
     for (;;) {
-        // ---- A7: top-level arg-max over the leaf-block maxima
-        double v = -CUDART_INF; int k = 0x7fffffff;
-        for (int t = tid; t < nblk; t += RELAX_THREADS)
-            if (better(bval[t], bidx[t], v, k)) { v = bval[t]; k = bidx[t]; }
-        warp_argmax(v, k);
-        if (lane == 0) { wv[warp] = v; wi[warp] = k; }
-        __syncthreads();
-        v = (lane < NW) ? wv[lane] : -CUDART_INF;
-        k = (lane < NW) ? wi[lane] : 0x7fffffff;
-        warp_argmax(v, k);                              // every warp reduces the NW partials redundantly
-        if (!(v > 1.0)) break;                          // no switchable spin left
-        if (max_flips > 0 && nflips >= max_flips) { status = 1; break; }
-
-        // ---- A8: flip k, update its neighbours incrementally, recompute their margins
-        const int8_t s_old = s[k];                      // s[k] is rewritten only after the barrier below
-        const int* rowk = nbr + (int64_t)k * Kp;
-        const double2* wTk = wT + (int64_t)k * Kp;
-        int ntouch = 0;
-        for (int t = tid; t <= Kp; t += RELAX_THREADS) {
-            int blk = -1;
-            if (t == Kp) {                              // the flipped spin itself
-                double2 hd = hdip[k], hf = hfix[k];
-                M[k] = margin(hd.x + hf.x, hd.y + hf.y, -(double)s_old, hc[k], ast);
-                blk = k / LB;
-            } else {
-                int i = rowk[t];
-                if (i >= 0) {
-                    double2 wt = wTk[t];
-                    double2 hd = hdip[i], hf = hfix[i];
-                    double two_s = 2.0 * (double)s_old;
-                    hd.x -= two_s * wt.x;               // h_i -= 2 s_k,old alpha g_ik
-                    hd.y -= two_s * wt.y;
-                    hdip[i] = hd;
-                    M[i] = margin(hd.x + hf.x, hd.y + hf.y, (double)s[i], hc[i], ast);
-                    blk = i / LB;
+        FS_PROF_T(c0);
+        int k = 0, s_old = 0;
+        if (warp == 0) {
+            // ---- A7: groups of the leaves the previous flip repaired, then the top arg-max (warp 0)
+            const int nd = sh_ndirty;
+            for (int b = 0; b < nd; b += 32) {
+                int g = (b + lane < nd) ? dirty[b + lane] : -1;
+                unsigned same = __match_any_sync(0xffffffffu, g);
+                unsigned lead = __ballot_sync(0xffffffffu, g >= 0 && (__ffs(same) - 1) == lane);
+                while (lead) {
+                    int gg = __shfl_sync(0xffffffffu, g, __ffs(lead) - 1);
+                    lead &= lead - 1;
+                    repair_group(gg, nblk, bkey, bidx, gkey, gidx_);
                 }
             }
-            touched[t] = blk;
+            __syncwarp();
+            FS_PROF_T(c0b);
+            FS_PROF_ADD(5, c0, c0b);
+            mkey_t v = 0ull; k = 0x7fffffff;
+            for (int t = lane; t < ngrp; t += 32) {
+                mkey_t kv = gkey[t]; int ki = gidx_[t];
+                if (kv > v || (kv == v && ki < k)) { v = kv; k = ki; }
+            }
+            warp_argmax_key(v, k);
+            bool stop = !(v > KEY_ONE);                 // no switchable spin left
+            if (!stop && max_flips > 0 && nflips >= max_flips) { stop = true; status = 1; }
+            if (stop) k = -1;
+            if (lane == 0) { sh_k = k; sh_stop = stop ? 1 + status : 0; sh_ntouched = 0; sh_ndirty = 0; }
         }
-        (void)ntouch;
+        if (!one_warp) {
+            __syncthreads();
+            k = sh_k;
+        }
+        FS_PROF_T(c1);
+        // ---- A8: flip k, update its neighbours incrementally, recompute their margins
+        if (k >= 0 && (one_warp ? warp == 0 : true)) {
+            const int* rowk = nbr + (int64_t)k * Kp;
+            const double2* wTk = wT + (int64_t)k * Kp;
+            s_old = s[k];                               // s[k] is rewritten only after the barrier below
+            const double two_s = 2.0 * (double)s_old;
+            for (int t0 = warp * 32; t0 <= Kp; t0 += RELAX_THREADS) {
+                const int t = t0 + lane;
+                int i = -1;
+                if (t <= Kp) i = (t == Kp) ? k : rowk[t];        // entry Kp is the flipped spin itself
+                int blk = -1;
+                if (i >= 0) {
+                    double2 hd = hdip[i], hf = hfix[i];
+                    double si = (double)s[i], ih = ihc[i];
+                    if (t == Kp) si = -(double)s_old;
+                    else {
+                        double2 wt = wTk[t];
+                        hd.x -= two_s * wt.x;           // h_i -= 2 s_k,old alpha g_ik
+                        hd.y -= two_s * wt.y;
+                        hdip[i] = hd;
+                    }
+                    double m = margin(hd.x + hf.x, hd.y + hf.y, si, ih, ast);
+                    M[i] = m;
+                    blk = i >> LBshift;
+                    if (m > 1.0 && t != Kp) {           // a likely next flip: bring its ELL rows to L2 now
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(nbr + (int64_t)i * Kp));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(wT + (int64_t)i * Kp));
+                    }
+                }
+                // distinct leaf blocks of this warp's entries -> compact list (duplicates across warps are harmless)
+                unsigned same = __match_any_sync(0xffffffffu, blk);
+                bool leader = blk >= 0 && (__ffs(same) - 1) == lane;
+                unsigned lead = __ballot_sync(0xffffffffu, leader);
+                int base = 0;
+                if (lane == 0 && lead) base = one_warp ? 0 : atomicAdd(&sh_ntouched, __popc(lead));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (leader) touched[base + __popc(lead & ((1u << lane) - 1u))] = blk;
+                if (one_warp && lane == 0) sh_ntouched = __popc(lead);
+            }
+            if (warp == 0 && lane == 0) sh_sold = s_old;
+        }
+        FS_PROF_T(c2);
         __syncthreads();
+        FS_PROF_T(c3);
+        if (sh_stop) { status = sh_stop - 1; break; }
         if (tid == 0) {
-            s[k] = (int8_t)(-s_old);
-            if (nflips < log_cap) flog[nflips] = k;
+            s[sh_k] = (int8_t)(-sh_sold);
+            if (nflips < log_cap) flog[nflips] = sh_k;
         }
         // ---- A7 repair: recompute the maxima of the touched leaf blocks (one warp per block)
-        for (int t = warp; t <= Kp; t += NW) {
-            int blk = touched[t];
-            if (blk < 0) continue;
-            bool dup = false;                           // skip if an earlier entry names the same block
-            for (int u = lane; u < t; u += 32) dup |= (touched[u] == blk);
-            if (__any_sync(0xffffffffu, dup)) continue;
-            double bv = -CUDART_INF; int bi = 0x7fffffff;
-            int64_t base = (int64_t)blk * LB;
-            for (int q = lane; q < LB; q += 32) {
-                int64_t i = base + q;
-                if (i < N) { double m = M[i]; if (better(m, (int)i, bv, bi)) { bv = m; bi = (int)i; } }
+        const int ntouched = sh_ntouched;
+        for (int t = warp; t < ntouched; t += NW) {
+            const int blk = touched[t];
+            mkey_t bv = 0ull; int bi = 0x7fffffff;
+            const int64_t base = ((int64_t)blk << LBshift) + lane;
+            for (int q0 = 0; q0 < LB; q0 += 256) {              // 8 independent loads in flight per lane
+                double m[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    int64_t i = base + q0 + 32 * u;
+                    m[u] = (q0 + 32 * u < LB && i < N) ? __ldcg(M + i) : -CUDART_INF;
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    mkey_t kv = margin_key(m[u]);
+                    if (kv > bv) { bv = kv; bi = (int)(base + q0 + 32 * u); }          // ascending index: strict > keeps the lowest
+                }
             }
-            warp_argmax(bv, bi);
-            if (lane == 0) { bval[blk] = bv; bidx[blk] = bi; }
+            warp_argmax_key(bv, bi);
+            if (lane == 0) { bkey[blk] = bv; bidx[blk] = bi; dirty[atomicAdd(&sh_ndirty, 1)] = blk >> 5; }
         }
         ++nflips;
+        FS_PROF_T(c4);
         __syncthreads();
+        FS_PROF_T(c5);
+        FS_PROF_ADD(0, c0, c1); FS_PROF_ADD(1, c1, c2); FS_PROF_ADD(2, c2, c3); FS_PROF_ADD(3, c3, c4); FS_PROF_ADD(4, c4, c5);
     }
     if (tid == 0) {
         ctr[r].total_flips += nflips;
         ctr[r].last_flips = nflips;
         ctr[r].status = status;
+#ifdef FS_RELAX_PROFILE
+        for (int q = 0; q < 6; ++q) atomicAdd((unsigned long long*)&g_relax_prof[q], (unsigned long long)prof[q]);
+        atomicAdd((unsigned long long*)&g_relax_prof[6], (unsigned long long)nflips);
+#endif
     }
 }
 
@@ -1124,8 +1246,9 @@ int fetch_counters(fs_sim* sim) {
 int do_relax(fs_sim* sim, int64_t max_flips) {
     int rc = do_scan(sim, false);
     if (rc) return rc;
+    int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
     k_relax<<<sim->R, RELAX_THREADS, sim->relax_smem, sim->stream>>>(
-        sim->N, sim->Kp, sim->LB, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr,
+        sim->N, sim->Kp, lb_shift, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr,
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
@@ -1202,7 +1325,8 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     if (!sim) return fail(FS_ERR_ARG, "out of host memory");
     sim->N = N; sim->R = R; sim->K = K; sim->Kp = Kp; sim->LB = LB; sim->nblk = nblk; sim->ncells = gp.ncells;
     sim->n_inter = I; sim->log_cap = log_cap; sim->p = *p; sim->grid = gp.g; sim->stream = st;
-    sim->ast = Astroid{1.0 / p->b, 1.0 / p->c, 2.0 / p->gamma, 2.0 / p->beta};
+    auto kind = [](double denom) { return denom == 3.0 ? 1 : (denom == 2.0 ? 2 : (denom == 1.0 ? 3 : 0)); };
+    sim->ast = Astroid{1.0 / p->b, 1.0 / p->c, 2.0 / p->gamma, 2.0 / p->beta, kind(p->gamma), kind(p->beta)};
     int dev = 0; cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sim->sm_count, cudaDevAttrMultiProcessorCount, dev);
     sim->pos = (double2*)(base + L.pos); sim->cs = (double2*)(base + L.cs);
@@ -1254,7 +1378,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
         k_weights<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(N, Kp, p->alpha, sim->pos, sim->cs, sim->nbr, sim->w, sim->wT);
         LAUNCHED();
     }
-    sim->relax_smem = (size_t)nblk * 12 + (size_t)(Kp + 1) * 4 + 16;
+    sim->relax_smem = ((size_t)nblk + (size_t)(nblk + 31) / 32) * 12 + (size_t)(Kp + 1) * 8 + 32;
     CREATE_TRY(cudaFuncSetAttribute(k_relax, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
     int hflags = 0;
     CREATE_TRY(cudaMemcpyAsync(&hflags, scr + 8, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -1376,6 +1500,15 @@ int fs_measure_fp64_peak(double* dfma_per_s, void* stream) {
     *dfma_per_s = best;
     return FS_OK;
 }
+
+#ifdef FS_RELAX_PROFILE
+int fs_debug_relax_profile(long long* out8, int reset) {
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpyFromSymbol(out8, g_relax_prof, sizeof(long long) * 8));
+    if (reset) { long long z[8] = {0}; CUDA_TRY(cudaMemcpyToSymbol(g_relax_prof, z, sizeof(z))); }
+    return FS_OK;
+}
+#endif
 
 int fs_update_fields(fs_sim* sim) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
