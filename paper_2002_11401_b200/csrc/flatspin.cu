@@ -526,7 +526,7 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
 // No host round trip and no grid-wide barrier per flip.
 // ------------------------------------------------------------------------------------------------
 #ifdef FS_RELAX_PROFILE
-__device__ long long g_relax_prof[8];                  // cycles in: groups+top, update, barrier 1, leaf repair, barrier 2; flips
+__device__ long long g_relax_prof[16];                  // cycles in: groups+top, update, barrier 1, leaf repair, barrier 2; flips
 #define FS_PROF_T(var) long long var = clock64()
 #define FS_PROF_ADD(slot, a, b) prof[slot] += (b) - (a)
 #else
@@ -564,16 +564,18 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, const double2* __restrict__ hfix_all,
         double* __restrict__ M_all, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
         int* __restrict__ log_all, Counters* __restrict__ ctr) {
-    // three-level arg-max hierarchy in shared memory: spins -> leaves (LB spins) -> groups (32 leaves) -> top
+    // four-level arg-max hierarchy in shared memory:
+    // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
     extern __shared__ unsigned char smem_raw[];
-    const int ngrp = (nblk + 31) >> 5, LB = 1 << LBshift;
+    const int ngrp = (nblk + 31) >> 5, nsup = (ngrp + 31) >> 5, LB = 1 << LBshift;
     mkey_t* bkey = reinterpret_cast<mkey_t*>(smem_raw);           // [nblk]
     mkey_t* gkey = bkey + nblk;                                   // [ngrp]
-    int* bidx = reinterpret_cast<int*>(gkey + ngrp);              // [nblk]
+    mkey_t* skey = gkey + ngrp;                                   // [nsup]
+    int* bidx = reinterpret_cast<int*>(skey + nsup);              // [nblk]
     int* gidx_ = bidx + nblk;                                     // [ngrp]
-    int* touched = gidx_ + ngrp;                                  // [Kp + 1] distinct leaf blocks touched by this flip
-    int* dirty = touched + (Kp + 1);                              // [Kp + 1] groups of the leaves repaired last
-    __shared__ int sh_k, sh_sold, sh_stop, sh_ntouched, sh_ndirty;
+    int* sidx = gidx_ + ngrp;                                     // [nsup]
+    int* touched = sidx + nsup;                                   // [Kp + 1] distinct leaf blocks touched by this flip
+    __shared__ int sh_k, sh_sold, sh_stop, sh_ntouched;
 
     const int r = blockIdx.x;
     const int64_t off = (int64_t)r * N;
@@ -593,43 +595,64 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     }
     __syncthreads();
     for (int g = warp; g < ngrp; g += NW) repair_group(g, nblk, bkey, bidx, gkey, gidx_);
-    if (tid == 0) { sh_stop = 0; sh_ntouched = 0; sh_ndirty = 0; }
+    __syncthreads();
+    for (int g = warp; g < nsup; g += NW) repair_group(g, ngrp, gkey, gidx_, skey, sidx);
+    if (tid == 0) { sh_stop = 0; sh_ntouched = 0; }
     __syncthreads();
 
     long long nflips = 0;
     int status = 0;
+    int pf_prev = -1;                                   // prefetch engines: last iteration's candidate
 #ifdef FS_RELAX_PROFILE
-    long long prof[6] = {0, 0, 0, 0, 0, 0};
+    long long prof[12] = {0};
 #endif
+    int pf_row = -1, pf_done = -1;                      // prefetch engines: candidate whose row / state is in flight
+    (void)pf_prev;
+    constexpr int PF_W0 = NW / 2;                       // warps PF_W0.. are prefetch engines at the top of every iteration
     for (;;) {
         FS_PROF_T(c0);
         int k = 0, s_old = 0;
         if (warp == 0) {
-            // ---- A7: groups of the leaves the previous flip repaired, then the top arg-max (warp 0)
-            const int nd = sh_ndirty;
-            for (int b = 0; b < nd; b += 32) {
-                int g = (b + lane < nd) ? dirty[b + lane] : -1;
-                unsigned same = __match_any_sync(0xffffffffu, g);
-                unsigned lead = __ballot_sync(0xffffffffu, g >= 0 && (__ffs(same) - 1) == lane);
-                while (lead) {
-                    int gg = __shfl_sync(0xffffffffu, g, __ffs(lead) - 1);
-                    lead &= lead - 1;
-                    repair_group(gg, nblk, bkey, bidx, gkey, gidx_);
-                }
-            }
-            __syncwarp();
-            FS_PROF_T(c0b);
-            FS_PROF_ADD(5, c0, c0b);
-            mkey_t v = 0ull; k = 0x7fffffff;
-            for (int t = lane; t < ngrp; t += 32) {
-                mkey_t kv = gkey[t]; int ki = gidx_[t];
-                if (kv > v || (kv == v && ki < k)) { v = kv; k = ki; }
-            }
+            // ---- A7: top arg-max over the <= 8 supergroup maxima (warp 0)
+            mkey_t v = lane < nsup ? skey[lane] : 0ull;
+            k = lane < nsup ? sidx[lane] : 0x7fffffff;
             warp_argmax_key(v, k);
             bool stop = !(v > KEY_ONE);                 // no switchable spin left
             if (!stop && max_flips > 0 && nflips >= max_flips) { stop = true; status = 1; }
             if (stop) k = -1;
-            if (lane == 0) { sh_k = k; sh_stop = stop ? 1 + status : 0; sh_ntouched = 0; sh_ndirty = 0; }
+            if (lane == 0) { sh_k = k; sh_stop = stop ? 1 + status : 0; sh_ntouched = 0; }
+        } else if (warp >= PF_W0) {
+            // ---- prefetch engines (not on the critical path): the best spin of every 8th group is a likely
+            // future flip.  Iteration n brings its ELL row to L2; iteration n+1 reads the row (an L2 hit by
+            // then) and brings its neighbours' state, its coupling row and its own leaf of margins to L2.
+            const int e = warp - PF_W0, ne = NW - PF_W0;
+            if (pf_row >= 0) {
+                for (int t = lane; t < Kp; t += 32) {
+                    int i = __ldcg(nbr + (int64_t)pf_row * Kp + t);
+                    if (i >= 0) {
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(hdip + i));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(hfix + i));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(ihc + i));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(M + i));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(s + i));
+                    }
+                }
+                for (int t = lane * 8; t < Kp; t += 256) asm volatile("prefetch.global.L2 [%0];" ::"l"(wT + (int64_t)pf_row * Kp + t));
+                const int64_t lbase = ((int64_t)pf_row >> LBshift) << LBshift;
+                for (int q = lane * 16; q < LB; q += 512)
+                    if (lbase + q < N) asm volatile("prefetch.global.L2 [%0];" ::"l"(M + lbase + q));
+                pf_done = pf_row; pf_row = -1;
+            }
+            mkey_t v = 0ull; int c = 0x7fffffff;
+            for (int g = e + ne * lane; g < ngrp; g += ne * 32) {
+                mkey_t kv = gkey[g]; int ki = gidx_[g];
+                if (kv > v || (kv == v && ki < c)) { v = kv; c = ki; }
+            }
+            warp_argmax_key(v, c);
+            if (v > KEY_ONE && c != pf_done) {
+                for (int t = lane * 32; t < Kp; t += 1024) asm volatile("prefetch.global.L2 [%0];" ::"l"(nbr + (int64_t)c * Kp + t));
+                pf_row = c;
+            }
         }
         if (!one_warp) {
             __syncthreads();
@@ -646,6 +669,9 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
                 const int t = t0 + lane;
                 int i = -1;
                 if (t <= Kp) i = (t == Kp) ? k : rowk[t];        // entry Kp is the flipped spin itself
+#ifdef FS_RELAX_PROFILE
+                int isum = __reduce_add_sync(0xffffffffu, i + s_old); FS_PROF_T(u1); FS_PROF_ADD(6, c1, u1); if (isum == 0x7fffffff) printf("");
+#endif
                 int blk = -1;
                 if (i >= 0) {
                     double2 hd = hdip[i], hf = hfix[i];
@@ -657,9 +683,18 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
                         hd.y -= two_s * wt.y;
                         hdip[i] = hd;
                     }
+#ifdef FS_RELAX_PROFILE
+                    if (hd.x + hf.x + si + ih == 1e300) printf(""); FS_PROF_T(u2b); FS_PROF_ADD(7, u1, u2b);
+#endif
                     double m = margin(hd.x + hf.x, hd.y + hf.y, si, ih, ast);
+#ifdef FS_RELAX_PROFILE
+                    if (m == 1e300) printf(""); FS_PROF_T(u3); FS_PROF_ADD(8, u2b, u3);
+#endif
                     M[i] = m;
                     blk = i >> LBshift;
+                    // the leaf maximum can only change if i was its arg-max or reaches its value
+                    const mkey_t nk = margin_key(m);
+                    if (!(i == bidx[blk] || (nk != 0ull && nk >= bkey[blk]))) blk = -1;
                     if (m > 1.0 && t != Kp) {           // a likely next flip: bring its ELL rows to L2 now
                         asm volatile("prefetch.global.L2 [%0];" ::"l"(nbr + (int64_t)i * Kp));
                         asm volatile("prefetch.global.L2 [%0];" ::"l"(wT + (int64_t)i * Kp));
@@ -685,7 +720,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             s[sh_k] = (int8_t)(-sh_sold);
             if (nflips < log_cap) flog[nflips] = sh_k;
         }
-        // ---- A7 repair: recompute the maxima of the touched leaf blocks (one warp per block)
+        // ---- A7 repair, level by level, one warp per touched leaf (duplicated group work is harmless)
         const int ntouched = sh_ntouched;
         for (int t = warp; t < ntouched; t += NW) {
             const int blk = touched[t];
@@ -705,21 +740,27 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
                 }
             }
             warp_argmax_key(bv, bi);
-            if (lane == 0) { bkey[blk] = bv; bidx[blk] = bi; dirty[atomicAdd(&sh_ndirty, 1)] = blk >> 5; }
+            if (lane == 0) { bkey[blk] = bv; bidx[blk] = bi; }
         }
+        FS_PROF_T(c3b);
+        __syncthreads();
+        for (int t = warp; t < ntouched; t += NW) repair_group(touched[t] >> 5, nblk, bkey, bidx, gkey, gidx_);
+        __syncthreads();
+        for (int t = warp; t < ntouched; t += NW) repair_group(touched[t] >> 10, ngrp, gkey, gidx_, skey, sidx);
         ++nflips;
         FS_PROF_T(c4);
         __syncthreads();
         FS_PROF_T(c5);
         FS_PROF_ADD(0, c0, c1); FS_PROF_ADD(1, c1, c2); FS_PROF_ADD(2, c2, c3); FS_PROF_ADD(3, c3, c4); FS_PROF_ADD(4, c4, c5);
+        FS_PROF_ADD(5, c3, c3b);
     }
     if (tid == 0) {
         ctr[r].total_flips += nflips;
         ctr[r].last_flips = nflips;
         ctr[r].status = status;
 #ifdef FS_RELAX_PROFILE
-        for (int q = 0; q < 6; ++q) atomicAdd((unsigned long long*)&g_relax_prof[q], (unsigned long long)prof[q]);
-        atomicAdd((unsigned long long*)&g_relax_prof[6], (unsigned long long)nflips);
+        for (int q = 0; q < 12; ++q) atomicAdd((unsigned long long*)&g_relax_prof[q], (unsigned long long)prof[q]);
+        atomicAdd((unsigned long long*)&g_relax_prof[15], (unsigned long long)nflips);
 #endif
     }
 }
@@ -1378,7 +1419,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
         k_weights<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(N, Kp, p->alpha, sim->pos, sim->cs, sim->nbr, sim->w, sim->wT);
         LAUNCHED();
     }
-    sim->relax_smem = ((size_t)nblk + (size_t)(nblk + 31) / 32) * 12 + (size_t)(Kp + 1) * 8 + 32;
+    sim->relax_smem = ((size_t)nblk + (size_t)(nblk + 31) / 32 + 8) * 12 + (size_t)(Kp + 1) * 4 + 32;
     CREATE_TRY(cudaFuncSetAttribute(k_relax, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
     int hflags = 0;
     CREATE_TRY(cudaMemcpyAsync(&hflags, scr + 8, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -1502,10 +1543,10 @@ int fs_measure_fp64_peak(double* dfma_per_s, void* stream) {
 }
 
 #ifdef FS_RELAX_PROFILE
-int fs_debug_relax_profile(long long* out8, int reset) {
+int fs_debug_relax_profile(long long* out16, int reset) {
     CUDA_TRY(cudaDeviceSynchronize());
-    CUDA_TRY(cudaMemcpyFromSymbol(out8, g_relax_prof, sizeof(long long) * 8));
-    if (reset) { long long z[8] = {0}; CUDA_TRY(cudaMemcpyToSymbol(g_relax_prof, z, sizeof(z))); }
+    CUDA_TRY(cudaMemcpyFromSymbol(out16, g_relax_prof, sizeof(long long) * 16));
+    if (reset) { long long z[16] = {0}; CUDA_TRY(cudaMemcpyToSymbol(g_relax_prof, z, sizeof(z))); }
     return FS_OK;
 }
 #endif
