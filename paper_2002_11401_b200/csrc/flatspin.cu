@@ -91,15 +91,6 @@ __device__ __forceinline__ bool better(double va, int ia, double vb, int ib) {
     return (va > vb) || (va == vb && ia < ib);
 }
 
-__device__ __forceinline__ void warp_argmax(double& v, int& i) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        double ov = __shfl_xor_sync(0xffffffffu, v, o);
-        int oi = __shfl_xor_sync(0xffffffffu, i, o);
-        if (better(ov, oi, v, i)) { v = ov; i = oi; }
-    }
-}
-
 // Philox4x32-10 (Salmon et al. SC'11), restated for the device.  counter = (spin, step, 0, 0),
 // key = (seed_lo, seed_hi)  (reading C-11).
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -443,7 +434,7 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
                                                const int8_t* __restrict__ s_all, const double2* __restrict__ hdip_all,
                                                double2* __restrict__ hfix_all, double* __restrict__ M_all,
                                                double* __restrict__ bval_all, int* __restrict__ bidx_all, int nblk,
-                                               Counters* __restrict__ ctr) {
+                                               unsigned* __restrict__ scnt_all /*[R][gridDim.x]*/, Counters* __restrict__ ctr) {
     __shared__ double wv[32];
     __shared__ int wi[32];
     __shared__ int is_last;
@@ -490,31 +481,58 @@ __global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, F
         }
     }
     if (!finalize) return;
-    // A7 top level (fs_scan only): the last CTA of this replica to finish reduces the leaf maxima
-    if (lane == 0 && nsw) atomicAdd(&ctr[r].acc_switch, nsw);
-    __threadfence();
+    // A7 top level (fs_scan only): the last CTA of this replica to finish reduces the leaf maxima and the
+    // per-CTA counts of switchable spins (one ticket atomic per CTA; everything else is plain stores)
+    __shared__ unsigned wcnt[32];
+    if (lane == 0) wcnt[w] = (unsigned)nsw;
     __syncthreads();
-    if (threadIdx.x == 0) is_last = (atomicAdd(&ctr[r].ticket, 1u) == gridDim.x - 1);
+    if (threadIdx.x == 0) {
+        unsigned c = 0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) c += wcnt[k];
+        scnt_all[(int64_t)r * gridDim.x + blockIdx.x] = c;
+        __threadfence();
+        is_last = (atomicAdd(&ctr[r].ticket, 1u) == gridDim.x - 1);
+    }
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    const volatile double* bval = bval_all + (int64_t)r * nblk;
-    const volatile int* bidx = bidx_all + (int64_t)r * nblk;
+    const double* bval = bval_all + (int64_t)r * nblk;
+    const int* bidx = bidx_all + (int64_t)r * nblk;
     double v = -CUDART_INF; int bi = 0x7fffffff;
-    for (int t = threadIdx.x; t < nblk; t += blockDim.x) {
-        double tv = bval[t]; int ti = bidx[t];
-        if (better(tv, ti, v, bi)) { v = tv; bi = ti; }
+    for (int t0 = threadIdx.x; t0 < nblk; t0 += 8 * blockDim.x) {           // 8 independent loads in flight per thread
+        double tv[8]; int ti[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            int t = t0 + u * blockDim.x;
+            tv[u] = t < nblk ? __ldcg(bval + t) : -CUDART_INF;
+            ti[u] = t < nblk ? __ldcg(bidx + t) : 0x7fffffff;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) if (better(tv[u], ti[u], v, bi)) { v = tv[u]; bi = ti[u]; }
     }
-    warp_argmax(v, bi);
+    unsigned long long cnt = 0;
+    for (int t0 = threadIdx.x; t0 < (int)gridDim.x; t0 += 8 * blockDim.x) {
+        unsigned cv[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) { int t = t0 + u * blockDim.x; cv[u] = t < (int)gridDim.x ? __ldcg(scnt_all + (int64_t)r * gridDim.x + t) : 0u; }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) cnt += cv[u];
+    }
+    warp_argmax_margin(v, bi);
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    __shared__ unsigned long long wc[32];
     __syncthreads();                                     // wv/wi are reused
-    if (lane == 0) { wv[w] = v; wi[w] = bi; }
+    if (lane == 0) { wv[w] = v; wi[w] = bi; wc[w] = cnt; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        for (int k = 1; k < (int)(blockDim.x >> 5); ++k) if (better(wv[k], wi[k], v, bi)) { v = wv[k]; bi = wi[k]; }
+        for (int k = 1; k < (int)(blockDim.x >> 5); ++k) {
+            if (better(wv[k], wi[k], v, bi)) { v = wv[k]; bi = wi[k]; }
+            cnt += wc[k];
+        }
         bool any = v > 1.0;
         ctr[r].best_index = any ? bi : -1;
         ctr[r].best_L = any ? v : -CUDART_INF;
-        ctr[r].n_switchable = (long long)atomicExch(&ctr[r].acc_switch, 0ull);
+        ctr[r].n_switchable = (long long)cnt;
         ctr[r].ticket = 0u;
     }
 }
@@ -563,7 +581,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         const int* __restrict__ nbr, const double2* __restrict__ wT, const double* __restrict__ ihc_all,
         int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, const double2* __restrict__ hfix_all,
         double* __restrict__ M_all, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
-        int* __restrict__ log_all, Counters* __restrict__ ctr) {
+        int* __restrict__ log_all, Counters* __restrict__ ctr,
+        const int* __restrict__ cellidx /*NULL: no lattice*/, uint16_t* __restrict__ sgrid, int64_t sgrid_stride) {
     // four-level arg-max hierarchy in shared memory:
     // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
     extern __shared__ unsigned char smem_raw[];
@@ -720,6 +739,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             s[sh_k] = (int8_t)(-sh_sold);
             if (nflips < log_cap) flog[nflips] = sh_k;
         }
+        if (tid == RELAX_THREADS - 32 && cellidx)           // keep the stencil gather's spin grid in step (an idle warp)
+            sgrid[(int64_t)r * sgrid_stride + cellidx[sh_k]] = (uint16_t)(sh_sold > 0 ? 0xbff0 : 0x3ff0);
         // ---- A7 repair, level by level, one warp per touched leaf (duplicated group work is harmless)
         const int ntouched = sh_ntouched;
         for (int t = warp; t < ntouched; t += NW) {
@@ -819,7 +840,7 @@ struct fs_sim {
     int *nbr = nullptr, *deg = nullptr;
     // per replica
     double* hc = nullptr; int8_t* s = nullptr; double2 *hdip = nullptr, *hfix = nullptr; double* M = nullptr;
-    double* bval = nullptr; int* bidx = nullptr; int* flog = nullptr; Counters* ctr = nullptr;
+    double* bval = nullptr; int* bidx = nullptr; unsigned* scnt = nullptr; int* flog = nullptr; Counters* ctr = nullptr;
     double2* hext = nullptr;     // [R] device copy of the global field
     // state
     bool fields_dirty = true;
@@ -836,7 +857,7 @@ struct fs_sim {
     void* lat_mem = nullptr;        // sub | cu | cv
     void* st_mem = nullptr;         // gidx | T | owner | rowtab | scratch
     uint8_t* lat_sub = nullptr; int *lat_cu = nullptr, *lat_cv = nullptr;
-    uint16_t* sgrid = nullptr;
+    uint16_t* sgrid = nullptr; int* cellidx = nullptr; bool sgrid_valid = false;
     int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
     int st_nw = 4, st_rs = 1, st_pv = 0; size_t st_smem = 0; bool st_ct = false;
     unsigned long long st_id = 0;   // identity for the ownership of the constant-memory table
@@ -855,7 +876,7 @@ struct Layout {
     size_t scratch, cell_of, cell_cnt, cell_start, cell_fill, items, deg;
     size_t grid_end;
     // K-dependent
-    size_t pos, cs, nbr, w, wT, hc, s, hdip, hfix, M, bval, bidx, flog, ctr, hext, total;
+    size_t pos, cs, nbr, w, wT, hc, s, hdip, hfix, M, bval, bidx, scnt, flog, ctr, hext, total;
 };
 
 int choose_leaf(int64_t N, int* LB, int* nblk) {
@@ -896,6 +917,7 @@ void layout_rest(Layout& L, int64_t N, int R, int Kp, int nblk, int64_t log_cap)
     L.bval = take(8 * (size_t)R * nblk);
     L.bidx = take(4 * (size_t)R * nblk);
     L.flog = take(4 * (size_t)R * log_cap);
+    L.scnt = take(4 * (size_t)R * (size_t)((N + SCAN_THREADS - 1) / SCAN_THREADS));
     L.ctr = take(sizeof(Counters) * (size_t)R);
     L.hext = take(16 * (size_t)R);
     L.total = o;
@@ -978,8 +1000,11 @@ int do_gather_stencil(fs_sim* sim) {
     const LatGrid& g = sim->lg;
     int TV = ST_OV * sim->st_nw;
     dim3 sgrid((unsigned)((g.Up + 31) / 32), (unsigned)((g.Vp + 31) / 32), (unsigned)g.nsub);
-    k_spin_grid<<<sgrid, 256, 0, sim->stream>>>(sim->N, g, sim->R, sim->gidx, sim->s, sim->sgrid);
-    LAUNCHED();
+    if (!sim->sgrid_valid) {                             // the relax loop keeps the grids in step with its flips
+        k_spin_grid<<<sgrid, 256, 0, sim->stream>>>(sim->N, g, sim->R, sim->gidx, sim->s, sim->sgrid);
+        LAUNCHED();
+        sim->sgrid_valid = true;
+    }
     dim3 grid((unsigned)((g.U + ST_TU - 1) / ST_TU), (unsigned)((g.V + TV - 1) / TV), (unsigned)(g.nsub * sim->R));
     int threads = 32 * sim->st_nw * sim->st_rs;
 #define FS_LAUNCH_STENCIL(MAXT, MINB, CTV)                                                          \
@@ -1214,17 +1239,17 @@ int detect_lattice(fs_sim* sim) {
     size_t slots = (size_t)nsub * nsub * wh;
     size_t o_gidx = 0, o_T = align_up(4 * (size_t)cells), o_owner = o_T + align_up(16 * slots),
            o_rows = o_owner + align_up(8 * slots), o_sg = o_rows + align_up(8 * (size_t)nsub * nsub * g.W),
-           o_end = o_sg + align_up(sg_bytes);
+           o_cell = o_sg + align_up(sg_bytes), o_end = o_cell + align_up(4 * (size_t)N);
     CUDA_TRY(cudaMalloc(&sim->st_mem, o_end));
     unsigned char* sb = (unsigned char*)sim->st_mem;
     sim->gidx = (int*)(sb + o_gidx); sim->T = (double2*)(sb + o_T); sim->owner = (unsigned long long*)(sb + o_owner);
-    sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (uint16_t*)(sb + o_sg);
+    sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (uint16_t*)(sb + o_sg); sim->cellidx = (int*)(sb + o_cell);
     CUDA_TRY(cudaMemsetAsync(sim->sgrid, 0, sg_bytes, st));
     CUDA_TRY(cudaMemsetAsync(sim->gidx, 0xff, 4 * (size_t)cells, st));
     CUDA_TRY(cudaMemsetAsync(sim->T, 0, 16 * slots, st));
     CUDA_TRY(cudaMemsetAsync(sim->owner, 0xff, 8 * slots, st));
     CUDA_TRY(cudaMemsetAsync(scr, 0, 4, st));                                      // flags
-    k_lat_scatter<<<nb256, 256, 0, st>>>(N, g, sim->lat_sub, sim->lat_cu, sim->lat_cv, sim->gidx, scr); LAUNCHED();
+    k_lat_scatter<<<nb256, 256, 0, st>>>(N, g, sim->lat_sub, sim->lat_cu, sim->lat_cv, sim->gidx, sim->cellidx, scr); LAUNCHED();
     for (int mode = 0; mode < 3; ++mode) {
         k_stencil_build<<<nbk, 256, 0, st>>>(mode, N, Kp, g, sim->nbr, sim->w, sim->lat_sub, sim->lat_cu, sim->lat_cv,
                                              sim->owner, sim->T, scr64 + 1); LAUNCHED();
@@ -1267,7 +1292,7 @@ int do_scan(fs_sim* sim, bool finalize) {
     dim3 grid((unsigned)((sim->N + threads - 1) / threads), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
     k_scan<<<grid, threads, 0, sim->stream>>>(sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc,
-                                               sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->ctr);
+                                               sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -1290,7 +1315,9 @@ int do_relax(fs_sim* sim, int64_t max_flips) {
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
     k_relax<<<sim->R, RELAX_THREADS, sim->relax_smem, sim->stream>>>(
         sim->N, sim->Kp, lb_shift, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr,
-        sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr);
+        sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr,
+        sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid,
+        sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -1376,6 +1403,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     sim->hc = (double*)(base + L.hc); sim->s = (int8_t*)(base + L.s);
     sim->hdip = (double2*)(base + L.hdip); sim->hfix = (double2*)(base + L.hfix); sim->M = (double*)(base + L.M);
     sim->bval = (double*)(base + L.bval); sim->bidx = (int*)(base + L.bidx); sim->flog = (int*)(base + L.flog);
+    sim->scnt = (unsigned*)(base + L.scnt);
     sim->ctr = (Counters*)(base + L.ctr); sim->hext = (double2*)(base + L.hext);
 
 #define CREATE_TRY(expr)                                                                           \
@@ -1461,7 +1489,7 @@ int fs_get_info(const fs_sim* sim, int64_t* N, int32_t* R, int32_t* K, int64_t* 
 int fs_set_spins(fs_sim* sim, const int8_t* s_dev) {
     if (!sim || !s_dev) return fail(FS_ERR_ARG, "null pointer");
     CUDA_TRY(cudaMemcpyAsync(sim->s, s_dev, (size_t)sim->R * sim->N, cudaMemcpyDeviceToDevice, sim->stream));
-    sim->fields_dirty = true;
+    sim->fields_dirty = true; sim->sgrid_valid = false;
     return FS_OK;
 }
 
@@ -1664,7 +1692,7 @@ int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t*
     if (!sim || !s_host || !h_host_out) return fail(FS_ERR_ARG, "null pointer");
     size_t rn = (size_t)sim->R * sim->N;
     CUDA_TRY(cudaMemcpyAsync(sim->s, s_host, rn, cudaMemcpyHostToDevice, sim->stream));
-    sim->fields_dirty = true;
+    sim->fields_dirty = true; sim->sgrid_valid = false;
     int rc = do_gather(sim);
     if (rc) return rc;
     rc = fs_scan_ensemble(sim, nullptr, nullptr, nullptr);

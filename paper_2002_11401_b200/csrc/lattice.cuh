@@ -108,11 +108,13 @@ __device__ __forceinline__ int64_t lat_cell(const LatGrid& g, int sub, int cu, i
     return ((int64_t)sub * g.Vp + (cv - g.v0 + g.Rv)) * g.Up + (cu - g.u0 + g.Ru);
 }
 
-// flags bit 2: two spins in one cell
+// flags bit 2: two spins in one cell.  cellidx[i] = position of spin i in one replica's spin grid sg[sub][Upa][Vpa].
 __global__ void k_lat_scatter(int64_t N, LatGrid g, const uint8_t* __restrict__ sub, const int* __restrict__ cu,
-                              const int* __restrict__ cv, int* __restrict__ gidx, int* __restrict__ flags) {
+                              const int* __restrict__ cv, int* __restrict__ gidx, int* __restrict__ cellidx,
+                              int* __restrict__ flags) {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= N) return;
+    cellidx[i] = (int)(((int64_t)sub[i] * g.Upa + (cu[i] - g.u0 + g.Ru)) * g.Vpa + (cv[i] - g.v0 + g.Rv));
     if (atomicCAS(&gidx[lat_cell(g, sub[i], cu[i], cv[i])], -1, (int)i) != -1) atomicOr(flags, 4);
 }
 

@@ -184,6 +184,26 @@ def test_partially_jittered_lattice_is_caught_by_verification(B):
     assert not lat["active"] and lat["reason"] == 8, lat
 
 
+def test_spin_grid_follows_relax(B):
+    """The stencil gather reads dense spin grids that the relax loop keeps in step with its flips: a
+    fresh stencil gather after relaxations must equal the oracle's recomputed fields (and the ELL gather)."""
+    w = W.config("4", scale=40)
+    sim, orc = mk(B, w)
+    assert sim.lattice()["active"]
+    sim.update_fields()                                   # builds the grids
+    for t in (0, 150, 160, 165, 170, 180, 200):
+        hx, hy = w.fields[t]
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        assert sim.relax() == orc.relax_B()[0]
+        sim.set_gather_variant(B.GATHER_STENCIL); sim.update_fields()
+        a = sim.get_fields(1).cpu().numpy()
+        assert field_err(a, orc.fields(1)) < FIELD_TOL
+        sim.set_gather_variant(B.GATHER_ELL_F64); sim.update_fields()
+        assert field_err(sim.get_fields(1).cpu().numpy(), a) < FIELD_TOL
+        sim.set_gather_variant(B.GATHER_AUTO)
+    assert int((sim.get_spins() == -1).sum()) > 0
+
+
 def test_stencil_ensemble_matches_ell(B):
     w = W.config("5", scale=30)
     R = 3
