@@ -428,55 +428,67 @@ __global__ void __launch_bounds__(256) k_gather(int64_t N, int Kp, const int* __
 // ------------------------------------------------------------------------------------------------
 struct FieldSpec { double sigma; uint64_t seed; uint32_t step; };
 
-__global__ void __launch_bounds__(1024) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs, int finalize,
+constexpr int SCAN_SPT = 4;                             // spins per thread: four independent load chains in flight
+constexpr int SCAN_SPB = SCAN_THREADS * SCAN_SPT;       // 1024 consecutive spins per CTA = 1024 / LB leaves
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs, int finalize,
                                                const double2* __restrict__ hext_all /*[R] (hx,hy)*/,
                                                const double2* __restrict__ cs, const double* __restrict__ hc_all,
                                                const int8_t* __restrict__ s_all, const double2* __restrict__ hdip_all,
                                                double2* __restrict__ hfix_all, double* __restrict__ M_all,
                                                double* __restrict__ bval_all, int* __restrict__ bidx_all, int nblk,
                                                unsigned* __restrict__ scnt_all /*[R][gridDim.x]*/, Counters* __restrict__ ctr) {
-    __shared__ double wv[32];
+    __shared__ double wv[32];                            // arg-max of every 32-spin slot of this CTA
     __shared__ int wi[32];
     __shared__ int is_last;
-    int r = blockIdx.y;
-    int64_t off = (int64_t)r * N;
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    double m = -CUDART_INF; int mi = 0x7fffffff;
-    if (i < N) {
-        double2 c = cs[i];
-        double2 he = hext_all[r];
-        double ex = he.x, ey = he.y;
-        double2 hf;
-        if (fs.sigma != 0.0) {
-            double2 t = thermal_xy(fs.sigma, fs.seed + (uint64_t)r, fs.step, (uint32_t)i);
-            // (ext + th) rotated together would round differently from the paper's sum of three fields;
-            // rotate separately and add (Eq. 2)
-            double tp = t.x * c.x + t.y * c.y, tq = -t.x * c.y + t.y * c.x;
-            double ep = ex * c.x + ey * c.y, eq = -ex * c.y + ey * c.x;
-            hf = make_double2(ep + tp, eq + tq);
-        } else {
-            hf = make_double2(ex * c.x + ey * c.y, -ex * c.y + ey * c.x);
-        }
-        hfix_all[off + i] = hf;
-        double2 hd = hdip_all[off + i];
-        m = margin(hd.x + hf.x, hd.y + hf.y, (double)s_all[off + i], hc_all[off + i], ast);
-        M_all[off + i] = m;
-        mi = (int)i;
+    const int r = blockIdx.y;
+    const int64_t off = (int64_t)r * N;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t base = (int64_t)blockIdx.x * SCAN_SPB + threadIdx.x;
+    const double2 he = hext_all[r];
+    // loads of all four spins first
+    double2 c[SCAN_SPT], hd[SCAN_SPT]; double ih[SCAN_SPT], sp[SCAN_SPT];
+#pragma unroll
+    for (int q = 0; q < SCAN_SPT; ++q) {
+        const int64_t i = base + q * SCAN_THREADS;
+        if (i < N) { c[q] = cs[i]; hd[q] = hdip_all[off + i]; ih[q] = hc_all[off + i]; sp[q] = (double)s_all[off + i]; }
+        else { c[q] = make_double2(1.0, 0.0); hd[q] = make_double2(0.0, 0.0); ih[q] = 1.0; sp[q] = 1.0; }
     }
-    unsigned long long nsw = __popcll(__ballot_sync(0xffffffffu, m > 1.0));
-    warp_argmax_margin(m, mi);
-    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (LB == 32) {
-        int blk = (int)(blockIdx.x * (int64_t)(blockDim.x >> 5) + w);
-        if (lane == 0 && blk < nblk) { bval_all[(int64_t)r * nblk + blk] = m; bidx_all[(int64_t)r * nblk + blk] = mi; }
-    } else {
-        if (lane == 0) { wv[w] = m; wi[w] = mi; }
-        __syncthreads();
-        int wpl = LB >> 5;                               // warps per leaf block
-        if (lane == 0 && (w % wpl) == 0) {
-            double bv = wv[w]; int bi = wi[w];
-            for (int k = 1; k < wpl; ++k) if (better(wv[w + k], wi[w + k], bv, bi)) { bv = wv[w + k]; bi = wi[w + k]; }
-            int blk = (int)((blockIdx.x * (int64_t)blockDim.x + threadIdx.x) / LB);
+    unsigned long long nsw = 0;
+#pragma unroll
+    for (int q = 0; q < SCAN_SPT; ++q) {
+        const int64_t i = base + q * SCAN_THREADS;
+        double m = -CUDART_INF; int mi = 0x7fffffff;
+        if (i < N) {
+            const double ex = he.x, ey = he.y;
+            double2 hf;
+            if (fs.sigma != 0.0) {
+                double2 t = thermal_xy(fs.sigma, fs.seed + (uint64_t)r, fs.step, (uint32_t)i);
+                // (ext + th) rotated together would round differently from the paper's sum of three fields;
+                // rotate separately and add (Eq. 2)
+                double tp = t.x * c[q].x + t.y * c[q].y, tq = -t.x * c[q].y + t.y * c[q].x;
+                double ep = ex * c[q].x + ey * c[q].y, eq = -ex * c[q].y + ey * c[q].x;
+                hf = make_double2(ep + tp, eq + tq);
+            } else {
+                hf = make_double2(ex * c[q].x + ey * c[q].y, -ex * c[q].y + ey * c[q].x);
+            }
+            hfix_all[off + i] = hf;
+            m = margin(hd[q].x + hf.x, hd[q].y + hf.y, sp[q], ih[q], ast);
+            M_all[off + i] = m;
+            mi = (int)i;
+        }
+        nsw += __popc(__ballot_sync(0xffffffffu, m > 1.0));
+        warp_argmax_margin(m, mi);
+        if (lane == 0) { wv[q * (SCAN_THREADS / 32) + w] = m; wi[q * (SCAN_THREADS / 32) + w] = mi; }   // slot = spin offset / 32
+    }
+    __syncthreads();
+    {
+        const int spl = LB >> 5, nleaf = SCAN_SPB / LB;  // 32-spin slots per leaf; leaves per CTA
+        if ((int)threadIdx.x < nleaf) {
+            const int s0 = threadIdx.x * spl;
+            double bv = wv[s0]; int bi = wi[s0];
+            for (int k = 1; k < spl; ++k) if (better(wv[s0 + k], wi[s0 + k], bv, bi)) { bv = wv[s0 + k]; bi = wi[s0 + k]; }
+            const int blk = blockIdx.x * nleaf + threadIdx.x;
             if (blk < nblk) { bval_all[(int64_t)r * nblk + blk] = bv; bidx_all[(int64_t)r * nblk + blk] = bi; }
         }
     }
@@ -1288,10 +1300,9 @@ int ensure_fields(fs_sim* sim) { return sim->fields_dirty ? do_gather(sim) : FS_
 int do_scan(fs_sim* sim, bool finalize) {
     int rc = ensure_fields(sim);
     if (rc) return rc;
-    int threads = sim->LB > SCAN_THREADS ? sim->LB : SCAN_THREADS;
-    dim3 grid((unsigned)((sim->N + threads - 1) / threads), (unsigned)sim->R);
+    dim3 grid((unsigned)((sim->N + SCAN_SPB - 1) / SCAN_SPB), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
-    k_scan<<<grid, threads, 0, sim->stream>>>(sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc,
+    k_scan<<<grid, SCAN_THREADS, 0, sim->stream>>>(sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc,
                                                sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
