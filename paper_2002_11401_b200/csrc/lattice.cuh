@@ -77,30 +77,34 @@ __global__ void k_lat_extent(int64_t N, int Kp, const int* __restrict__ nbr, con
                              const int* __restrict__ cu, const int* __restrict__ cv, int* __restrict__ ext,
                              unsigned long long* __restrict__ wmax) {
     int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    int ru = 0, rv = 0;
+    int ru = 0, rv = 0, ulo = 0x7fffffff, vlo = 0x7fffffff, uhi = (int)0x80000000, vhi = (int)0x80000000;
     double wm = 0.0;
     if (t < N * Kp) {
         int64_t i = t / Kp;
         int j = nbr[t];
+        int ui = cu[i], vi = cv[i];
         if (j >= 0) {
-            ru = abs(cu[j] - cu[i]); rv = abs(cv[j] - cv[i]);
+            ru = abs(cu[j] - ui); rv = abs(cv[j] - vi);
             double2 ww = w[t];
             wm = fmax(fabs(ww.x), fabs(ww.y));
         }
-        if (t % Kp == 0) {
-            atomicMin(&ext[0], cu[i]); atomicMin(&ext[1], cv[i]);
-            atomicMax(&ext[2], cu[i]); atomicMax(&ext[3], cv[i]);
-        }
+        ulo = uhi = ui; vlo = vhi = vi;
     }
-    for (int o = 16; o > 0; o >>= 1) {
-        ru = max(ru, __shfl_xor_sync(0xffffffffu, ru, o));
-        rv = max(rv, __shfl_xor_sync(0xffffffffu, rv, o));
-        wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
-    }
+    // one set of atomics per warp, and only if it can change the result (plain reads first)
+    ru = __reduce_max_sync(0xffffffffu, ru); rv = __reduce_max_sync(0xffffffffu, rv);
+    ulo = __reduce_min_sync(0xffffffffu, ulo); vlo = __reduce_min_sync(0xffffffffu, vlo);
+    uhi = __reduce_max_sync(0xffffffffu, uhi); vhi = __reduce_max_sync(0xffffffffu, vhi);
+    for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
     if ((threadIdx.x & 31) == 0) {
-        if (ru) atomicMax(&ext[4], ru);
-        if (rv) atomicMax(&ext[5], rv);
-        if (wm > 0.0) atomicMax(wmax, (unsigned long long)__double_as_longlong(wm));
+        volatile int* e = ext;
+        if (ulo < e[0]) atomicMin(&ext[0], ulo);
+        if (vlo < e[1]) atomicMin(&ext[1], vlo);
+        if (uhi > e[2]) atomicMax(&ext[2], uhi);
+        if (vhi > e[3]) atomicMax(&ext[3], vhi);
+        if (ru > e[4]) atomicMax(&ext[4], ru);
+        if (rv > e[5]) atomicMax(&ext[5], rv);
+        unsigned long long wb = (unsigned long long)__double_as_longlong(wm);
+        if (wb > *(volatile unsigned long long*)wmax) atomicMax(wmax, wb);
     }
 }
 
@@ -136,14 +140,15 @@ __global__ void k_stencil_build(int mode, int64_t N, int Kp, LatGrid g, const in
         int j = nbr[t];
         if (j >= 0) {
             int64_t slot = stencil_slot(g, sub[i], sub[j], cu[j] - cu[i], cv[j] - cv[i]);
-            if (mode == 0) atomicMin(&owner[slot], (unsigned long long)t);
+            if (mode == 0) { if (*(volatile unsigned long long*)(owner + slot) > (unsigned long long)t) atomicMin(&owner[slot], (unsigned long long)t); }
             else if (mode == 1) { if (owner[slot] == (unsigned long long)t) T[slot] = w[t]; }
             else { double2 a = w[t], b = T[slot]; d = fmax(fabs(a.x - b.x), fabs(a.y - b.y)); }
         }
     }
     if (mode == 2) {
         for (int o = 16; o > 0; o >>= 1) d = fmax(d, __shfl_xor_sync(0xffffffffu, d, o));
-        if ((threadIdx.x & 31) == 0 && d > 0.0) atomicMax(dev, (unsigned long long)__double_as_longlong(d));
+        if ((threadIdx.x & 31) == 0 && d > 0.0 && (unsigned long long)__double_as_longlong(d) > *(volatile unsigned long long*)dev)
+            atomicMax(dev, (unsigned long long)__double_as_longlong(d));
     }
 }
 
