@@ -62,7 +62,6 @@ int fail(int code, const char* fmt, ...) {
 constexpr int RELAX_THREADS = 512;
 constexpr int MAX_LEAF_BLOCKS = 8192;   // leaf-block maxima kept in the relax CTA's shared memory
 constexpr int MAX_K = 8192;             // maximum degree supported by the warp bitonic sort
-constexpr int SCAN_THREADS = 256;
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
@@ -428,10 +427,18 @@ __global__ void __launch_bounds__(256) k_gather(int64_t N, int Kp, const int* __
 // ------------------------------------------------------------------------------------------------
 struct FieldSpec { double sigma; uint64_t seed; uint32_t step; };
 
-constexpr int SCAN_SPT = 4;                             // spins per thread: four independent load chains in flight
-constexpr int SCAN_SPB = SCAN_THREADS * SCAN_SPT;       // 1024 consecutive spins per CTA = 1024 / LB leaves
+struct ScanGroup { double v; int idx; unsigned cnt; };  // result of one group of 32 scan CTAs
+// uint32 words of scan scratch per replica: per-CTA counts, group tickets, group results
+__host__ __device__ inline size_t scan_aux_stride(int ncta) {
+    int ngroups = (ncta + 31) >> 5;
+    return (size_t)((ncta + ngroups + 3) & ~3) + 4 * (size_t)ngroups;
+}
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs, int finalize,
+constexpr int SCAN_SPB = 1024;                          // consecutive spins per CTA = 1024 / LB leaves
+
+// THREADS x SPT = 1024: SPT spins per thread (independent load chains in flight)
+template <int SCAN_SPT>
+__global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs, int finalize,
                                                const double2* __restrict__ hext_all /*[R] (hx,hy)*/,
                                                const double2* __restrict__ cs, const double* __restrict__ hc_all,
                                                const int8_t* __restrict__ s_all, const double2* __restrict__ hdip_all,
@@ -444,6 +451,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(int64_t N, int LB, Astroi
     const int r = blockIdx.y;
     const int64_t off = (int64_t)r * N;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    constexpr int SCAN_THREADS = SCAN_SPB / SCAN_SPT;
     const int64_t base = (int64_t)blockIdx.x * SCAN_SPB + threadIdx.x;
     const double2 he = hext_all[r];
     // loads of all four spins first
@@ -493,54 +501,75 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(int64_t N, int LB, Astroi
         }
     }
     if (!finalize) return;
-    // A7 top level (fs_scan only): the last CTA of this replica to finish reduces the leaf maxima and the
-    // per-CTA counts of switchable spins (one ticket atomic per CTA; everything else is plain stores)
+    // A7 top level (fs_scan only), two-level "last one out" reduction so that no CTA has a long serial tail:
+    // CTAs form groups of 32; the last CTA of a group to finish reduces the group's leaf maxima and
+    // switchable counts; the last group to finish reduces the <= 64 group results.  One ticket atomic per
+    // CTA and one per group; everything else is plain stores + fences.
     __shared__ unsigned wcnt[32];
+    __shared__ unsigned long long wc[32];
+    const int ncta = gridDim.x, ngroups = (ncta + 31) >> 5, g = blockIdx.x >> 5;
+    unsigned* scnt = scnt_all + (int64_t)r * scan_aux_stride(ncta);           // [ncta] per-CTA counts
+    unsigned* gticket = scnt + ncta;                                           // [ngroups]
+    ScanGroup* gres = reinterpret_cast<ScanGroup*>(scnt + ((ncta + ngroups + 3) & ~3));   // [ngroups], 16-byte aligned
     if (lane == 0) wcnt[w] = (unsigned)nsw;
     __syncthreads();
     if (threadIdx.x == 0) {
         unsigned c = 0;
-        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) c += wcnt[k];
-        scnt_all[(int64_t)r * gridDim.x + blockIdx.x] = c;
+        for (int k = 0; k < SCAN_THREADS / 32; ++k) c += wcnt[k];
+        scnt[blockIdx.x] = c;
         __threadfence();
-        is_last = (atomicAdd(&ctr[r].ticket, 1u) == gridDim.x - 1);
+        is_last = (atomicAdd(&gticket[g], 1u) == (unsigned)(min(32, ncta - 32 * g) - 1));
     }
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    const double* bval = bval_all + (int64_t)r * nblk;
-    const int* bidx = bidx_all + (int64_t)r * nblk;
     double v = -CUDART_INF; int bi = 0x7fffffff;
-    for (int t0 = threadIdx.x; t0 < nblk; t0 += 8 * blockDim.x) {           // 8 independent loads in flight per thread
-        double tv[8]; int ti[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            int t = t0 + u * blockDim.x;
-            tv[u] = t < nblk ? __ldcg(bval + t) : -CUDART_INF;
-            ti[u] = t < nblk ? __ldcg(bidx + t) : 0x7fffffff;
-        }
-#pragma unroll
-        for (int u = 0; u < 8; ++u) if (better(tv[u], ti[u], v, bi)) { v = tv[u]; bi = ti[u]; }
-    }
     unsigned long long cnt = 0;
-    for (int t0 = threadIdx.x; t0 < (int)gridDim.x; t0 += 8 * blockDim.x) {
-        unsigned cv[8];
+    {
+        const int nleaf = SCAN_SPB / LB;
+        const int b0 = 32 * g * nleaf, b1 = min(nblk, 32 * (g + 1) * nleaf);
+        const double* bval = bval_all + (int64_t)r * nblk;
+        const int* bidx = bidx_all + (int64_t)r * nblk;
+        for (int t0 = b0 + threadIdx.x; t0 < b1; t0 += 4 * SCAN_THREADS) {     // <= 1024 leaves: one batch of 4 loads
+            double tv[4]; int ti[4];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) { int t = t0 + u * blockDim.x; cv[u] = t < (int)gridDim.x ? __ldcg(scnt_all + (int64_t)r * gridDim.x + t) : 0u; }
+            for (int u = 0; u < 4; ++u) {
+                int t = t0 + u * SCAN_THREADS;
+                tv[u] = t < b1 ? __ldcg(bval + t) : -CUDART_INF;
+                ti[u] = t < b1 ? __ldcg(bidx + t) : 0x7fffffff;
+            }
 #pragma unroll
-        for (int u = 0; u < 8; ++u) cnt += cv[u];
+            for (int u = 0; u < 4; ++u) if (better(tv[u], ti[u], v, bi)) { v = tv[u]; bi = ti[u]; }
+        }
+        if (threadIdx.x < 32 && 32 * g + (int)threadIdx.x < ncta) cnt = __ldcg(scnt + 32 * g + threadIdx.x);
     }
     warp_argmax_margin(v, bi);
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
-    __shared__ unsigned long long wc[32];
     __syncthreads();                                     // wv/wi are reused
     if (lane == 0) { wv[w] = v; wi[w] = bi; wc[w] = cnt; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        for (int k = 1; k < (int)(blockDim.x >> 5); ++k) {
+        for (int k = 1; k < SCAN_THREADS / 32; ++k) {
             if (better(wv[k], wi[k], v, bi)) { v = wv[k]; bi = wi[k]; }
             cnt += wc[k];
         }
+        gres[g].v = v; gres[g].idx = bi; gres[g].cnt = (unsigned)cnt;
+        gticket[g] = 0u;
+        __threadfence();
+        is_last = (atomicAdd(&ctr[r].ticket, 1u) == (unsigned)(ngroups - 1));
+    }
+    __syncthreads();
+    if (!is_last || threadIdx.x >= 32) return;
+    __threadfence();
+    v = -CUDART_INF; bi = 0x7fffffff; cnt = 0;
+    for (int t = lane; t < ngroups; t += 32) {
+        double tv = __ldcg(&gres[t].v); int ti = __ldcg(&gres[t].idx);
+        cnt += __ldcg(&gres[t].cnt);
+        if (better(tv, ti, v, bi)) { v = tv; bi = ti; }
+    }
+    warp_argmax_margin(v, bi);
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if (lane == 0) {
         bool any = v > 1.0;
         ctr[r].best_index = any ? bi : -1;
         ctr[r].best_L = any ? v : -CUDART_INF;
@@ -929,7 +958,7 @@ void layout_rest(Layout& L, int64_t N, int R, int Kp, int nblk, int64_t log_cap)
     L.bval = take(8 * (size_t)R * nblk);
     L.bidx = take(4 * (size_t)R * nblk);
     L.flog = take(4 * (size_t)R * log_cap);
-    L.scnt = take(4 * (size_t)R * (size_t)((N + SCAN_THREADS - 1) / SCAN_THREADS));
+    L.scnt = take(4 * (size_t)R * scan_aux_stride((int)((N + 1023) / 1024)));
     L.ctr = take(sizeof(Counters) * (size_t)R);
     L.hext = take(16 * (size_t)R);
     L.total = o;
@@ -1302,8 +1331,10 @@ int do_scan(fs_sim* sim, bool finalize) {
     if (rc) return rc;
     dim3 grid((unsigned)((sim->N + SCAN_SPB - 1) / SCAN_SPB), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
-    k_scan<<<grid, SCAN_THREADS, 0, sim->stream>>>(sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc,
-                                               sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr);
+#define FS_SCAN_ARGS sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc, sim->s, sim->hdip, \
+                     sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr
+    k_scan<2><<<grid, SCAN_SPB / 2, 0, sim->stream>>>(FS_SCAN_ARGS);
+#undef FS_SCAN_ARGS
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -1432,6 +1463,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     CREATE_TRY(cudaMemcpyAsync(sim->pos, pos_dev, 16 * (size_t)N, cudaMemcpyDeviceToDevice, st));
     CREATE_TRY(cudaMemcpyAsync(sim->hc, hc_dev, 8 * (size_t)R * N, cudaMemcpyDeviceToDevice, st));
     CREATE_TRY(cudaMemsetAsync(sim->ctr, 0, sizeof(Counters) * R, st));
+    CREATE_TRY(cudaMemsetAsync(sim->scnt, 0, 4 * (size_t)R * scan_aux_stride((int)((N + SCAN_SPB - 1) / SCAN_SPB)), st));
     CREATE_TRY(cudaMemsetAsync(sim->hdip, 0, 16 * (size_t)R * N, st));
     CREATE_TRY(cudaMemcpyAsync(sim->hext, sim->hext_host, sizeof(double2) * R, cudaMemcpyHostToDevice, st));
     int nb = (int)((N + 255) / 256);
