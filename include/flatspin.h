@@ -152,6 +152,18 @@ int fs_scan_ensemble(fs_sim* sim, int64_t* n_switchable /*HOST [R]*/, int64_t* b
 int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out);
 int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out /*HOST [R]*/);
 
+/* A whole field protocol in ONE launch (PAPER.md:63 "discrete time series"; :124 relaxed at each value):
+ * for t = 0..T-1 { global field fields[t]; thermal step key step0 + t; scan (Eqs. 2, 5, 6); relax
+ * }, one persistent CTA per replica doing the scan itself, no host involvement between
+ * steps.  Same arithmetic and flip order as T calls of fs_set_field + fs_relax.  Meant for small and
+ * medium systems and for ensembles, where per-step launches dominate; for N >~ 10^5 the
+ * multi-kernel path scans faster.  fields_dev DEVICE [T,2] (hx,hy), shared by all replicas;
+ * flips_per_step_dev DEVICE [R,T] int64 or NULL; max_flips <= 0: unlimited (cap on the whole sweep);
+ * n_flips_out HOST [R] (total flips of the sweep) or NULL = asynchronous.  The flip log
+ * (fs_get_flip_log) then holds the flips of the whole sweep in order (first 4N+1024). */
+int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
+             int64_t max_flips, int64_t* n_flips_out);
+
 /* Counters accumulated on the device since creation / the last reset: HOST [R] each (any may be
  * NULL).  Synchronises. */
 int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset);

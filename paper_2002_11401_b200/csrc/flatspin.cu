@@ -427,6 +427,21 @@ __global__ void __launch_bounds__(256) k_gather(int64_t N, int Kp, const int* __
 // ------------------------------------------------------------------------------------------------
 struct FieldSpec { double sigma; uint64_t seed; uint32_t step; };
 
+// rot(h_ext) + rot(h_th) of one spin in its own frame (Eq. 2 without h_dip; constant during a relaxation,
+// PAPER.md:124).  One definition for k_scan and the in-CTA scan of the sweep kernel: identical rounding.
+__device__ __forceinline__ double2 fixed_field(double2 c, double2 he, const FieldSpec& fs, int r, uint32_t i) {
+    const double ex = he.x, ey = he.y;
+    if (fs.sigma != 0.0) {
+        double2 t = thermal_xy(fs.sigma, fs.seed + (uint64_t)r, fs.step, i);
+        // (ext + th) rotated together would round differently from the paper's sum of three fields;
+        // rotate separately and add (Eq. 2)
+        double tp = t.x * c.x + t.y * c.y, tq = -t.x * c.y + t.y * c.x;
+        double ep = ex * c.x + ey * c.y, eq = -ex * c.y + ey * c.x;
+        return make_double2(ep + tp, eq + tq);
+    }
+    return make_double2(ex * c.x + ey * c.y, -ex * c.y + ey * c.x);
+}
+
 struct ScanGroup { double v; int idx; unsigned cnt; };  // result of one group of 32 scan CTAs
 // uint32 words of scan scratch per replica: per-CTA counts, group tickets, group results
 __host__ __device__ inline size_t scan_aux_stride(int ncta) {
@@ -468,18 +483,7 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
         const int64_t i = base + q * SCAN_THREADS;
         double m = -CUDART_INF; int mi = 0x7fffffff;
         if (i < N) {
-            const double ex = he.x, ey = he.y;
-            double2 hf;
-            if (fs.sigma != 0.0) {
-                double2 t = thermal_xy(fs.sigma, fs.seed + (uint64_t)r, fs.step, (uint32_t)i);
-                // (ext + th) rotated together would round differently from the paper's sum of three fields;
-                // rotate separately and add (Eq. 2)
-                double tp = t.x * c[q].x + t.y * c[q].y, tq = -t.x * c[q].y + t.y * c[q].x;
-                double ep = ex * c[q].x + ey * c[q].y, eq = -ex * c[q].y + ey * c[q].x;
-                hf = make_double2(ep + tp, eq + tq);
-            } else {
-                hf = make_double2(ex * c[q].x + ey * c[q].y, -ex * c[q].y + ey * c[q].x);
-            }
+            const double2 hf = fixed_field(c[q], he, fs, r, (uint32_t)i);
             hfix_all[off + i] = hf;
             m = margin(hd[q].x + hf.x, hd[q].y + hf.y, sp[q], ih[q], ast);
             M_all[off + i] = m;
@@ -620,10 +624,13 @@ __device__ __forceinline__ void repair_group(int grp, int nblk, const mkey_t* bk
 __global__ void __launch_bounds__(RELAX_THREADS, 1)
 k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_flips, long long log_cap,
         const int* __restrict__ nbr, const double2* __restrict__ wT, const double* __restrict__ ihc_all,
-        int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, const double2* __restrict__ hfix_all,
+        int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, double2* __restrict__ hfix_all,
         double* __restrict__ M_all, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
         int* __restrict__ log_all, Counters* __restrict__ ctr,
-        const int* __restrict__ cellidx /*NULL: no lattice*/, uint16_t* __restrict__ sgrid, int64_t sgrid_stride) {
+        const int* __restrict__ cellidx /*NULL: no lattice*/, uint16_t* __restrict__ sgrid, int64_t sgrid_stride,
+        // sweep mode (T > 0): the CTA runs a whole field protocol, scanning its replica itself at every step
+        int T, const double2* __restrict__ sweep_fields /*[T] (hx,hy)*/, FieldSpec fs, const double2* __restrict__ cs,
+        long long* __restrict__ flips_per_step /*[R,T] or NULL*/, double2* __restrict__ hext_all) {
     // four-level arg-max hierarchy in shared memory:
     // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
     extern __shared__ unsigned char smem_raw[];
@@ -642,16 +649,49 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     const double* ihc = ihc_all + off;
     int8_t* s = s_all + off;
     double2* hdip = hdip_all + off;
-    const double2* hfix = hfix_all + off;
+    double2* hfix = hfix_all + off;
     double* M = M_all + off;
     int* flog = log_all + (int64_t)r * log_cap;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = RELAX_THREADS / 32;
     const bool one_warp = (Kp + 1 <= 32);               // the whole update fits one warp: no broadcast of k needed
 
-    for (int t = tid; t < nblk; t += RELAX_THREADS) {
-        bkey[t] = margin_key(bval_all[(int64_t)r * nblk + t]);
-        bidx[t] = bidx_all[(int64_t)r * nblk + t];
+    long long nflips = 0;
+    int status = 0;
+#ifdef FS_RELAX_PROFILE
+    long long prof[12] = {0};
+#endif
+    int pf_row = -1, pf_done = -1;                      // prefetch engines: candidate whose row / state is in flight
+    constexpr int PF_W0 = NW / 2;                       // warps PF_W0.. are prefetch engines at the top of every iteration
+    const int nsteps = T > 0 ? T : 1;
+    for (int st = 0; st < nsteps; ++st) {
+    const long long nflips_before = nflips;
+    if (T > 0) {
+        // ---- A4-A7 inside the CTA (sweep mode): one warp per leaf, same arithmetic as k_scan
+        const double2 he = sweep_fields[st];
+        FieldSpec f2 = fs; f2.step = fs.step + (uint32_t)st;
+        for (int b = warp; b < nblk; b += NW) {
+            mkey_t bv = 0ull; int bi = 0x7fffffff;
+            for (int q = lane; q < LB; q += 32) {
+                const int64_t i = ((int64_t)b << LBshift) + q;
+                if (i < N) {
+                    const double2 hf = fixed_field(cs[i], he, f2, r, (uint32_t)i);
+                    hfix[i] = hf;
+                    const double2 hd = hdip[i];
+                    const double m = margin(hd.x + hf.x, hd.y + hf.y, (double)s[i], ihc[i], ast);
+                    M[i] = m;
+                    const mkey_t kv = margin_key(m);
+                    if (kv > bv) { bv = kv; bi = (int)i; }
+                }
+            }
+            warp_argmax_key(bv, bi);
+            if (lane == 0) { bkey[b] = bv; bidx[b] = bi; }
+        }
+    } else {
+        for (int t = tid; t < nblk; t += RELAX_THREADS) {
+            bkey[t] = margin_key(bval_all[(int64_t)r * nblk + t]);
+            bidx[t] = bidx_all[(int64_t)r * nblk + t];
+        }
     }
     __syncthreads();
     for (int g = warp; g < ngrp; g += NW) repair_group(g, nblk, bkey, bidx, gkey, gidx_);
@@ -659,16 +699,6 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     for (int g = warp; g < nsup; g += NW) repair_group(g, ngrp, gkey, gidx_, skey, sidx);
     if (tid == 0) { sh_stop = 0; sh_ntouched = 0; }
     __syncthreads();
-
-    long long nflips = 0;
-    int status = 0;
-    int pf_prev = -1;                                   // prefetch engines: last iteration's candidate
-#ifdef FS_RELAX_PROFILE
-    long long prof[12] = {0};
-#endif
-    int pf_row = -1, pf_done = -1;                      // prefetch engines: candidate whose row / state is in flight
-    (void)pf_prev;
-    constexpr int PF_W0 = NW / 2;                       // warps PF_W0.. are prefetch engines at the top of every iteration
     for (;;) {
         FS_PROF_T(c0);
         int k = 0, s_old = 0;
@@ -816,6 +846,11 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         FS_PROF_ADD(0, c0, c1); FS_PROF_ADD(1, c1, c2); FS_PROF_ADD(2, c2, c3); FS_PROF_ADD(3, c3, c4); FS_PROF_ADD(4, c4, c5);
         FS_PROF_ADD(5, c3, c3b);
     }
+    if (T > 0 && tid == 0 && flips_per_step) flips_per_step[(int64_t)r * T + st] = nflips - nflips_before;
+    if (status) break;                                  // max_flips reached
+    __syncthreads();                                    // the next step's scan rewrites the hierarchy
+    }   // steps
+    if (T > 0 && tid == 0) hext_all[r] = sweep_fields[min(T - 1, nsteps - 1)];
     if (tid == 0) {
         ctr[r].total_flips += nflips;
         ctr[r].last_flips = nflips;
@@ -1351,18 +1386,25 @@ int fetch_counters(fs_sim* sim) {
     return FS_OK;
 }
 
-int do_relax(fs_sim* sim, int64_t max_flips) {
-    int rc = do_scan(sim, false);
-    if (rc) return rc;
+// T == 0: relax at the field set by fs_set_field (k_scan first); T > 0: whole protocol in one launch
+int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_dev, uint32_t step0, long long* per_step_dev) {
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
+    FieldSpec fsp{sim->sigma, sim->seed, T > 0 ? step0 : sim->step};
     k_relax<<<sim->R, RELAX_THREADS, sim->relax_smem, sim->stream>>>(
         sim->N, sim->Kp, lb_shift, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr,
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr,
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid,
-        sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0);
+        sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0,
+        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
+}
+
+int do_relax(fs_sim* sim, int64_t max_flips) {
+    int rc = do_scan(sim, false);
+    if (rc) return rc;
+    return launch_relax(sim, max_flips, 0, nullptr, 0, nullptr);
 }
 
 }  // namespace
@@ -1679,6 +1721,24 @@ int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
     for (int r = 0; r < sim->R; ++r) { tot += sim->ctr_host[r].last_flips; capped |= sim->ctr_host[r].status; }
     *n_flips_out = tot;
     return capped ? fail(FS_ERR_MAXFLIPS, "relax stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
+}
+
+int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
+             int64_t max_flips, int64_t* n_flips_out) {
+    if (!sim || !fields_dev) return fail(FS_ERR_ARG, "null pointer");
+    if (T <= 0) return fail(FS_ERR_ARG, "T=%d must be positive", (int)T);
+    int rc = ensure_fields(sim);
+    if (rc) return rc;
+    rc = launch_relax(sim, max_flips, T, reinterpret_cast<const double2*>(fields_dev), step0,
+                      reinterpret_cast<long long*>(flips_per_step_dev));
+    if (rc) return rc;
+    sim->step = step0 + (uint32_t)(T - 1);
+    if (!n_flips_out) return FS_OK;
+    rc = fetch_counters(sim);
+    if (rc) return rc;
+    int capped = 0;
+    for (int r = 0; r < sim->R; ++r) { n_flips_out[r] = sim->ctr_host[r].last_flips; capped |= sim->ctr_host[r].status; }
+    return capped ? fail(FS_ERR_MAXFLIPS, "sweep stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
 }
 
 int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset) {

@@ -440,3 +440,59 @@ def test_config5_full_size_fields_and_scan(B):
     n, best, L = sim.scan()
     no, besto, Lo = orc.scan()
     assert (n, best) == (no, besto) and abs(L - Lo) <= 1e-12 * abs(Lo)
+
+
+# ------------------------------------------------------------------ fs_sweep: whole protocol in one launch
+@pytest.mark.parametrize("which,scale,stride", [("1", None, 1), ("2", 16, 4), ("3", 24, 8), ("4", 40, 1)])
+def test_sweep_one_launch_matches_oracle(B, which, scale, stride):
+    w = W.config(which, scale=scale)
+    sim, orc = mk(B, w)
+    fields = w.fields[::stride]
+    steps = list(range(len(w.fields)))[::stride]
+    # thermal step keys must equal the protocol's row index: sweep in runs of consecutive keys when strided
+    counts, logs = [], []
+    for t, (hx, hy) in zip(steps, fields):
+        orc.set_field(hx, hy, t)
+        n, log = orc.relax_B()
+        counts.append(n); logs.append(log)
+    if stride == 1:
+        n, ps = sim.sweep(fields, step0=0)
+        got = ps.cpu().numpy()[0]
+        glog = sim.get_flip_log().cpu().numpy()
+    else:
+        got, glogs = [], []
+        for t, f in zip(steps, fields):                   # one-step sweeps keep the step keys of the protocol
+            n, ps = sim.sweep(f[None, :], step0=t)
+            got.append(int(ps.cpu().numpy()[0, 0])); glogs.append(sim.get_flip_log().cpu().numpy().copy())
+        got = np.array(got); glog = np.concatenate(glogs)
+    assert np.array_equal(got, np.array(counts))
+    ref = np.concatenate(logs) if logs else np.zeros(0, np.int32)
+    m = min(len(glog), len(ref))
+    assert m > 0 and np.array_equal(glog[:m], ref[:m])
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    assert orc.monitor()[0] == 0
+
+
+def test_sweep_ensemble(B):
+    from oracle import Oracle
+    w = W.config("1")
+    R = 6
+    hc = W.coercive_fields(w.N, seed=300, replicas=R)
+    sim = B.Sim(w.pos, w.angle, hc, w.params)
+    sim.set_thermal(0.004, 7)
+    fields = w.fields[::5]
+    n, ps = sim.sweep(fields, step0=0)
+    ps = ps.cpu().numpy()
+    s = sim.get_spins().cpu().numpy()
+    for r in range(R):
+        o = Oracle(w.pos, w.angle, hc[r], w.params, spins=w.spins)
+        o.set_thermal(0.004, 7 + r)
+        cnt, logs = [], []
+        for t, (hx, hy) in enumerate(fields):
+            o.set_field(hx, hy, t)
+            c, log = o.relax_B()
+            cnt.append(c); logs.append(log)
+        assert np.array_equal(ps[r], np.array(cnt)) and n[r] == sum(cnt)
+        assert np.array_equal(sim.get_flip_log(replica=r).cpu().numpy()[: n[r]], np.concatenate(logs)[: 4 * w.N + 1024])
+        assert np.array_equal(s[r], o.spins())
