@@ -180,6 +180,54 @@ def relax_sweep(B, torch, which="4", scale=None):
     return out
 
 
+def protocol_sweeps(B, torch, cpu=True):
+    """Whole-sweep wall time of configs 1-3 (BASELINE.json metric (3)): the stepwise path (fs_set_field +
+    fs_relax per field value, asynchronous) and fs_sweep (whole protocol in one launch), with the Tier B
+    oracle on the host beside them; plus an ensemble of config-1 replicas."""
+    out = []
+    for which in ("1", "2", "3"):
+        w = W.config(which)
+        sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+        row = {"workload": w.name, "N": w.N, "K": sim.K, "steps": len(w.fields)}
+        for mode in ("stepwise", "one_launch"):
+            sim.set_spins(w.spins); sim.update_fields(); sim.counters(reset=True)
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            if mode == "stepwise":
+                for t, (hx, hy) in enumerate(w.fields):
+                    sim.set_field(hx, hy, t); sim.relax(sync=False)
+            else:
+                sim.sweep(w.fields, step0=0, per_step=False, sync=False)
+            torch.cuda.synchronize(); dt = time.perf_counter() - t0
+            flips = int(sim.counters()[0].sum())
+            row[mode] = {"wall_s": dt, "flips": flips, "flips_per_s": flips / dt}
+        sim.close()
+        if cpu:
+            from oracle import Oracle
+            orc = Oracle(w.pos, w.angle, w.hc, w.params, spins=w.spins)
+            orc.build_neighbors()
+            stride = 1 if which != "3" else 4
+            t0 = time.perf_counter(); flips = 0
+            for t, (hx, hy) in list(enumerate(w.fields))[::stride]:
+                orc.set_field(hx, hy, t); flips += orc.relax_B(cap=1)[0]
+            dt = time.perf_counter() - t0
+            row["cpu_oracle_tier_b"] = {"wall_s": dt, "flips": flips, "cores": 1,
+                                        "sample": "whole protocol" if stride == 1 else f"every {stride}th field value"}
+        out.append(row)
+    # ensemble: R replicas of config 1 (different disorder), whole protocol in one launch, one CTA per replica
+    w = W.config("1")
+    R = 1184
+    hc = W.coercive_fields(w.N, seed=1000, replicas=R)
+    sim = B.Sim(w.pos, w.angle, hc, w.params)
+    sim.update_fields(); torch.cuda.synchronize(); t0 = time.perf_counter()
+    sim.sweep(w.fields, step0=0, per_step=False, sync=False)
+    torch.cuda.synchronize(); dt = time.perf_counter() - t0
+    flips = int(sim.counters()[0].sum())
+    sim.close()
+    ens = {"workload": w.name, "replicas": R, "N": w.N, "steps": len(w.fields), "wall_s": dt, "flips": flips,
+           "flips_per_s": flips / dt, "replica_sweeps_per_s": R / dt}
+    return out, ens
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     if not torch.cuda.is_available():
@@ -314,6 +362,10 @@ def run_ours(args, rank, world, local_rank):
                 line["relax"]["cpu_baseline"] = oracle_relax_sample()
         except Exception as e:   # never lose the headline line
             line["relax"] = {"error": repr(e)}
+        try:
+            line["sweeps"], line["ensemble"] = protocol_sweeps(B, torch, cpu=not args.no_cpu)
+        except Exception as e:
+            line["sweeps"] = {"error": repr(e)}
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
