@@ -627,7 +627,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, double2* __restrict__ hfix_all,
         double* __restrict__ M_all, const double* __restrict__ bval_all, const int* __restrict__ bidx_all,
         int* __restrict__ log_all, Counters* __restrict__ ctr,
-        const int* __restrict__ cellidx /*NULL: no lattice*/, uint16_t* __restrict__ sgrid, int64_t sgrid_stride,
+        const int* __restrict__ cellidx /*NULL: no lattice*/, sgcell_t* __restrict__ sgrid, int64_t sgrid_stride,
         // sweep mode (T > 0): the CTA runs a whole field protocol, scanning its replica itself at every step
         int T, const double2* __restrict__ sweep_fields /*[T] (hx,hy)*/, FieldSpec fs, const double2* __restrict__ cs,
         long long* __restrict__ flips_per_step /*[R,T] or NULL*/, double2* __restrict__ hext_all) {
@@ -811,7 +811,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             if (nflips < log_cap) flog[nflips] = sh_k;
         }
         if (tid == RELAX_THREADS - 32 && cellidx)           // keep the stencil gather's spin grid in step (an idle warp)
-            sgrid[(int64_t)r * sgrid_stride + cellidx[sh_k]] = (uint16_t)(sh_sold > 0 ? 0xbff0 : 0x3ff0);
+            sgrid[(int64_t)r * sgrid_stride + cellidx[sh_k]] = (sh_sold > 0 ? SG_DOWN : SG_UP);
         // ---- A7 repair, level by level, one warp per touched leaf (duplicated group work is harmless)
         const int ntouched = sh_ntouched;
         for (int t = warp; t < ntouched; t += NW) {
@@ -933,7 +933,7 @@ struct fs_sim {
     void* lat_mem = nullptr;        // sub | cu | cv
     void* st_mem = nullptr;         // gidx | T | owner | rowtab | scratch
     uint8_t* lat_sub = nullptr; int *lat_cu = nullptr, *lat_cv = nullptr;
-    uint16_t* sgrid = nullptr; int* cellidx = nullptr; bool sgrid_valid = false;
+    sgcell_t* sgrid = nullptr; int* cellidx = nullptr; bool sgrid_valid = false;
     int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
     int st_nw = 4, st_rs = 1, st_pv = 0; size_t st_smem = 0; bool st_ct = false;
     unsigned long long st_id = 0;   // identity for the ownership of the constant-memory table
@@ -1122,10 +1122,10 @@ bool stencil_ct(const LatGrid& g) {
 
 size_t stencil_smem(const LatGrid& g, int nw, int rs, int* pv_out) {
     int TV = ST_OV * nw, SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv;
-    int pv = SH + 2; while ((pv & 3) != 2) ++pv;                     // row pitch = 2 mod 4 cells: lanes -> distinct banks
+    int pv = (SH + 1) | 1;                                           // odd row pitch (4-byte cells): lanes -> distinct banks
     size_t tsm = stencil_ct(g) ? 0 : 16 * (size_t)g.nsub * g.W * g.H;
     size_t tables = (tsm + 8 * (size_t)g.nsub * g.W + 128 * (size_t)TV + 15) & ~(size_t)15;
-    size_t tiles = 2 * (size_t)g.nsub * SU * pv, red = (size_t)(rs - 1) * nw * 4096;
+    size_t tiles = 4 * (size_t)g.nsub * SU * pv, red = (size_t)(rs - 1) * nw * 4096;
     if (pv_out) *pv_out = pv;
     return tables + std::max(tiles, red);
 }
@@ -1310,7 +1310,7 @@ int detect_lattice(fs_sim* sim) {
         g.Upa = (g.U + ST_TU - 1) / ST_TU * ST_TU + 2 * g.Ru;           // whole tiles + halo: the prologue needs no bounds tests
         g.Vpa = (g.V + TV - 1) / TV * TV + 2 * g.Rv;
     }
-    const size_t sg_bytes = 2 * (size_t)sim->R * nsub * g.Vpa * g.Upa;
+    const size_t sg_bytes = 4 * (size_t)sim->R * nsub * g.Vpa * g.Upa;
     // tables
     size_t slots = (size_t)nsub * nsub * wh;
     size_t o_gidx = 0, o_T = align_up(4 * (size_t)cells), o_owner = o_T + align_up(16 * slots),
@@ -1319,7 +1319,7 @@ int detect_lattice(fs_sim* sim) {
     CUDA_TRY(cudaMalloc(&sim->st_mem, o_end));
     unsigned char* sb = (unsigned char*)sim->st_mem;
     sim->gidx = (int*)(sb + o_gidx); sim->T = (double2*)(sb + o_T); sim->owner = (unsigned long long*)(sb + o_owner);
-    sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (uint16_t*)(sb + o_sg); sim->cellidx = (int*)(sb + o_cell);
+    sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (sgcell_t*)(sb + o_sg); sim->cellidx = (int*)(sb + o_cell);
     CUDA_TRY(cudaMemsetAsync(sim->sgrid, 0, sg_bytes, st));
     CUDA_TRY(cudaMemsetAsync(sim->gidx, 0xff, 4 * (size_t)cells, st));
     CUDA_TRY(cudaMemsetAsync(sim->T, 0, 16 * slots, st));

@@ -26,6 +26,10 @@ constexpr int NSUB_MAX = 8;            // more sublattices than this: use the EL
 constexpr int STENCIL_RMAX = 40;       // larger stencil half-extent: use the ELL gather
 constexpr int ST_OV = 8;               // outputs per thread along v (sliding register window)
 constexpr int ST_TU = 32;              // tile extent along u = one warp
+// one spin-grid cell = the high word of the spin as a double (+1.0, -1.0, or 0 = no magnet): a 4-byte
+// shared-memory load lands directly in the upper register of a DFMA operand whose lower register stays 0
+typedef uint32_t sgcell_t;
+constexpr sgcell_t SG_UP = 0x3ff00000u, SG_DOWN = 0xbff00000u;
 
 struct LatFrame { double ox, oy, i11, i12, i21, i22; };   // (u, v) = Ainv (r - o)
 
@@ -181,12 +185,11 @@ __global__ void k_stencil_count(int64_t N, LatGrid g, const uint8_t* __restrict_
     if ((threadIdx.x & 31) == 0 && n) atomicAdd(total, n);
 }
 
-// dense spin grids sg[rep][sub][Upa][Vpa] (v fastest), one 16-bit cell per lattice site = the upper 16
-// bits of the spin as a double (+1.0 -> 0x3ff0, -1.0 -> 0xbff0, no magnet -> 0), rebuilt from s once
-// per gather.  32 x 32 tiles are transposed through shared memory: gidx is read along u, sg written
+// dense spin grids sg[rep][sub][Upa][Vpa] (v fastest), one sgcell_t per lattice site, rebuilt from s when
+// the spins were rewritten from outside (the relax loop keeps them in step with its own flips).  32 x 32 tiles are transposed through shared memory: gidx is read along u, sg written
 // along v, both coalesced.
 __global__ void k_spin_grid(int64_t N, LatGrid g, int R, const int* __restrict__ gidx, const int8_t* __restrict__ s_all,
-                            uint16_t* __restrict__ sg) {
+                            sgcell_t* __restrict__ sg) {
     __shared__ int tile[32][33];
     const int sub = blockIdx.z, gu0 = blockIdx.x * 32, gv0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;           // 32 x 8 threads
@@ -201,7 +204,7 @@ __global__ void k_spin_grid(int64_t N, LatGrid g, int R, const int* __restrict__
         int idx = tile[tx][k];
         for (int r = 0; r < R; ++r) {
             int sv = idx >= 0 ? (int)s_all[(int64_t)r * N + idx] : 0;
-            sg[(((int64_t)r * g.nsub + sub) * g.Upa + gu) * g.Vpa + gv] = (uint16_t)(sv > 0 ? 0x3ff0 : (sv < 0 ? 0xbff0 : 0));
+            sg[(((int64_t)r * g.nsub + sub) * g.Upa + gu) * g.Vpa + gv] = (sv > 0 ? SG_UP : (sv < 0 ? SG_DOWN : 0u));
         }
     }
 }
@@ -218,19 +221,19 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // ------------------------------------------------------------------------------------------------
 // A3, stencil variant.  CTA = NW x RS warps; tile = 32 cells along u (one per lane) x 8*NW cells
-// along v (8 consecutive outputs per thread).  Prologue: the 16-bit spin tiles (+ halo) of every
-// source sublattice, the coupling tables T[si][*], their row intervals and the spin index of every
-// output go to shared memory with cp.async in one shot (one global round trip per CTA, no staging
-// through registers).  Main loop: for each stencil row du the thread slides an 8-wide register window
-// along v, which is the contiguous direction of its shared-memory row (immediate offsets, row pitch
-// = 2 mod 4 cells so the 32 lanes hit 32 banks); per stencil slot one 2-byte shared load (shifted
-// into the high word of a double whose low word is a register that stays zero) + one broadcast
-// 16-byte weight load feed 16 DFMA.  The stencil rows are dealt round-robin to RS warp groups that
-// share the tile (RS times the warps for the same shared-memory traffic: the FP64 pipe wants >= 4
-// warps per scheduler); their partial sums are added through shared memory in a fixed order.
+// along v (8 consecutive outputs per thread).  Prologue: the spin tiles (+ halo, 4-byte cells) of every
+// source sublattice, the row intervals and the spin index of every output go to shared memory with
+// cp.async in one shot (one global round trip per CTA, no staging through registers).  Main loop: for
+// each stencil row du the thread slides an 8-wide register window along v, which is the contiguous
+// direction of its shared-memory row (immediate offsets, odd row pitch so the 32 lanes hit 32 banks);
+// per stencil slot one 4-byte shared load (the high word of a double whose low word is zero) and the
+// weight pair (CT variant: two uniform-register loads through the constant cache; otherwise one
+// broadcast 16-byte shared load) feed 16 DFMA.  The stencil rows are dealt round-robin to RS warp
+// groups that share the tile (RS times the warps for the same shared-memory traffic: the FP64 pipe
+// wants >= 4 warps per scheduler); their partial sums are added through shared memory in a fixed order.
 // blockIdx.z = replica * nsub + target sublattice.  blockDim = 32 * NW * RS.
 // ------------------------------------------------------------------------------------------------
-#define FS_ST_LD(K, Z) __hiloint2double((int)((unsigned)sp[K] << 16), Z)
+#define FS_ST_LD(K, Z) __hiloint2double((int)sp[K], Z)
 #define FS_ST_FMA(X0, X1, X2, X3, X4, X5, X6, X7, K)                                   \
         const double2 t##K = CT ? c_T[tofs + K] : tp[K];                               \
         a0x = fma(X0, t##K.x, a0x); a0y = fma(X0, t##K.y, a0y);                        \
@@ -259,7 +262,7 @@ __constant__ int2 c_rows[CR_MAX];
 
 template <int MAXT, int MINB, bool CT>
 __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGrid g, int NW, int Pv,
-                                                               const int* __restrict__ gidx, const uint16_t* __restrict__ sg,
+                                                               const int* __restrict__ gidx, const sgcell_t* __restrict__ sg,
                                                                const double2* __restrict__ T, const int2* __restrict__ rowtab,
                                                                double2* __restrict__ hdip_all) {
     extern __shared__ __align__(16) unsigned char st_raw[];
@@ -269,7 +272,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     const size_t tsm_n = CT ? 0 : (size_t)g.nsub * WH;                      // no shared copy of T in the CT variant
     int2* rows = reinterpret_cast<int2*>(Tsm + tsm_n);                      // [nsub][W]
     int* oidx = reinterpret_cast<int*>(rows + (size_t)g.nsub * g.W);        // [TV][32] spin index of every output
-    uint16_t* S = reinterpret_cast<uint16_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 15) & ~(size_t)15));   // [nsub][SU][Pv]
+    sgcell_t* S = reinterpret_cast<sgcell_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 15) & ~(size_t)15));   // [nsub][SU][Pv]
     const int si = blockIdx.z % g.nsub, rep = blockIdx.z / g.nsub;
     const int tu0 = blockIdx.x * ST_TU, tv0 = blockIdx.y * TV;       // tile origin, interior coordinates
     // the warp index via a shuffle from lane 0: the compiler then knows everything derived from it is
@@ -279,14 +282,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
 
     // ---- prologue: everything this CTA reads, in flight at once
     {
-        const int HP = SH >> 1;                        // SH is even: 2-cell (4-byte) pieces per row
-        const uint16_t* src = sg + (((int64_t)rep * g.nsub * g.Upa + tu0) * g.Vpa + tv0);
+        const sgcell_t* src = sg + (((int64_t)rep * g.nsub * g.Upa + tu0) * g.Vpa + tv0);
         const int nwarps = blockDim.x >> 5, wid = threadIdx.x >> 5;
         for (int sj = 0; sj < g.nsub; ++sj)
             for (int ul = wid; ul < SU; ul += nwarps) {            // one tile row per warp: no index divisions
-                uint16_t* drow = S + ((size_t)sj * SU + ul) * Pv;
-                const uint16_t* srow = src + ((int64_t)sj * g.Upa + ul) * g.Vpa;
-                for (int c = lane; c < HP; c += 32) cp_async4(drow + 2 * c, srow + 2 * c);
+                sgcell_t* drow = S + ((size_t)sj * SU + ul) * Pv;
+                const sgcell_t* srow = src + ((int64_t)sj * g.Upa + ul) * g.Vpa;
+                for (int c = lane; c < SH; c += 32) cp_async4(drow + c, srow + c);
             }
     }
     if (!CT)
@@ -307,16 +309,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
                  : "=r"(z0), "=r"(z1), "=r"(z2), "=r"(z3), "=r"(z4), "=r"(z5), "=r"(z6), "=r"(z7));
 
     for (int sj = 0; sj < g.nsub; ++sj) {
-        const uint16_t* Sj = S + ((size_t)sj * SU + lane) * Pv + warp * ST_OV + g.Rv;
+        const sgcell_t* Sj = S + ((size_t)sj * SU + lane) * Pv + warp * ST_OV + g.Rv;
         const double2* Tj = Tsm + (CT ? 0 : (size_t)sj * WH + g.Rv);
         const int tj = (si * g.nsub + sj) * WH + g.Rv;
-        for (int r = 0; r < g.W; ++r) {                // r = du + Ru: a uniform counter, so that the row interval
-            if (r % RS != rs) continue;                // and the weight offsets below live in uniform registers
+        // r = du + Ru is a uniform loop counter, so that the row interval and the weight offsets below live
+        // in uniform registers (starting every CTA at a different row to break lockstep was tried: no gain)
+        for (int r = 0; r < g.W; ++r) {
+            if ((r & (RS - 1)) != rs) continue;        // RS is a power of two
             const int2 rt = CT ? c_rows[(si * g.nsub + sj) * g.W + r] : rows[sj * g.W + r];
             int n = rt.y - rt.x + 1;
             if (n <= 0) continue;
             // output (lane, warp*8+q) at slot (du, dv) reads S[sj][lane + du + Ru][warp*8 + q + dv + Rv]
-            const uint16_t* sp = Sj + (size_t)r * Pv + rt.x;
+            const sgcell_t* sp = Sj + (size_t)r * Pv + rt.x;
             const double2* tp = Tj + (CT ? 0 : r * g.H + rt.x);
             int tofs = tj + r * g.H + rt.x;
             double x0 = FS_ST_LD(0, z0), x1 = FS_ST_LD(1, z1), x2 = FS_ST_LD(2, z2), x3 = FS_ST_LD(3, z3);
