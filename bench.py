@@ -228,6 +228,21 @@ def protocol_sweeps(B, torch, cpu=True):
     return out, ens
 
 
+def max_over_ranks(dist, values_ms, device):
+    """Replicas only: every rank times its own replica; the job's time is the slowest rank's."""
+    import torch
+    t = torch.tensor(list(values_ms), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_value(units_per_rank_step, steps, world, ms):
+    """Whole-job throughput: every rank processed `units_per_rank_step` per step (weak scaling, no collective
+    on the data path), all ranks finished within `ms` (max over ranks)."""
+    return world * units_per_rank_step * steps / (ms * 1e-3)
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     if not torch.cuda.is_available():
@@ -303,12 +318,9 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
 
-    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = float(t[0]), float(t[1])
-    value = world * I * args.steps / (ms * 1e-3)
-    e2e_value = world * I * args.steps / (e2e_ms * 1e-3)
+    ms, e2e_ms = max_over_ranks(dist, [ms, e2e_s * 1e3], dev)
+    value = whole_job_value(I, args.steps, world, ms)
+    e2e_value = whole_job_value(I, args.steps, world, e2e_ms)
 
     peak, peak_src = measured_peaks()
     if use_stencil:
