@@ -118,6 +118,12 @@ int fs_set_field(fs_sim* sim, double hx, double hy, uint32_t step);
 /* Per-replica global fields: h_host HOST [R,2] (hx,hy). */
 int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step);
 
+/* Per-spin external field h_ext^(i) ("global, per-spin or a spatial vector field"): h_dev DEVICE
+ * [N,2] (global x,y components), shared by all replicas, ADDED to the global field of fs_set_field / fs_sweep
+ * before the rotation into the spin's frame (reading D-4).  Copied (library-owned buffer); NULL
+ * clears it.  Takes effect at the next scan / relax / sweep. */
+int fs_set_local_field(fs_sim* sim, const double* h_dev);
+
 /* Choose the gather kernel variant (FS_GATHER_*).  Default auto. */
 int fs_set_gather_variant(fs_sim* sim, int variant);
 

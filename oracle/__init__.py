@@ -51,6 +51,7 @@ def lib():
         L.orc_get_spins.argtypes = [vp, vp]
         L.orc_set_thermal.argtypes = [vp, dbl, C.c_uint64]
         L.orc_set_field.argtypes = [vp, dbl, dbl, C.c_uint32]
+        L.orc_set_local_field.argtypes = [vp, vp]
         L.orc_coupling.argtypes = [vp, i64, i64, vp]
         L.orc_field_one.argtypes = [vp, i64, i32, vp]
         L.orc_fields.argtypes = [vp, i32, vp]
@@ -144,6 +145,13 @@ class Oracle:
 
     def set_thermal(self, sigma, seed): self.L.orc_set_thermal(self.h, float(sigma), int(seed))
     def set_field(self, hx, hy, step=0): self.L.orc_set_field(self.h, float(hx), float(hy), int(step))
+
+    def set_local_field(self, h):
+        """Per-spin external field [N,2] (global x,y components) added to the global one; None clears."""
+        if h is None:
+            self.L.orc_set_local_field(self.h, None); return
+        h = np.ascontiguousarray(h, np.float64); assert h.shape == (self.N, 2)
+        self.L.orc_set_local_field(self.h, h.ctypes.data)
 
     def coupling(self, i, j):
         g = np.zeros(2); self.L.orc_coupling(self.h, int(i), int(j), g.ctypes.data); return g

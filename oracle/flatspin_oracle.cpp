@@ -199,10 +199,15 @@ struct Oracle {
     }
     std::vector<int32_t> tmp_nb;
 
-    // external field rotated into the local frame (Fig. 2)
+    // external field rotated into the local frame (Fig. 2).  PAPER.md:61: the external field
+    // may be global, per-spin h_ext^(i), or a spatial vector field: here h_ext^(i) = global + local_i, summed
+    // in global x,y components and then rotated (reading D-4); local_i defaults to zero.
+    std::vector<double> lx, ly;
     void hext(int64_t i, double h[2]) const {
-        h[0] = hx * ct[i] + hy * st[i];
-        h[1] = -hx * st[i] + hy * ct[i];
+        double ex = hx, ey = hy;
+        if (!lx.empty()) { ex = hx + lx[i]; ey = hy + ly[i]; }
+        h[0] = ex * ct[i] + ey * st[i];
+        h[1] = -ex * st[i] + ey * ct[i];
     }
     // thermal field: global x,y components sigma*(z0,z1), rotated like h_ext (C-9);
     // drawn once per (seed, step, spin) and constant during relaxation (C-10).
@@ -416,6 +421,11 @@ int64_t orc_neighbors_of(void* h, int64_t i, int32_t* out, int64_t cap) {
 void orc_set_spins(void* h, const int8_t* s) { Oracle* o = (Oracle*)h; o->s.assign(s, s + o->N); o->hd_valid = false; }
 void orc_get_spins(void* h, int8_t* s) { Oracle* o = (Oracle*)h; std::memcpy(s, o->s.data(), o->N); }
 void orc_set_thermal(void* h, double sigma, uint64_t seed) { Oracle* o = (Oracle*)h; o->sigma = sigma; o->seed = seed; }
+void orc_set_local_field(void* h, const double* hl /*[N,2] or NULL*/) {
+    Oracle* o = (Oracle*)h;
+    o->lx.clear(); o->ly.clear();
+    if (hl) { o->lx.resize(o->N); o->ly.resize(o->N); for (int64_t i = 0; i < o->N; ++i) { o->lx[i] = hl[2 * i]; o->ly[i] = hl[2 * i + 1]; } }
+}
 void orc_set_field(void* h, double hx, double hy, uint32_t step) { Oracle* o = (Oracle*)h; o->hx = hx; o->hy = hy; o->step = step; }
 void orc_coupling(void* h, int64_t i, int64_t j, double* g) { ((Oracle*)h)->coupling(i, j, g); }
 void orc_field_one(void* h, int64_t i, int which, double* out) { ((Oracle*)h)->field(i, which, out); }

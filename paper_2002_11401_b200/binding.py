@@ -23,7 +23,7 @@ EXPORTS = [
     "fs_get_spins", "fs_set_thermal", "fs_set_field", "fs_set_field_ensemble", "fs_set_gather_variant",
     "fs_update_fields", "fs_scan", "fs_scan_ensemble", "fs_relax", "fs_relax_ensemble", "fs_get_counters",
     "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
-    "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep",
+    "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep", "fs_set_local_field",
 ]
 
 
@@ -76,6 +76,7 @@ def load_library(path: str | None = None):
         "fs_last_error": [],
         "fs_get_lattice": [vp, vp, vp],
         "fs_sweep": [vp, vp, i32, C.c_uint32, vp, i64, vp],
+        "fs_set_local_field": [vp, vp],
         "fs_measure_fp64_peak": [P(dbl), vp],
     }
     for name, args in sig.items():
@@ -179,6 +180,15 @@ class Sim:
     def set_field_ensemble(self, h, step=0):
         h = np.ascontiguousarray(h, np.float64); assert h.shape == (self.R, 2)
         _check(self.L, self.L.fs_set_field_ensemble(self.h, h.ctypes.data, int(step)))
+
+    def set_local_field(self, h):
+        """Per-spin external field [N,2] added to the global one; None clears it."""
+        if h is None:
+            _check(self.L, self.L.fs_set_local_field(self.h, None)); return
+        t = torch.as_tensor(np.ascontiguousarray(h, np.float64)).to(self.device).contiguous()
+        assert tuple(t.shape) == (self.N, 2)
+        _check(self.L, self.L.fs_set_local_field(self.h, t.data_ptr()))
+        self.stream.synchronize()
 
     def set_gather_variant(self, v):
         _check(self.L, self.L.fs_set_gather_variant(self.h, int(v)))

@@ -459,7 +459,8 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
                                                const int8_t* __restrict__ s_all, const double2* __restrict__ hdip_all,
                                                double2* __restrict__ hfix_all, double* __restrict__ M_all,
                                                double* __restrict__ bval_all, int* __restrict__ bidx_all, int nblk,
-                                               unsigned* __restrict__ scnt_all /*[R][gridDim.x]*/, Counters* __restrict__ ctr) {
+                                               unsigned* __restrict__ scnt_all /*[R][gridDim.x]*/, Counters* __restrict__ ctr,
+                                               const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/) {
     __shared__ double wv[32];                            // arg-max of every 32-spin slot of this CTA
     __shared__ int wi[32];
     __shared__ int is_last;
@@ -483,7 +484,9 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
         const int64_t i = base + q * SCAN_THREADS;
         double m = -CUDART_INF; int mi = 0x7fffffff;
         if (i < N) {
-            const double2 hf = fixed_field(c[q], he, fs, r, (uint32_t)i);
+            double2 hei = he;                             // h_ext^(i) = global + per-spin
+            if (hloc) { const double2 l = hloc[i]; hei = make_double2(he.x + l.x, he.y + l.y); }
+            const double2 hf = fixed_field(c[q], hei, fs, r, (uint32_t)i);
             hfix_all[off + i] = hf;
             m = margin(hd[q].x + hf.x, hd[q].y + hf.y, sp[q], ih[q], ast);
             M_all[off + i] = m;
@@ -630,7 +633,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         const int* __restrict__ cellidx /*NULL: no lattice*/, sgcell_t* __restrict__ sgrid, int64_t sgrid_stride,
         // sweep mode (T > 0): the CTA runs a whole field protocol, scanning its replica itself at every step
         int T, const double2* __restrict__ sweep_fields /*[T] (hx,hy)*/, FieldSpec fs, const double2* __restrict__ cs,
-        long long* __restrict__ flips_per_step /*[R,T] or NULL*/, double2* __restrict__ hext_all) {
+        long long* __restrict__ flips_per_step /*[R,T] or NULL*/, double2* __restrict__ hext_all,
+        const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/) {
     // four-level arg-max hierarchy in shared memory:
     // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
     extern __shared__ unsigned char smem_raw[];
@@ -675,7 +679,9 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             for (int q = lane; q < LB; q += 32) {
                 const int64_t i = ((int64_t)b << LBshift) + q;
                 if (i < N) {
-                    const double2 hf = fixed_field(cs[i], he, f2, r, (uint32_t)i);
+                    double2 hei = he;
+                    if (hloc) { const double2 l = hloc[i]; hei = make_double2(he.x + l.x, he.y + l.y); }
+                    const double2 hf = fixed_field(cs[i], hei, f2, r, (uint32_t)i);
                     hfix[i] = hf;
                     const double2 hd = hdip[i];
                     const double m = margin(hd.x + hf.x, hd.y + hf.y, (double)s[i], ihc[i], ast);
@@ -867,12 +873,13 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
 // ------------------------------------------------------------------------------------------------
 __global__ void k_fields_out(int64_t N, int which, FieldSpec fs, const double2* __restrict__ hext_all,
                              const double2* __restrict__ cs, const double2* __restrict__ hdip_all,
-                             double2* __restrict__ out_all) {
+                             double2* __restrict__ out_all, const double2* __restrict__ hloc) {
     int r = blockIdx.y;
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= N) return;
     double2 c = cs[i];
     double2 he = hext_all[r];
+    if (hloc) { const double2 l = hloc[i]; he = make_double2(he.x + l.x, he.y + l.y); }
     double2 d = hdip_all[(int64_t)r * N + i];
     double2 e = make_double2(he.x * c.x + he.y * c.y, -he.x * c.y + he.y * c.x);
     double2 t = make_double2(0.0, 0.0);
@@ -923,6 +930,7 @@ struct fs_sim {
     double sigma = 0.0; uint64_t seed = 0; uint32_t step = 0;
     double2* hext_host = nullptr;   // pinned staging [R]
     Counters* ctr_host = nullptr;   // pinned staging [R]
+    double2* hloc = nullptr;        // per-spin external field [N] (library-owned), NULL = none
     int gather_variant = FS_GATHER_AUTO;
     size_t relax_smem = 0;
     // regular-lattice stencil (lattice.cuh); library-owned device memory, freed by fs_destroy
@@ -1367,7 +1375,7 @@ int do_scan(fs_sim* sim, bool finalize) {
     dim3 grid((unsigned)((sim->N + SCAN_SPB - 1) / SCAN_SPB), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
 #define FS_SCAN_ARGS sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc, sim->s, sim->hdip, \
-                     sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr
+                     sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr, sim->hloc
     k_scan<2><<<grid, SCAN_SPB / 2, 0, sim->stream>>>(FS_SCAN_ARGS);
 #undef FS_SCAN_ARGS
     LAUNCHED();
@@ -1395,7 +1403,7 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr,
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid,
         sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0,
-        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext);
+        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -1556,6 +1564,7 @@ int fs_destroy(fs_sim* sim) {
     if (!sim) return FS_OK;
     if (sim->hext_host) cudaFreeHost(sim->hext_host);
     if (sim->ctr_host) cudaFreeHost(sim->ctr_host);
+    if (sim->hloc) cudaFree(sim->hloc);
     if (sim->lat_mem) cudaFree(sim->lat_mem);
     if (sim->st_mem) cudaFree(sim->st_mem);
     delete sim;
@@ -1605,6 +1614,17 @@ int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step) {
     for (int r = 0; r < sim->R; ++r) sim->hext_host[r] = make_double2(h_host[2 * r], h_host[2 * r + 1]);
     sim->step = step;
     return push_field(sim);
+}
+
+int fs_set_local_field(fs_sim* sim, const double* h_dev) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (!h_dev) {
+        if (sim->hloc) { CUDA_TRY(cudaStreamSynchronize(sim->stream)); cudaFree(sim->hloc); sim->hloc = nullptr; }
+        return FS_OK;
+    }
+    if (!sim->hloc) CUDA_TRY(cudaMalloc(&sim->hloc, 16 * (size_t)sim->N));
+    CUDA_TRY(cudaMemcpyAsync(sim->hloc, h_dev, 16 * (size_t)sim->N, cudaMemcpyDeviceToDevice, sim->stream));
+    return FS_OK;
 }
 
 int fs_set_gather_variant(fs_sim* sim, int variant) {
@@ -1759,7 +1779,7 @@ int fs_get_fields(fs_sim* sim, int which, double* h_dev_out) {
     if (which == FS_FIELD_TOTAL || which == FS_FIELD_DIP) { int rc = ensure_fields(sim); if (rc) return rc; }
     dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
-    k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, which, fsp, sim->hext, sim->cs, sim->hdip, (double2*)h_dev_out);
+    k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, which, fsp, sim->hext, sim->cs, sim->hdip, (double2*)h_dev_out, sim->hloc);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -1803,7 +1823,7 @@ int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t*
     // total field into hfix's sibling buffer M is not large enough; reuse hfix (rewritten by the next scan)
     dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
-    k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, FS_FIELD_TOTAL, fsp, sim->hext, sim->cs, sim->hdip, sim->hfix);
+    k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, FS_FIELD_TOTAL, fsp, sim->hext, sim->cs, sim->hdip, sim->hfix, sim->hloc);
     LAUNCHED();
     CUDA_TRY(cudaMemcpyAsync(h_host_out, sim->hfix, 16 * rn, cudaMemcpyDeviceToHost, sim->stream));
     rc = fetch_counters(sim);

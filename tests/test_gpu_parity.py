@@ -496,3 +496,39 @@ def test_sweep_ensemble(B):
         assert np.array_equal(ps[r], np.array(cnt)) and n[r] == sum(cnt)
         assert np.array_equal(sim.get_flip_log(replica=r).cpu().numpy()[: n[r]], np.concatenate(logs)[: 4 * w.N + 1024])
         assert np.array_equal(s[r], o.spins())
+
+
+# ------------------------------------------------------------------ per-spin external field
+def test_local_field_parity(B):
+    """A smooth spatial vector field h_ext(r) sampled per spin, on top of the global ramp: fields, scan, relax
+    (stepwise and one-launch sweep) against the oracle; clearing it restores the global-only results."""
+    w = W.config("4", scale=30)
+    loc = 0.03 * np.stack([np.sin(0.4 * w.pos[:, 0]) * np.cos(0.3 * w.pos[:, 1]),
+                           np.cos(0.5 * w.pos[:, 0] + 0.2 * w.pos[:, 1])], axis=1)
+    sim, orc = mk(B, w)
+    sim.set_local_field(loc); orc.set_local_field(loc)
+    hx, hy = w.fields[120]
+    sim.set_field(hx, hy, 120); orc.set_field(hx, hy, 120)
+    sim.update_fields()
+    _check_all_fields(sim, orc)
+    assert sim.scan()[:2] == orc.scan()[:2]
+    total = 0
+    for t in range(120, 200, 4):
+        hx, hy = w.fields[t]
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        n = sim.relax(); no, log = orc.relax_B()
+        assert n == no and (n == 0 or np.array_equal(sim.get_flip_log().cpu().numpy(), log))
+        total += n
+    assert total > 0 and np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    # one-launch sweep with the local field, from a fresh state
+    sim2, orc2 = mk(B, w)
+    sim2.set_local_field(loc); orc2.set_local_field(loc)
+    cnt = []
+    for t, (hx, hy) in enumerate(w.fields):
+        orc2.set_field(hx, hy, t); cnt.append(orc2.relax_B()[0])
+    n, ps = sim2.sweep(w.fields, step0=0)
+    assert np.array_equal(ps.cpu().numpy()[0], np.array(cnt))
+    assert np.array_equal(sim2.get_spins().cpu().numpy(), orc2.spins())
+    assert field_err(sim2.get_fields(0).cpu().numpy(), orc2.fields(0)) < FIELD_TOL
+    sim2.set_local_field(None); orc2.set_local_field(None)
+    assert field_err(sim2.get_fields(2).cpu().numpy(), orc2.fields(2)) < FIELD_TOL

@@ -448,3 +448,34 @@ def test_switching_order_invariant_to_time_resolution_without_coupling():
             o.set_field(hx, hy, t); logs.append(o.relax_B()[1])
         orders.append(np.concatenate(logs))
     assert len(orders[0]) == w.N and np.array_equal(orders[0], orders[1])
+
+
+# ------------------------------------------------------------------ per-spin external field
+def test_local_field_pins():
+    """h_ext^(i) = global + local_i (reading D-4).  Pins: a uniform local field equals the same global field
+    bit for bit; a local field on one spin changes only that spin's external field, by its rotation into the
+    spin's frame (closed form); an isolated spin switches under a local field exactly as under a global one
+    (classical astroid: at h_perp = 0 it switches iff h_par < -h_c)."""
+    pos, ang = W.square_closed(4)
+    N = len(ang)
+    p = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    hc = W.coercive_fields(N, seed=2)
+    a = Oracle(pos, ang, hc, p); b = Oracle(pos, ang, hc, p)
+    a.set_field(0.03, -0.07, 0)
+    b.set_field(0.0, 0.0, 0); b.set_local_field(np.tile([0.03, -0.07], (N, 1)))
+    assert np.array_equal(a.fields(2), b.fields(2)) and np.array_equal(a.fields(0), b.fields(0))
+    loc = np.zeros((N, 2)); loc[7] = [0.11, 0.05]                 # spin 7 is horizontal (theta = 0) in this geometry
+    assert ang[7] == 0.0 and ang[N - 1] == math.pi / 2
+    b.set_local_field(loc)
+    e = b.fields(2)
+    assert np.array_equal(e[7], [0.11, 0.05]) and np.count_nonzero(e) == 2
+    loc = np.zeros((N, 2)); loc[N - 1] = [0.11, 0.05]             # vertical spin: par = h_y, perp = -h_x
+    b.set_local_field(loc)
+    assert np.allclose(b.fields(2)[N - 1], [0.05, -0.11], rtol=0, atol=1e-17)
+    b.set_local_field(None)
+    assert np.count_nonzero(b.fields(2)) == 0
+    # isolated spin, classical astroid: switches iff local h_par < -h_c
+    one = Oracle(np.array([[0.0, 0.0]]), np.array([0.0]), np.array([0.2]), p)
+    one.set_field(0.0, 0.0, 0)
+    one.set_local_field(np.array([[-0.1999, 0.0]])); assert one.relax_A()[0] == 0
+    one.set_local_field(np.array([[-0.2001, 0.0]])); assert one.relax_A()[0] == 1 and one.spins()[0] == -1
