@@ -943,7 +943,7 @@ struct fs_sim {
     uint8_t* lat_sub = nullptr; int *lat_cu = nullptr, *lat_cv = nullptr;
     sgcell_t* sgrid = nullptr; int* cellidx = nullptr; bool sgrid_valid = false;
     int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
-    int st_nw = 4, st_rs = 1, st_pv = 0; size_t st_smem = 0; bool st_ct = false;
+    int st_nw = 4, st_rs = 1, st_pv = 0, st_ov = ST_OV; size_t st_smem = 0; bool st_ct = false;
     unsigned long long st_id = 0;   // identity for the ownership of the constant-memory table
     double st_maxdev = 0.0, st_wmax = 0.0;
     long long st_slots = 0;         // stencil slots present (sum over sublattice pairs)
@@ -1082,7 +1082,7 @@ void launch_gather_g(fs_sim* sim) {
 
 int do_gather_stencil(fs_sim* sim) {
     const LatGrid& g = sim->lg;
-    int TV = ST_OV * sim->st_nw;
+    int TV = sim->st_ov * sim->st_nw;
     dim3 sgrid((unsigned)((g.Up + 31) / 32), (unsigned)((g.Vp + 31) / 32), (unsigned)g.nsub);
     if (!sim->sgrid_valid) {                             // the relax loop keeps the grids in step with its flips
         k_spin_grid<<<sgrid, 256, 0, sim->stream>>>(sim->N, g, sim->R, sim->gidx, sim->s, sim->sgrid);
@@ -1091,9 +1091,16 @@ int do_gather_stencil(fs_sim* sim) {
     }
     dim3 grid((unsigned)((g.U + ST_TU - 1) / ST_TU), (unsigned)((g.V + TV - 1) / TV), (unsigned)(g.nsub * sim->R));
     int threads = 32 * sim->st_nw * sim->st_rs;
-#define FS_LAUNCH_STENCIL(MAXT, MINB, CTV)                                                          \
-    k_gather_stencil<MAXT, MINB, CTV><<<grid, threads, sim->st_smem, sim->stream>>>(                \
+#define FS_LAUNCH_STENCIL1(MAXT, MINB, CTV, OVV)                                                    \
+    k_gather_stencil<MAXT, MINB, CTV, OVV><<<grid, threads, sim->st_smem, sim->stream>>>(           \
         sim->N, g, sim->st_nw, sim->st_pv, sim->gidx, sim->sgrid, sim->T, sim->rowtab, sim->hdip)
+    // 8 outputs per thread: 72 (<= 128 threads) or 80 registers.  A 16-output variant (128 registers, half the
+    // window set-ups per DFMA) was measured at 64.4 us against 63.3 us on config 5 and is not instantiated.
+#define FS_LAUNCH_STENCIL(CTV)                                                                      \
+    do {                                                                                            \
+        if (threads <= 128) FS_LAUNCH_STENCIL1(128, 7, CTV, 8);                                     \
+        else FS_LAUNCH_STENCIL1(256, 3, CTV, 8);                                                    \
+    } while (0)
     if (sim->st_ct) {
         // the constant-memory table is shared by all simulations of the process: take it over if needed
         std::lock_guard<std::mutex> lock(g_ct_mutex);
@@ -1105,13 +1112,14 @@ int do_gather_stencil(fs_sim* sim) {
                                              cudaMemcpyDeviceToDevice, sim->stream));
             g_ct_owner = sim->st_id;
         }
-        if (threads <= 128) FS_LAUNCH_STENCIL(128, 7, true); else FS_LAUNCH_STENCIL(256, 3, true);
+        FS_LAUNCH_STENCIL(true);
         if (!g_ct_event) CUDA_TRY(cudaEventCreateWithFlags(&g_ct_event, cudaEventDisableTiming));
         CUDA_TRY(cudaEventRecord(g_ct_event, sim->stream));
     } else {
-        if (threads <= 128) FS_LAUNCH_STENCIL(128, 7, false); else FS_LAUNCH_STENCIL(256, 3, false);
+        FS_LAUNCH_STENCIL(false);
     }
 #undef FS_LAUNCH_STENCIL
+#undef FS_LAUNCH_STENCIL1
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     sim->fields_dirty = false;
@@ -1121,44 +1129,46 @@ int do_gather_stencil(fs_sim* sim) {
 // Shape of the stencil kernel for this lattice: NW v-slabs x RS row groups per CTA.  Small model: every
 // CTA does work ~ NW; an SM runs ceil(ctas / SMs) of them (one wave if they fit) and needs >= 20
 // resident warps to keep its FP64 pipe busy.  Ties go to the larger tile (less halo), then fewer groups.
-struct StencilShape { int nw, rs, pv; size_t smem; };
+struct StencilShape { int nw, rs, pv, ov; size_t smem; };
 
 bool stencil_ct(const LatGrid& g) {
     return (int64_t)g.nsub * g.nsub * g.W * g.H <= CT_MAX && g.nsub * g.nsub * g.W <= CR_MAX &&
            env_int("FS_STENCIL_NO_CT", 0) == 0;
 }
 
-size_t stencil_smem(const LatGrid& g, int nw, int rs, int* pv_out) {
-    int TV = ST_OV * nw, SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv;
+size_t stencil_smem(const LatGrid& g, int nw, int rs, int ov, int* pv_out) {
+    int TV = ov * nw, SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv;
     int pv = (SH + 1) | 1;                                           // odd row pitch (4-byte cells): lanes -> distinct banks
     size_t tsm = stencil_ct(g) ? 0 : 16 * (size_t)g.nsub * g.W * g.H;
     size_t tables = (tsm + 8 * (size_t)g.nsub * g.W + 128 * (size_t)TV + 15) & ~(size_t)15;
-    size_t tiles = 4 * (size_t)g.nsub * SU * pv, red = (size_t)(rs - 1) * nw * 4096;
+    size_t tiles = 4 * (size_t)g.nsub * SU * pv, red = (size_t)(rs - 1) * nw * 512 * ov;
     if (pv_out) *pv_out = pv;
     return tables + std::max(tiles, red);
 }
 
 bool plan_stencil(const fs_sim* sim, const LatGrid& g, StencilShape* out) {
     double best = 1e300; bool found = false;
+    const int ov = ST_OV;
     for (int nw = 8; nw >= 1; nw >>= 1)
-        for (int rs = 1; rs <= 4 && nw * rs <= 8; rs <<= 1) {
+        for (int rs = 1; rs <= 4 && nw * rs <= (ov == 16 ? 4 : 8); rs <<= 1) {
             if (rs > g.W) continue;
-            int pv; size_t smem = stencil_smem(g, nw, rs, &pv);
+            int pv; size_t smem = stencil_smem(g, nw, rs, ov, &pv);
             if (smem > 200 * 1024) continue;
-            int threads = 32 * nw * rs, TV = ST_OV * nw;
+            int threads = 32 * nw * rs, TV = ov * nw;
             int64_t ctas = (int64_t)((g.U + ST_TU - 1) / ST_TU) * ((g.V + TV - 1) / TV) * g.nsub * sim->R;
-            int regs = threads <= 128 ? 72 : 80;
+            int regs = ov == 16 ? 128 : (threads <= 128 ? 72 : 80);
             int64_t resident = std::min<int64_t>(std::min<int64_t>(65536 / (regs * threads), (227 * 1024) / (int64_t)(smem + 1024)),
                                                  std::min<int64_t>(2048 / threads, 32));
             if (resident < 1) continue;
             int64_t per_sm = (ctas + sim->sm_count - 1) / sim->sm_count;
             int64_t waves = (per_sm + resident - 1) / resident;
             double warps = (double)std::min(per_sm, resident) * nw * rs;
-            double eff = std::min(1.0, warps / 20.0);
+            double eff = std::min(1.0, warps * (ov / 8) / 20.0);     // a 16-output warp carries twice the independent DFMAs
             // multi-wave launches pay for a partly filled last wave
-            double cost = (waves == 1 ? (double)per_sm : (double)waves * resident) * nw / eff;
-            cost *= 1.0 + 0.02 * (rs - 1) + 0.16 / nw;               // reduction epilogue; halo staging per output
-            if (cost < best - 1e-9) { best = cost; *out = StencilShape{nw, rs, pv, smem}; found = true; }
+            double cost = (waves == 1 ? (double)per_sm : (double)waves * resident) * nw * (ov / 8) / eff;
+            // reduction epilogue; halo staging per output; per-row window set-up per output
+            cost *= 1.0 + 0.02 * (rs - 1) + 0.16 * 8 / (nw * ov) + (ov == 16 ? 0.0 : 0.10);
+            if (cost < best - 1e-9) { best = cost; *out = StencilShape{nw, rs, pv, ov, smem}; found = true; }
         }
     return found;
 }
@@ -1308,13 +1318,14 @@ int detect_lattice(fs_sim* sim) {
     if (!plan_stencil(sim, g, &shp)) return lattice_fail(sim, FS_LATTICE_STENCIL_TOO_WIDE);
     if (env_int("FS_STENCIL_NW", 0) > 0) {                           // tuning override
         shp.nw = env_int("FS_STENCIL_NW", 0); shp.rs = std::max(1, env_int("FS_STENCIL_RS", 1));
-        shp.smem = stencil_smem(g, shp.nw, shp.rs, &shp.pv);
+        shp.ov = ST_OV;
+        shp.smem = stencil_smem(g, shp.nw, shp.rs, shp.ov, &shp.pv);
     }
-    sim->st_nw = shp.nw; sim->st_rs = shp.rs; sim->st_pv = shp.pv; sim->st_smem = shp.smem;
+    sim->st_nw = shp.nw; sim->st_rs = shp.rs; sim->st_pv = shp.pv; sim->st_ov = shp.ov; sim->st_smem = shp.smem;
     sim->st_ct = stencil_ct(g);
     sim->st_id = ++g_ct_next_id;
     {
-        int TV = ST_OV * sim->st_nw;
+        int TV = sim->st_ov * sim->st_nw;
         g.Upa = (g.U + ST_TU - 1) / ST_TU * ST_TU + 2 * g.Ru;           // whole tiles + halo: the prologue needs no bounds tests
         g.Vpa = (g.V + TV - 1) / TV * TV + 2 * g.Rv;
     }
@@ -1355,10 +1366,11 @@ int detect_lattice(fs_sim* sim) {
     if (!(sim->st_maxdev * (double)sim->K <= 2e-13 * sim->st_wmax)) return lattice_fail(sim, FS_LATTICE_WEIGHT_MISMATCH);
     if (sim->st_smem > 48 * 1024) {
         int b = (int)sim->st_smem;
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+
     }
     sim->lg = g;
     sim->stencil_ok = true; sim->stencil_reason = 0;

@@ -24,7 +24,7 @@
 
 constexpr int NSUB_MAX = 8;            // more sublattices than this: use the ELL gather
 constexpr int STENCIL_RMAX = 40;       // larger stencil half-extent: use the ELL gather
-constexpr int ST_OV = 8;               // outputs per thread along v (sliding register window)
+constexpr int ST_OV = 8;               // default outputs per thread along v (sliding register window); 16 is the other variant
 constexpr int ST_TU = 32;              // tile extent along u = one warp
 // one spin-grid cell = the high word of the spin as a double (+1.0, -1.0, or 0 = no magnet): a 4-byte
 // shared-memory load lands directly in the upper register of a DFMA operand whose lower register stays 0
@@ -233,24 +233,6 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // wants >= 4 warps per scheduler); their partial sums are added through shared memory in a fixed order.
 // blockIdx.z = replica * nsub + target sublattice.  blockDim = 32 * NW * RS.
 // ------------------------------------------------------------------------------------------------
-#define FS_ST_LD(K, Z) __hiloint2double((int)sp[K], Z)
-#define FS_ST_FMA(X0, X1, X2, X3, X4, X5, X6, X7, K)                                   \
-        const double2 t##K = CT ? c_T[tofs + K] : tp[K];                               \
-        a0x = fma(X0, t##K.x, a0x); a0y = fma(X0, t##K.y, a0y);                        \
-        a1x = fma(X1, t##K.x, a1x); a1y = fma(X1, t##K.y, a1y);                        \
-        a2x = fma(X2, t##K.x, a2x); a2y = fma(X2, t##K.y, a2y);                        \
-        a3x = fma(X3, t##K.x, a3x); a3y = fma(X3, t##K.y, a3y);                        \
-        a4x = fma(X4, t##K.x, a4x); a4y = fma(X4, t##K.y, a4y);                        \
-        a5x = fma(X5, t##K.x, a5x); a5y = fma(X5, t##K.y, a5y);                        \
-        a6x = fma(X6, t##K.x, a6x); a6y = fma(X6, t##K.y, a6y);                        \
-        a7x = fma(X7, t##K.x, a7x); a7y = fma(X7, t##K.y, a7y);
-// one slot of a full group of 8 (no exit test); slot K consumes the window and refills its oldest cell
-#define FS_ST_FULL(X0, X1, X2, X3, X4, X5, X6, X7, Z, K)                               \
-    { FS_ST_FMA(X0, X1, X2, X3, X4, X5, X6, X7, K) X0 = FS_ST_LD(8 + K, Z); }
-// one slot of the ragged tail
-#define FS_ST_TAIL(X0, X1, X2, X3, X4, X5, X6, X7, Z, K)                               \
-    { FS_ST_FMA(X0, X1, X2, X3, X4, X5, X6, X7, K) if (--n == 0) break; X0 = FS_ST_LD(8 + K, Z); }
-
 // Coupling tables of the lattice that used the stencil last (all sublattice pairs), for the CT variant of
 // k_gather_stencil: a warp-uniform weight read through the constant cache lands in a uniform register,
 // and DFMA R, R, UR, R reads only two vector-register pairs: 62 DFMA/clk/SM measured against 51 with
@@ -260,13 +242,13 @@ constexpr int CR_MAX = 960;            // row intervals (7.5 KB)
 __constant__ double2 c_T[CT_MAX];
 __constant__ int2 c_rows[CR_MAX];
 
-template <int MAXT, int MINB, bool CT>
+template <int MAXT, int MINB, bool CT, int OV>
 __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGrid g, int NW, int Pv,
                                                                const int* __restrict__ gidx, const sgcell_t* __restrict__ sg,
                                                                const double2* __restrict__ T, const int2* __restrict__ rowtab,
                                                                double2* __restrict__ hdip_all) {
     extern __shared__ __align__(16) unsigned char st_raw[];
-    const int RS = (blockDim.x >> 5) / NW, TV = ST_OV * NW;
+    const int RS = (blockDim.x >> 5) / NW, TV = OV * NW;
     const int SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv, WH = g.W * g.H;
     double2* Tsm = reinterpret_cast<double2*>(st_raw);                      // [nsub][WH]
     const size_t tsm_n = CT ? 0 : (size_t)g.nsub * WH;                      // no shared copy of T in the CT variant
@@ -276,7 +258,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     const int si = blockIdx.z % g.nsub, rep = blockIdx.z / g.nsub;
     const int tu0 = blockIdx.x * ST_TU, tv0 = blockIdx.y * TV;       // tile origin, interior coordinates
     // the warp index via a shuffle from lane 0: the compiler then knows everything derived from it is
-    // warp-uniform and keeps row intervals / weight offsets / weights in uniform registers
+    // warp-uniform
     const int wid_u = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31, warp = wid_u % NW, rs = wid_u / NW;
 
@@ -302,14 +284,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     cp_async_wait_all();
     __syncthreads();
 
-    double a0x = 0, a0y = 0, a1x = 0, a1y = 0, a2x = 0, a2y = 0, a3x = 0, a3y = 0;
-    double a4x = 0, a4y = 0, a5x = 0, a5y = 0, a6x = 0, a6y = 0, a7x = 0, a7y = 0;
-    int z0, z1, z2, z3, z4, z5, z6, z7;                // eight zeros the compiler cannot merge: the low words of x0..x7
-    asm volatile("mov.u32 %0, 0; mov.u32 %1, 0; mov.u32 %2, 0; mov.u32 %3, 0; mov.u32 %4, 0; mov.u32 %5, 0; mov.u32 %6, 0; mov.u32 %7, 0;"
-                 : "=r"(z0), "=r"(z1), "=r"(z2), "=r"(z3), "=r"(z4), "=r"(z5), "=r"(z6), "=r"(z7));
+    double ax[OV], ay[OV], x[OV];                      // all indices below are compile-time after unrolling: registers
+#pragma unroll
+    for (int q = 0; q < OV; ++q) { ax[q] = 0.0; ay[q] = 0.0; }
+#define FS_ST_LD(K) __hiloint2double((int)sp[K], 0)
 
     for (int sj = 0; sj < g.nsub; ++sj) {
-        const sgcell_t* Sj = S + ((size_t)sj * SU + lane) * Pv + warp * ST_OV + g.Rv;
+        const sgcell_t* Sj = S + ((size_t)sj * SU + lane) * Pv + warp * OV + g.Rv;
         const double2* Tj = Tsm + (CT ? 0 : (size_t)sj * WH + g.Rv);
         const int tj = (si * g.nsub + sj) * WH + g.Rv;
         // r = du + Ru is a uniform loop counter, so that the row interval and the weight offsets below live
@@ -319,70 +300,66 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
             const int2 rt = CT ? c_rows[(si * g.nsub + sj) * g.W + r] : rows[sj * g.W + r];
             int n = rt.y - rt.x + 1;
             if (n <= 0) continue;
-            // output (lane, warp*8+q) at slot (du, dv) reads S[sj][lane + du + Ru][warp*8 + q + dv + Rv]
+            // output (lane, warp*OV+q) at slot (du, dv) reads S[sj][lane + du + Ru][warp*OV + q + dv + Rv]
             const sgcell_t* sp = Sj + (size_t)r * Pv + rt.x;
             const double2* tp = Tj + (CT ? 0 : r * g.H + rt.x);
             int tofs = tj + r * g.H + rt.x;
-            double x0 = FS_ST_LD(0, z0), x1 = FS_ST_LD(1, z1), x2 = FS_ST_LD(2, z2), x3 = FS_ST_LD(3, z3);
-            double x4 = FS_ST_LD(4, z4), x5 = FS_ST_LD(5, z5), x6 = FS_ST_LD(6, z6), x7 = FS_ST_LD(7, z7);
-            for (; n >= 8; n -= 8, sp += 8, tp += 8, tofs += 8) {
-                FS_ST_FULL(x0, x1, x2, x3, x4, x5, x6, x7, z0, 0)
-                FS_ST_FULL(x1, x2, x3, x4, x5, x6, x7, x0, z1, 1)
-                FS_ST_FULL(x2, x3, x4, x5, x6, x7, x0, x1, z2, 2)
-                FS_ST_FULL(x3, x4, x5, x6, x7, x0, x1, x2, z3, 3)
-                FS_ST_FULL(x4, x5, x6, x7, x0, x1, x2, x3, z4, 4)
-                FS_ST_FULL(x5, x6, x7, x0, x1, x2, x3, x4, z5, 5)
-                FS_ST_FULL(x6, x7, x0, x1, x2, x3, x4, x5, z6, 6)
-                FS_ST_FULL(x7, x0, x1, x2, x3, x4, x5, x6, z7, 7)
+#pragma unroll
+            for (int q = 0; q < OV; ++q) x[q] = FS_ST_LD(q);
+            // full groups of OV slots (no exit test): slot K consumes the window and refills its oldest cell
+            for (; n >= OV; n -= OV, sp += OV, tp += OV, tofs += OV) {
+#pragma unroll
+                for (int K = 0; K < OV; ++K) {
+                    const double2 t = CT ? c_T[tofs + K] : tp[K];
+#pragma unroll
+                    for (int q = 0; q < OV; ++q) {
+                        ax[q] = fma(x[(q + K) % OV], t.x, ax[q]);
+                        ay[q] = fma(x[(q + K) % OV], t.y, ay[q]);
+                    }
+                    x[K] = FS_ST_LD(OV + K);
+                }
             }
-            if (n > 0) do {
-                FS_ST_TAIL(x0, x1, x2, x3, x4, x5, x6, x7, z0, 0)
-                FS_ST_TAIL(x1, x2, x3, x4, x5, x6, x7, x0, z1, 1)
-                FS_ST_TAIL(x2, x3, x4, x5, x6, x7, x0, x1, z2, 2)
-                FS_ST_TAIL(x3, x4, x5, x6, x7, x0, x1, x2, z3, 3)
-                FS_ST_TAIL(x4, x5, x6, x7, x0, x1, x2, x3, z4, 4)
-                FS_ST_TAIL(x5, x6, x7, x0, x1, x2, x3, x4, z5, 5)
-                FS_ST_TAIL(x6, x7, x0, x1, x2, x3, x4, x5, z6, 6)
-            } while (0);
+            if (n > 0) {                               // ragged tail: at most OV - 1 slots
+#pragma unroll
+                for (int K = 0; K < OV - 1; ++K) {
+                    const double2 t = CT ? c_T[tofs + K] : tp[K];
+#pragma unroll
+                    for (int q = 0; q < OV; ++q) {
+                        ax[q] = fma(x[(q + K) % OV], t.x, ax[q]);
+                        ay[q] = fma(x[(q + K) % OV], t.y, ay[q]);
+                    }
+                    if (--n == 0) break;
+                    x[K] = FS_ST_LD(OV + K);
+                }
+            }
         }
     }
-    // ---- epilogue: add the row groups' partial sums (fixed order), scatter the 8 outputs to their spins
+#undef FS_ST_LD
+    // ---- epilogue: add the row groups' partial sums (fixed order), scatter the OV outputs to their spins
     if (RS > 1) {
         __syncthreads();                               // everyone is done with the tiles
         double* red_base = reinterpret_cast<double*>(S);
-        double* red = red_base + ((size_t)((rs - 1) * NW + warp) * 16) * 32 + lane;
+        double* red = red_base + ((size_t)((rs - 1) * NW + warp) * 2 * OV) * 32 + lane;
         if (rs > 0) {
-            red[0 * 32] = a0x; red[1 * 32] = a0y; red[2 * 32] = a1x; red[3 * 32] = a1y;
-            red[4 * 32] = a2x; red[5 * 32] = a2y; red[6 * 32] = a3x; red[7 * 32] = a3y;
-            red[8 * 32] = a4x; red[9 * 32] = a4y; red[10 * 32] = a5x; red[11 * 32] = a5y;
-            red[12 * 32] = a6x; red[13 * 32] = a6y; red[14 * 32] = a7x; red[15 * 32] = a7y;
+#pragma unroll
+            for (int q = 0; q < OV; ++q) { red[(2 * q) * 32] = ax[q]; red[(2 * q + 1) * 32] = ay[q]; }
         }
         __syncthreads();
         if (rs > 0) return;
         for (int k = 1; k < RS; ++k) {
-            const double* rd = red_base + ((size_t)((k - 1) * NW + warp) * 16) * 32 + lane;
-            a0x += rd[0 * 32]; a0y += rd[1 * 32]; a1x += rd[2 * 32]; a1y += rd[3 * 32];
-            a2x += rd[4 * 32]; a2y += rd[5 * 32]; a3x += rd[6 * 32]; a3y += rd[7 * 32];
-            a4x += rd[8 * 32]; a4y += rd[9 * 32]; a5x += rd[10 * 32]; a5y += rd[11 * 32];
-            a6x += rd[12 * 32]; a6y += rd[13 * 32]; a7x += rd[14 * 32]; a7y += rd[15 * 32];
+            const double* rd = red_base + ((size_t)((k - 1) * NW + warp) * 2 * OV) * 32 + lane;
+#pragma unroll
+            for (int q = 0; q < OV; ++q) { ax[q] += rd[(2 * q) * 32]; ay[q] += rd[(2 * q + 1) * 32]; }
         }
     }
     double2* __restrict__ hdip = hdip_all + (int64_t)rep * N;
-    const int* oi = oidx + (warp * ST_OV) * 32 + lane;
-    int i;
-    if ((i = oi[0 * 32]) >= 0) hdip[i] = make_double2(a0x, a0y);
-    if ((i = oi[1 * 32]) >= 0) hdip[i] = make_double2(a1x, a1y);
-    if ((i = oi[2 * 32]) >= 0) hdip[i] = make_double2(a2x, a2y);
-    if ((i = oi[3 * 32]) >= 0) hdip[i] = make_double2(a3x, a3y);
-    if ((i = oi[4 * 32]) >= 0) hdip[i] = make_double2(a4x, a4y);
-    if ((i = oi[5 * 32]) >= 0) hdip[i] = make_double2(a5x, a5y);
-    if ((i = oi[6 * 32]) >= 0) hdip[i] = make_double2(a6x, a6y);
-    if ((i = oi[7 * 32]) >= 0) hdip[i] = make_double2(a7x, a7y);
+    const int* oi = oidx + (warp * OV) * 32 + lane;
+#pragma unroll
+    for (int q = 0; q < OV; ++q) {
+        const int i = oi[q * 32];
+        if (i >= 0) hdip[i] = make_double2(ax[q], ay[q]);
+    }
 }
-#undef FS_ST_FULL
-#undef FS_ST_TAIL
-#undef FS_ST_FMA
-#undef FS_ST_LD
 
 // DFMA-chain calibration: every thread runs 8 independent chains of `iters` DFMAs.
 __global__ void k_dfma_peak(int iters, double seed, double* __restrict__ sink) {
