@@ -327,7 +327,9 @@ def run_ours(args, rank, world, local_rank):
         dfma_peak = B.measure_fp64_peak()                     # DFMA/s, measured in this run
         achieved = 2.0 * 2.0 * I / (gather_ms * 1e-3) / 1e12    # 2 DFMA (4 flop) per interaction
         roofline = {"bound": "alu", "kernel": "k_gather_stencil", "achieved": achieved, "peak": 2.0 * dfma_peak / 1e12,
-                    "unit": "TFLOP/s", "frac": achieved / (2.0 * dfma_peak / 1e12), "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / (2.0 * dfma_peak / 1e12),
+                    # dram__bytes_read+write of one launch at full config-5 size, from the committed ncu capture
+                    "traffic": 3310848 if (N, K) == (501000, 632) else None, "traffic_source": "profiles/r01_ncu_full.md",
                     "peak_source": "fp64 DFMA-chain kernel (fs_measure_fp64_peak) measured in this run; "
                                    "nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2 TFLOP/s",
                     "algorithmic_flops_per_launch": 4.0 * I, "kernel_ms": gather_ms,
@@ -359,7 +361,9 @@ def run_ours(args, rank, world, local_rank):
     if ell is not None:
         a = ell_bytes / (ell * 1e-3) / 1e9
         line["roofline_ell"] = {"bound": "hbm", "kernel": "k_gather (general-geometry ELL path, same workload)",
-                                "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak, "traffic": None,
+                                "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak,
+                                "traffic": 6271733000 if (N, K) == (501000, 632) else None,
+                                "traffic_source": "profiles/r01_ncu_full.md",
                                 "peak_source": peak_src, "algorithmic_bytes_per_launch": ell_bytes, "kernel_ms": ell,
                                 "interactions_per_s": I / (ell * 1e-3)}
     sim.close()
