@@ -496,6 +496,11 @@ def test_sweep_ensemble(B):
         assert np.array_equal(ps[r], np.array(cnt)) and n[r] == sum(cnt)
         assert np.array_equal(sim.get_flip_log(replica=r).cpu().numpy()[: n[r]], np.concatenate(logs)[: 4 * w.N + 1024])
         assert np.array_equal(s[r], o.spins())
+    # the per-replica spin grids followed the sweep: a fresh stencil gather equals a fresh ELL gather
+    assert sim.lattice()["active"]
+    sim.set_gather_variant(B.GATHER_STENCIL); sim.update_fields(); a = sim.get_fields(1).cpu().numpy()
+    sim.set_gather_variant(B.GATHER_ELL_F64); sim.update_fields(); b = sim.get_fields(1).cpu().numpy()
+    assert np.abs(a - b).max() / np.abs(b).max() < 1e-13
 
 
 # ------------------------------------------------------------------ per-spin external field
