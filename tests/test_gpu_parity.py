@@ -537,3 +537,64 @@ def test_local_field_parity(B):
     assert field_err(sim2.get_fields(0).cpu().numpy(), orc2.fields(0)) < FIELD_TOL
     sim2.set_local_field(None); orc2.set_local_field(None)
     assert field_err(sim2.get_fields(2).cpu().numpy(), orc2.fields(2)) < FIELD_TOL
+
+
+# ------------------------------------------------------------------ more edge cases of the boundary
+def test_workspace_errors_and_reuse(B):
+    import ctypes as C
+    import torch
+    L = B.load_library()
+    w = W.config("1")
+    pos = torch.as_tensor(w.pos).cuda(); ang = torch.as_tensor(w.angle).cuda(); hc = torch.as_tensor(w.hc).cuda()
+    p = B.FsParams(*[w.params[k] for k in ("alpha", "b", "c", "beta", "gamma", "neighbor_distance")])
+    nbytes = C.c_size_t()
+    sp = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    assert L.fs_workspace_bytes(w.N, 1, pos.data_ptr(), C.byref(p), C.byref(nbytes), sp) == 0 and nbytes.value > 0
+    ws = torch.empty(nbytes.value + 512, dtype=torch.uint8, device="cuda")
+    base = (ws.data_ptr() + 255) // 256 * 256
+    h = C.c_void_p()
+    # too small, then misaligned: both refused with FS_ERR_WORKSPACE and a message, no handle created
+    assert L.fs_create(C.byref(h), w.N, pos.data_ptr(), ang.data_ptr(), hc.data_ptr(), C.byref(p), base, 1024, sp) == B.FS_ERR_WORKSPACE
+    assert b"workspace" in L.fs_last_error()
+    assert L.fs_create(C.byref(h), w.N, pos.data_ptr(), ang.data_ptr(), hc.data_ptr(), C.byref(p), base + 8, nbytes.value, sp) == B.FS_ERR_WORKSPACE
+    # exact size works; the same workspace can be reused after fs_destroy
+    for _ in range(2):
+        assert L.fs_create(C.byref(h), w.N, pos.data_ptr(), ang.data_ptr(), hc.data_ptr(), C.byref(p), base, nbytes.value, sp) == 0
+        n = C.c_int64()
+        assert L.fs_set_field(h, -0.2, -0.2, 0) == 0 and L.fs_relax(h, 0, C.byref(n)) == 0 and n.value == w.N
+        assert L.fs_destroy(h) == 0
+    # null pointers and bad selectors are reported, not dereferenced
+    assert L.fs_get_fields(None, 0, None) == B.FS_ERR_ARG
+    assert L.fs_sweep(None, None, 3, 0, None, 0, None) == B.FS_ERR_ARG
+
+
+def test_sweep_max_flips_cap(B):
+    w = W.config("1")
+    sim, orc = mk(B, w)
+    n, ps = sim.sweep(w.fields, step0=0, max_flips=100)
+    assert n[0] == 100 and int(ps.sum().item()) == 100          # stopped inside the protocol, state still valid
+    ref = []
+    for t, (hx, hy) in enumerate(w.fields):
+        orc.set_field(hx, hy, t); ref.append(orc.relax_B()[1])
+        if sum(len(r) for r in ref) >= 100:
+            break
+    assert np.array_equal(sim.get_flip_log().cpu().numpy()[:100], np.concatenate(ref)[:100])
+
+
+def test_many_replicas_more_than_sms(B):
+    """R = 300 replicas (> 148 SMs, several CTAs per SM and more than one wave of relax CTAs)."""
+    from oracle import Oracle
+    pos, ang = W.square_closed(3)
+    N = len(ang); R = 300
+    p = dict(alpha=0.002, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    hc = W.coercive_fields(N, seed=40, replicas=R)
+    sim = B.Sim(pos, ang, hc, p)
+    sim.set_field(-0.15, -0.16, 0)
+    n = sim.relax_ensemble()
+    s = sim.get_spins().cpu().numpy()
+    for r in (0, 1, 147, 148, 149, 299):
+        o = Oracle(pos, ang, hc[r], p)
+        o.set_field(-0.15, -0.16, 0)
+        no, log = o.relax_B()
+        assert n[r] == no and np.array_equal(sim.get_flip_log(replica=r).cpu().numpy(), log)
+        assert np.array_equal(s[r], o.spins())
