@@ -170,6 +170,13 @@ int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out /*HOS
 int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
              int64_t max_flips, int64_t* n_flips_out);
 
+/* fs_sweep with a thermal field strength per step: sigma_dev DEVICE [T] (annealing with an
+ * exponentially decreasing thermal field); NULL = the constant sigma of fs_set_thermal.  The seed is the one
+ * of fs_set_thermal; after the call fs_get_fields(THERMAL/TOTAL) still uses fs_set_thermal's sigma (call
+ * fs_set_thermal with the last value to read the final thermal field). */
+int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_dev, int32_t T, uint32_t step0,
+                    int64_t* flips_per_step_dev, int64_t max_flips, int64_t* n_flips_out);
+
 /* Counters accumulated on the device since creation / the last reset: HOST [R] each (any may be
  * NULL).  Synchronises. */
 int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset);

@@ -23,7 +23,7 @@ EXPORTS = [
     "fs_get_spins", "fs_set_thermal", "fs_set_field", "fs_set_field_ensemble", "fs_set_gather_variant",
     "fs_update_fields", "fs_scan", "fs_scan_ensemble", "fs_relax", "fs_relax_ensemble", "fs_get_counters",
     "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
-    "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep", "fs_set_local_field",
+    "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep", "fs_sweep_anneal", "fs_set_local_field",
 ]
 
 
@@ -77,6 +77,7 @@ def load_library(path: str | None = None):
         "fs_get_lattice": [vp, vp, vp],
         "fs_sweep": [vp, vp, i32, C.c_uint32, vp, i64, vp],
         "fs_set_local_field": [vp, vp],
+        "fs_sweep_anneal": [vp, vp, vp, i32, C.c_uint32, vp, i64, vp],
         "fs_measure_fp64_peak": [P(dbl), vp],
     }
     for name, args in sig.items():
@@ -226,17 +227,20 @@ class Sim:
         _check(self.L, self.L.fs_relax(self.h, int(max_flips), C.byref(n)), allow=(FS_ERR_MAXFLIPS,))
         return int(n.value)
 
-    def sweep(self, fields, step0=0, per_step=True, max_flips=0, sync=True):
-        """Whole protocol in one launch.  fields [T,2].  Returns (flips per replica [R] or None if not sync,
-        flips per step tensor [R,T] on the device or None)."""
+    def sweep(self, fields, step0=0, per_step=True, max_flips=0, sync=True, sigma=None):
+        """Whole protocol in one launch.  fields [T,2]; sigma [T] = thermal std per step (annealing) or None.
+        Returns (flips per replica [R] or None if not sync, flips per step tensor [R,T] on the device or None)."""
         f = torch.as_tensor(np.ascontiguousarray(fields, np.float64)).to(self.device)
         T = int(f.shape[0])
+        sg = None if sigma is None else torch.as_tensor(np.ascontiguousarray(sigma, np.float64)).to(self.device)
+        assert sg is None or sg.numel() == T
         ps = torch.zeros((self.R, T), dtype=torch.int64, device=self.device) if per_step else None
         n = np.zeros(self.R, np.int64)
-        _check(self.L, self.L.fs_sweep(self.h, f.data_ptr(), T, int(step0), ps.data_ptr() if per_step else None,
-                                       int(max_flips), n.ctypes.data if sync else None), allow=(FS_ERR_MAXFLIPS,))
+        _check(self.L, self.L.fs_sweep_anneal(self.h, f.data_ptr(), None if sg is None else sg.data_ptr(), T, int(step0),
+                                              ps.data_ptr() if per_step else None, int(max_flips),
+                                              n.ctypes.data if sync else None), allow=(FS_ERR_MAXFLIPS,))
         if not sync:
-            self._keep = f                                 # the kernel reads it asynchronously
+            self._keep = (f, sg)                           # the kernel reads them asynchronously
         return (n if sync else None), ps
 
     def relax_ensemble(self, max_flips=0):

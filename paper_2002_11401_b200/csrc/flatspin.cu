@@ -634,7 +634,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         // sweep mode (T > 0): the CTA runs a whole field protocol, scanning its replica itself at every step
         int T, const double2* __restrict__ sweep_fields /*[T] (hx,hy)*/, FieldSpec fs, const double2* __restrict__ cs,
         long long* __restrict__ flips_per_step /*[R,T] or NULL*/, double2* __restrict__ hext_all,
-        const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/) {
+        const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/,
+        const double* __restrict__ sweep_sigma /*[T] thermal std per step (annealing) or NULL*/) {
     // four-level arg-max hierarchy in shared memory:
     // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
     extern __shared__ unsigned char smem_raw[];
@@ -674,6 +675,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         // ---- A4-A7 inside the CTA (sweep mode): one warp per leaf, same arithmetic as k_scan
         const double2 he = sweep_fields[st];
         FieldSpec f2 = fs; f2.step = fs.step + (uint32_t)st;
+        if (sweep_sigma) f2.sigma = sweep_sigma[st];
         for (int b = warp; b < nblk; b += NW) {
             mkey_t bv = 0ull; int bi = 0x7fffffff;
             for (int q = lane; q < LB; q += 32) {
@@ -1407,7 +1409,8 @@ int fetch_counters(fs_sim* sim) {
 }
 
 // T == 0: relax at the field set by fs_set_field (k_scan first); T > 0: whole protocol in one launch
-int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_dev, uint32_t step0, long long* per_step_dev) {
+int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_dev, uint32_t step0, long long* per_step_dev,
+                 const double* sigma_dev = nullptr) {
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
     FieldSpec fsp{sim->sigma, sim->seed, T > 0 ? step0 : sim->step};
     k_relax<<<sim->R, RELAX_THREADS, sim->relax_smem, sim->stream>>>(
@@ -1415,7 +1418,7 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr,
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid,
         sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0,
-        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc);
+        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev);
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -1755,14 +1758,14 @@ int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
     return capped ? fail(FS_ERR_MAXFLIPS, "relax stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
 }
 
-int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
-             int64_t max_flips, int64_t* n_flips_out) {
+int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_dev, int32_t T, uint32_t step0,
+                    int64_t* flips_per_step_dev, int64_t max_flips, int64_t* n_flips_out) {
     if (!sim || !fields_dev) return fail(FS_ERR_ARG, "null pointer");
     if (T <= 0) return fail(FS_ERR_ARG, "T=%d must be positive", (int)T);
     int rc = ensure_fields(sim);
     if (rc) return rc;
     rc = launch_relax(sim, max_flips, T, reinterpret_cast<const double2*>(fields_dev), step0,
-                      reinterpret_cast<long long*>(flips_per_step_dev));
+                      reinterpret_cast<long long*>(flips_per_step_dev), sigma_dev);
     if (rc) return rc;
     sim->step = step0 + (uint32_t)(T - 1);
     if (!n_flips_out) return FS_OK;
@@ -1771,6 +1774,11 @@ int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, i
     int capped = 0;
     for (int r = 0; r < sim->R; ++r) { n_flips_out[r] = sim->ctr_host[r].last_flips; capped |= sim->ctr_host[r].status; }
     return capped ? fail(FS_ERR_MAXFLIPS, "sweep stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
+}
+
+int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
+             int64_t max_flips, int64_t* n_flips_out) {
+    return fs_sweep_anneal(sim, fields_dev, nullptr, T, step0, flips_per_step_dev, max_flips, n_flips_out);
 }
 
 int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset) {

@@ -598,3 +598,30 @@ def test_many_replicas_more_than_sms(B):
         no, log = o.relax_B()
         assert n[r] == no and np.array_equal(sim.get_flip_log(replica=r).cpu().numpy(), log)
         assert np.array_equal(s[r], o.spins())
+
+
+def test_annealing_sweep_matches_oracle(B):
+    """annealing = a protocol whose thermal field strength decreases exponentially.  One launch
+    (fs_sweep_anneal) against the oracle stepping the same sigma_t, on the 50x50-style recipe of PAPER.md:196
+    scaled down (square closed, b = 0.4, nd = 3), zero external field."""
+    pos, ang = W.square_closed(14)
+    N = len(ang)
+    p = dict(alpha=0.0018, b=0.4, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=3.0)
+    hc = W.coercive_fields(N, hk=0.186, seed=9)
+    spins = W.random_spins(N, seed=4)
+    from oracle import Oracle
+    sim = B.Sim(pos, ang, hc, p); sim.set_spins(spins); sim.set_thermal(0.0, 77)
+    orc = Oracle(pos, ang, hc, p, spins=spins)
+    T = 60
+    sigma = 0.12 * np.exp(-np.arange(T) / 12.0)
+    fields = np.zeros((T, 2))
+    cnt = []
+    for t in range(T):
+        orc.set_thermal(float(sigma[t]), 77); orc.set_field(0.0, 0.0, t)
+        cnt.append(orc.relax_B()[0])
+    n, ps = sim.sweep(fields, step0=0, sigma=sigma)
+    assert sum(cnt) > 50 and np.array_equal(ps.cpu().numpy()[0], np.array(cnt))
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    sim.set_thermal(float(sigma[-1]), 77)
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    assert orc.monitor()[0] == 0
