@@ -58,6 +58,12 @@ def rotated_square(n: int, rot: float = math.pi / 4):
     return pos, angle + rot
 
 
+def pinwheel_lucky_knot(n: int, rot: float = math.pi / 4):
+    """Pinwheel "lucky-knot" edges (Fig. 3e): the closed-square lattice with every magnet rotated
+    45 degrees -> N = 2 n (n+1).  Same construction as BASELINE.json config 3 (`rotated_square`)."""
+    return rotated_square(n, rot)
+
+
 def pinwheel_diamond(n: int, rot: float = math.pi / 4):
     """Pinwheel "diamond" with 2 n^2 magnets (PAPER.md:286: 25x25 -> 1250; :288: 708x708 -> >1e6).
 
