@@ -59,7 +59,6 @@ int fail(int code, const char* fmt, ...) {
     } while (0)
 #define LAUNCHED() (g_launches.fetch_add(1, std::memory_order_relaxed))
 
-constexpr int RELAX_THREADS = 512;
 constexpr int MAX_LEAF_BLOCKS = 8192;   // leaf-block maxima kept in the relax CTA's shared memory
 constexpr int MAX_K = 8192;             // maximum degree supported by the warp bitonic sort
 
@@ -624,7 +623,8 @@ __device__ __forceinline__ void repair_group(int grp, int nblk, const mkey_t* bk
     if ((threadIdx.x & 31) == 0) { gkey[grp] = v; gidx_[grp] = i; }
 }
 
-__global__ void __launch_bounds__(RELAX_THREADS, 1)
+template <int RELAX_THREADS>                           // 512 (one big system per CTA) or 128 (ensembles of small systems)
+__global__ void __launch_bounds__(RELAX_THREADS, RELAX_THREADS == 128 ? 8 : (RELAX_THREADS == 64 ? 16 : 1))
 k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_flips, long long log_cap,
         const int* __restrict__ nbr, const double2* __restrict__ wT, const double* __restrict__ ihc_all,
         int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, double2* __restrict__ hfix_all,
@@ -1413,12 +1413,19 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
                  const double* sigma_dev = nullptr) {
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
     FieldSpec fsp{sim->sigma, sim->seed, T > 0 ? step0 : sim->step};
-    k_relax<<<sim->R, RELAX_THREADS, sim->relax_smem, sim->stream>>>(
-        sim->N, sim->Kp, lb_shift, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr,
-        sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr,
-        sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid,
-        sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0,
-        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev);
+    // ensembles of small systems: when there are more replicas than SMs and the whole update fits one warp,
+    // 128-thread CTAs (8 per SM, 64 registers) instead of 512-thread ones (1 per SM); beyond 8 replicas per
+    // SM, 64-thread CTAs (16 per SM).  Measured on 220-spin replicas: 75k / 421k / 539k replica-sweeps per s.
+    const bool small_cta = sim->R > sim->sm_count && sim->Kp + 1 <= 32 && sim->nblk <= 1024;
+#define FS_RELAX_ARGS sim->N, sim->Kp, lb_shift, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr, \
+        sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr, \
+        sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid, \
+        sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0, \
+        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev
+    if (small_cta && sim->R > 8 * sim->sm_count) k_relax<64><<<sim->R, 64, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+    else if (small_cta) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+    else k_relax<512><<<sim->R, 512, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+#undef FS_RELAX_ARGS
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
@@ -1556,7 +1563,9 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
         LAUNCHED();
     }
     sim->relax_smem = ((size_t)nblk + (size_t)(nblk + 31) / 32 + 8) * 12 + (size_t)(Kp + 1) * 4 + 32;
-    CREATE_TRY(cudaFuncSetAttribute(k_relax, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
+    CREATE_TRY(cudaFuncSetAttribute(k_relax<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
+    CREATE_TRY(cudaFuncSetAttribute(k_relax<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
+    CREATE_TRY(cudaFuncSetAttribute(k_relax<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
     int hflags = 0;
     CREATE_TRY(cudaMemcpyAsync(&hflags, scr + 8, sizeof(int), cudaMemcpyDeviceToHost, st));
     CREATE_TRY(cudaStreamSynchronize(st));
