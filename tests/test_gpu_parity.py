@@ -625,3 +625,28 @@ def test_annealing_sweep_matches_oracle(B):
     sim.set_thermal(float(sigma[-1]), 77)
     assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
     assert orc.monitor()[0] == 0
+
+
+@pytest.mark.parametrize("which,scale,stride", [("4", 120, 1), ("3", 50, 4), ("2", 30, 2), ("1", 24, 1)])
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_other_disorder_and_thermal_seeds(B, which, scale, stride, seed):
+    """Bit-exact flip sequences are not luck of seed 0: other h_c disorder draws and thermal seeds."""
+    from oracle import Oracle
+    w = W.config(which, scale=scale)
+    hc = W.coercive_fields(w.N, seed=seed)
+    sim = B.Sim(w.pos, w.angle, hc, w.params); orc = Oracle(w.pos, w.angle, hc, w.params, spins=w.spins)
+    sim.set_spins(w.spins)
+    if w.sigma_th:
+        sim.set_thermal(w.sigma_th, seed + 10); orc.set_thermal(w.sigma_th, seed + 10)
+    total = 0
+    for t, (hx, hy) in list(enumerate(w.fields))[::stride]:
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        n = sim.relax(); no, log = orc.relax_B()
+        if n != no or (n and not np.array_equal(sim.get_flip_log().cpu().numpy(), log)):
+            ev, gap, thr = orc.monitor()
+            assert ev > 0, f"flip sequence differs at step {t} with no near-tie recorded"
+            pytest.xfail(f"near-tie at step {t} (gap {gap:.1e}): order not well posed")
+        total += n
+    assert total >= w.N
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
