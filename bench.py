@@ -230,6 +230,35 @@ def protocol_sweeps(B, torch, cpu=True):
     return out, ens
 
 
+def paper_workloads(B, torch):
+    """The two timings the paper itself prints besides Fig. 9, on its own parameter set
+    (section IV.C; the field range is not printed, workloads.paper_pinwheel_reversal states the choice):
+    one reversal of the 25 x 25 pinwheel ASI (1250 magnets, K = 2500 field values; paper: ~6 s including
+    result storage) and of the 708 x 708 pinwheel ASI (1,002,528 magnets; paper: "several days")."""
+    out = []
+    for n, paper in ((25, "approximately 6 seconds (PAPER.md:286)"), (708, "several days (PAPER.md:288)")):
+        w = W.paper_pinwheel_reversal(n, 0.0)
+        t0 = time.perf_counter()
+        sim = B.Sim(w.pos, w.angle, w.hc, w.params); torch.cuda.synchronize(); tc = time.perf_counter() - t0
+        sim.set_spins(w.spins); sim.update_fields(); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for t, (hx, hy) in enumerate(w.fields):
+            sim.set_field(hx, hy, t); sim.relax(sync=False)
+        torch.cuda.synchronize(); dt = time.perf_counter() - t0
+        flips = int(sim.counters()[0].sum())
+        s = sim.get_spins()
+        row = {"workload": w.name, "N": w.N, "K_neighbors": sim.K, "field_values": len(w.fields), "create_s": tc,
+               "reversal_wall_s": dt, "flips": flips, "reversed": bool((s == -torch.as_tensor(w.spins, device=s.device)).all().item()),
+               "paper": paper + ", Tesla V100, other hardware and includes I/O: context, not a target"}
+        if n == 25:
+            sim.set_spins(w.spins); sim.update_fields(); torch.cuda.synchronize(); t0 = time.perf_counter()
+            sim.sweep(w.fields, per_step=False, sync=False); torch.cuda.synchronize()
+            row["one_launch_wall_s"] = time.perf_counter() - t0
+        sim.close()
+        out.append(row)
+    return out
+
+
 def max_over_ranks(dist, values_ms, device):
     """Replicas only: every rank times its own replica; the job's time is the slowest rank's."""
     import torch
@@ -392,6 +421,10 @@ def run_ours(args, rank, world, local_rank):
             line["sweeps"], line["ensemble"] = protocol_sweeps(B, torch, cpu=not args.no_cpu)
         except Exception as e:
             line["sweeps"] = {"error": repr(e)}
+        try:
+            line["paper_workloads"] = paper_workloads(B, torch)
+        except Exception as e:
+            line["paper_workloads"] = {"error": repr(e)}
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

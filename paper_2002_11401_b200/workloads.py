@@ -217,3 +217,30 @@ def config(which, scale: int | None = None) -> Workload:
                         np.array([[0.10 * math.cos(phi), 0.10 * math.sin(phi)]]),
                         note="field + scan only, spins not flipped")
     raise ValueError(f"unknown config {which!r}")
+
+
+# --------------------------------------------------------------------------- the paper's own parameter sets
+def paper_pinwheel_reversal(n: int = 25, theta_deg: float = 0.0, K: int = 2500, amplitude: float = 0.08) -> Workload:
+    """PAPER.md:220-240 (section IV.C) and :286-288: pinwheel "diamond" ASI of n x n units (25 -> 1250 magnets,
+    708 -> 1,002,528), b = 0.28, c = 1, beta = 4.8, gamma = 3, alpha = 0.00033, h_k = 0.098, k_disorder = 0.05,
+    neighbor distance 10, one reversal in K = 2500 field values at angle theta (0, -6, 30 degrees in Fig. 7).
+    The paper does not print the field range: `amplitude` (+A -> -A, enough to reverse the array) is this
+    recipe's choice; the array starts polarised along +x."""
+    pos, ang = pinwheel_diamond(n)
+    spins = np.where(np.cos(ang) > 0, 1, -1).astype(np.int8)
+    return Workload(f"paperIVC_pinwheel_diamond_{n}x{n}_theta{theta_deg:g}", pos, ang,
+                    coercive_fields(len(ang), hk=0.098, k_disorder=0.05, seed=0), spins,
+                    _params(0.00033, 0.28, 1.0, 4.8, 3.0, 10.0), ramp(amplitude, -amplitude, K, theta_deg, legs=1),
+                    note="PAPER.md:230 parameters; field range not given in the paper")
+
+
+def paper_kagome_dirac_strings(n: int = 29, K: int = 400, amplitude: float = 0.12) -> Workload:
+    """PAPER.md:174-188 (section IV.A): kagome ASI of 29 x 29 hexagons (2638 magnets) polarised to the left,
+    reversal field to the right with a downward offset of 3.6 degrees; alpha = 0.00103, h_k = 0.216, beta = 2.5,
+    gamma = 3, b = 0.212, c = 1, sigma_th = 0.002, k_disorder = 0.05.  Neighbourhood and field range are not
+    printed: neighbor distance sqrt(3) (as BASELINE.json config 2) and 0 -> +A in K steps are this recipe's."""
+    pos, ang = kagome(n)
+    spins = np.where(np.cos(ang) > 1e-9, -1, np.where(np.cos(ang) < -1e-9, 1, -1)).astype(np.int8)   # m_x <= 0
+    return Workload(f"paperIVA_kagome_{n}x{n}", pos, ang, coercive_fields(len(ang), hk=0.216, k_disorder=0.05, seed=0),
+                    spins, _params(0.00103, 0.212, 1.0, 2.5, 3.0, SQRT3), ramp(0.0, amplitude, K, -3.6, legs=1),
+                    sigma_th=0.002, thermal_seed=0, note="PAPER.md:182 parameters; neighbourhood and field range not given")

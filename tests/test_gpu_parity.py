@@ -650,3 +650,21 @@ def test_other_disorder_and_thermal_seeds(B, which, scale, stride, seed):
     assert total >= w.N
     assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
     assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+
+
+# ------------------------------------------------------------------ the paper's own parameter sets as workloads
+def test_paper_pinwheel_reversal_parameters(B):
+    """PAPER.md:230 (IV.C): 25x25 pinwheel diamond = 1250 magnets, nd = 10, beta = 4.8 (general
+    exponent path), field at 30 degrees: two-step reversal.  Every 25th of the 2501 field values."""
+    w = W.paper_pinwheel_reversal(25, 30.0)
+    assert w.N == 1250
+    total, sim, orc = run_parity(B, w, stride=25)
+    assert total >= w.N and sim.K == 632
+
+
+def test_paper_kagome_dirac_string_parameters(B):
+    """PAPER.md:180-182 (IV.A): 29x29 hexagons = 2638 magnets, beta = 2.5, b = 0.212, sigma_th = 0.002."""
+    w = W.paper_kagome_dirac_strings(29, K=200)
+    assert w.N == 2638
+    total, sim, orc = run_parity(B, w, stride=2)
+    assert total > w.N // 4
