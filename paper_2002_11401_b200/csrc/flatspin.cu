@@ -719,7 +719,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             if (!stop && max_flips > 0 && nflips >= max_flips) { stop = true; status = 1; }
             if (stop) k = -1;
             if (lane == 0) { sh_k = k; sh_stop = stop ? 1 + status : 0; sh_ntouched = 0; }
-        } else if (warp >= PF_W0) {
+        } else if (warp >= PF_W0 && one_warp) {         // (with K + 1 > 32 every warp is needed for the update itself)
             // ---- prefetch engines (not on the critical path): the best spin of every 8th group is a likely
             // future flip.  Iteration n brings its ELL row to L2; iteration n+1 reads the row (an L2 hit by
             // then) and brings its neighbours' state, its coupling row and its own leaf of margins to L2.
@@ -1424,6 +1424,7 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
         T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev
     if (small_cta && sim->R > 8 * sim->sm_count) k_relax<64><<<sim->R, 64, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else if (small_cta) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+    else if (sim->Kp + 1 > 512 && env_int("FS_RELAX_1024", 1)) k_relax<1024><<<sim->R, 1024, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else k_relax<512><<<sim->R, 512, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
 #undef FS_RELAX_ARGS
     LAUNCHED();
@@ -1566,6 +1567,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     CREATE_TRY(cudaFuncSetAttribute(k_relax<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
     CREATE_TRY(cudaFuncSetAttribute(k_relax<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
     CREATE_TRY(cudaFuncSetAttribute(k_relax<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
+    CREATE_TRY(cudaFuncSetAttribute(k_relax<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
     int hflags = 0;
     CREATE_TRY(cudaMemcpyAsync(&hflags, scr + 8, sizeof(int), cudaMemcpyDeviceToHost, st));
     CREATE_TRY(cudaStreamSynchronize(st));
