@@ -798,13 +798,19 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
                         asm volatile("prefetch.global.L2 [%0];" ::"l"(wT + (int64_t)i * Kp));
                     }
                 }
-                // distinct leaf blocks of this warp's entries -> compact list (duplicates across warps are harmless)
-                unsigned same = __match_any_sync(0xffffffffu, blk);
-                bool leader = blk >= 0 && (__ffs(same) - 1) == lane;
+                // leaf blocks to rescan -> compact list.  Duplicates are harmless (the same leaf is rescanned
+                // twice with the same result), so they are only removed cheaply: ELL rows are sorted, hence the
+                // leaf index is non-decreasing along the lanes and a compare with the previous lane finds
+                // nearly all repeats (a MATCH.ANY here cost ~450 cycles on the per-flip critical path).
+                int prev = __shfl_up_sync(0xffffffffu, blk, 1);
+                if (lane == 0) prev = -2;
+                const bool leader = blk >= 0 && blk != prev;
                 unsigned lead = __ballot_sync(0xffffffffu, leader);
                 int base = 0;
-                if (lane == 0 && lead) base = one_warp ? 0 : atomicAdd(&sh_ntouched, __popc(lead));
-                base = __shfl_sync(0xffffffffu, base, 0);
+                if (!one_warp) {
+                    if (lane == 0 && lead) base = atomicAdd(&sh_ntouched, __popc(lead));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                }
                 if (leader) touched[base + __popc(lead & ((1u << lane) - 1u))] = blk;
                 if (one_warp && lane == 0) sh_ntouched = __popc(lead);
             }
