@@ -158,6 +158,19 @@ int fs_scan_ensemble(fs_sim* sim, int64_t* n_switchable /*HOST [R]*/, int64_t* b
 int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out);
 int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out /*HOST [R]*/);
 
+/* Exact batched flips: for one large system (R = 1, 1 <= K <= 64, N >= 16384, no max_flips cap)
+ * fs_relax first runs a kernel on all SMs that commits, per round, the longest prefix of the sequential flip
+ * sequence of PAPER.md:122 (":129-130 switching is sequential") that it can prove exact: up to `max_seeds` top
+ * candidates, joined into components where their closed neighbourhoods overlap, each relaxed locally by one warp,
+ * merged by effective key, cut at the first conflict (batch.cuh has the argument).  The flip log, spins and fields
+ * are identical to the one-flip-at-a-time loop, which still finishes the tail once fewer than `seq_threshold`
+ * spins are switchable.  max_seeds = 0 switches the batched kernel off; the default is min(4096, N / (8 (K+1))).
+ * fs_get_batch_stats: out4 HOST [4] = {max_seeds in use (0 = off), flips committed by the batched kernel, its
+ * rounds (mean committed prefix = flips / rounds), seq_threshold} since creation / the last counter reset.
+ * Synchronises. */
+int fs_set_batch(fs_sim* sim, int32_t max_seeds, int32_t seq_threshold);
+int fs_get_batch_stats(fs_sim* sim, int64_t* out4);
+
 /* A whole field protocol in ONE launch (PAPER.md:63 "discrete time series"; :124 relaxed at each value):
  * for t = 0..T-1 { global field fields[t]; thermal step key step0 + t; scan (Eqs. 2, 5, 6); relax
  * }, one persistent CTA per replica doing the scan itself, no host involvement between
@@ -166,7 +179,10 @@ int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out /*HOS
  * multi-kernel path scans faster.  fields_dev DEVICE [T,2] (hx,hy), shared by all replicas;
  * flips_per_step_dev DEVICE [R,T] int64 or NULL; max_flips <= 0: unlimited (cap on the whole sweep);
  * n_flips_out HOST [R] (total flips of the sweep) or NULL = asynchronous.  The flip log
- * (fs_get_flip_log) then holds the flips of the whole sweep in order (first 4N+1024). */
+ * (fs_get_flip_log) then holds the flips of the whole sweep in order (first 4N+1024).
+ * If the cap stops a replica inside the protocol (FS_ERR_MAXFLIPS, reported only with n_flips_out != NULL) its
+ * state is that of the step it reached: the global field is fields[that step], flips_per_step of the steps
+ * never run is 0, and the thermal step key used by fs_get_fields becomes step0 + (the step replica 0 reached). */
 int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
              int64_t max_flips, int64_t* n_flips_out);
 

@@ -24,6 +24,7 @@ EXPORTS = [
     "fs_update_fields", "fs_scan", "fs_scan_ensemble", "fs_relax", "fs_relax_ensemble", "fs_get_counters",
     "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
     "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep", "fs_sweep_anneal", "fs_set_local_field",
+    "fs_set_batch", "fs_get_batch_stats",
 ]
 
 
@@ -79,6 +80,8 @@ def load_library(path: str | None = None):
         "fs_set_local_field": [vp, vp],
         "fs_sweep_anneal": [vp, vp, vp, i32, C.c_uint32, vp, i64, vp],
         "fs_measure_fp64_peak": [P(dbl), vp],
+        "fs_set_batch": [vp, i32, i32],
+        "fs_get_batch_stats": [vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -193,6 +196,15 @@ class Sim:
 
     def set_gather_variant(self, v):
         _check(self.L, self.L.fs_set_gather_variant(self.h, int(v)))
+
+    def set_batch(self, max_seeds, seq_threshold=64):
+        """Exact batched flips: seeds per round (0 = off) and the candidate count below which k_relax takes over."""
+        _check(self.L, self.L.fs_set_batch(self.h, int(max_seeds), int(seq_threshold)))
+
+    def batch_stats(self) -> dict:
+        out = np.zeros(4, np.int64)
+        _check(self.L, self.L.fs_get_batch_stats(self.h, out.ctypes.data))
+        return {"max_seeds": int(out[0]), "flips": int(out[1]), "rounds": int(out[2]), "seq_threshold": int(out[3])}
 
     def lattice(self) -> dict:
         info = np.zeros(10, np.int32); d = np.zeros(2, np.float64)

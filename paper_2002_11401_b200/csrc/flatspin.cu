@@ -43,9 +43,9 @@ thread_local char g_err[512] = "";
 std::atomic<long long> g_launches{0};
 // ownership of the constant-memory coupling table (lattice.cuh c_T)
 std::mutex g_ct_mutex;
-unsigned long long g_ct_owner = 0;
+unsigned long long g_ct_owner_dev[64] = {0};               // per device: __constant__ memory and events are per device
 std::atomic<unsigned long long> g_ct_next_id{0};
-cudaEvent_t g_ct_event = nullptr;
+cudaEvent_t g_ct_event_dev[64] = {nullptr};
 
 int fail(int code, const char* fmt, ...) {
     va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof(g_err), fmt, ap); va_end(ap);
@@ -64,11 +64,31 @@ constexpr int MAX_K = 8192;             // maximum degree supported by the warp 
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
-// tuning overrides for experiments (unset in normal use)
-int env_int(const char* name, int dflt) {
-    const char* v = std::getenv(name);
-    return v && *v ? std::atoi(v) : dflt;
+// The dynamic shared-memory limit is an attribute of the kernel function (per device), not of a simulation:
+// it is only ever raised, so that simulations of different sizes can coexist in one process.
+constexpr int MAX_DEVICES = 64;
+std::mutex g_smem_mutex;
+template <typename F>
+cudaError_t raise_smem_limit(F* func, size_t bytes) {
+    static size_t current[MAX_DEVICES] = {0};          // one table per kernel instantiation
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(g_smem_mutex);
+    if (dev < 0 || dev >= MAX_DEVICES) return cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (bytes <= current[dev]) return cudaSuccess;
+    e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) current[dev] = bytes;
+    return e;
 }
+
+// every entry point runs on the simulation's device, whatever device is current in the calling thread
+struct DeviceGuard {
+    int prev = -1, dev;
+    explicit DeviceGuard(int d) : dev(d) { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; if (prev != dev) cudaSetDevice(dev); }
+    ~DeviceGuard() { if (prev >= 0 && prev != dev) cudaSetDevice(prev); }
+};
 
 struct Counters {            // one per replica, device resident
     long long total_flips;
@@ -77,6 +97,9 @@ struct Counters {            // one per replica, device resident
     long long best_index;
     double best_L;
     int status;              // 1 = stopped by max_flips
+    int last_step;           // sweep mode: index of the last step reached (T - 1 unless the cap stopped it)
+    long long batch_flips;   // flips committed by k_relax_batch in the current relax (k_relax continues from here)
+    long long batch_total, batch_rounds;   // since creation / the last reset: flips and rounds of k_relax_batch
     unsigned int ticket;     // k_scan: CTAs of this replica that have finished (last one finalises)
     unsigned long long acc_switch;   // k_scan: running count of switchable spins
 };
@@ -623,6 +646,8 @@ __device__ __forceinline__ void repair_group(int grp, int nblk, const mkey_t* bk
     if ((threadIdx.x & 31) == 0) { gkey[grp] = v; gidx_[grp] = i; }
 }
 
+#include "batch.cuh"
+
 template <int RELAX_THREADS>                           // 512 (one big system per CTA) or 128 (ensembles of small systems)
 __global__ void __launch_bounds__(RELAX_THREADS, RELAX_THREADS == 128 ? 8 : (RELAX_THREADS == 64 ? 16 : 1))
 k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_flips, long long log_cap,
@@ -635,7 +660,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         int T, const double2* __restrict__ sweep_fields /*[T] (hx,hy)*/, FieldSpec fs, const double2* __restrict__ cs,
         long long* __restrict__ flips_per_step /*[R,T] or NULL*/, double2* __restrict__ hext_all,
         const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/,
-        const double* __restrict__ sweep_sigma /*[T] thermal std per step (annealing) or NULL*/) {
+        const double* __restrict__ sweep_sigma /*[T] thermal std per step (annealing) or NULL*/,
+        int use_base /*continue the flip count and log of k_relax_batch (ctr[r].batch_flips)*/) {
     // four-level arg-max hierarchy in shared memory:
     // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
     extern __shared__ unsigned char smem_raw[];
@@ -661,7 +687,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     constexpr int NW = RELAX_THREADS / 32;
     const bool one_warp = (Kp + 1 <= 32);               // the whole update fits one warp: no broadcast of k needed
 
-    long long nflips = 0;
+    long long nflips = use_base ? ctr[r].batch_flips : 0;
+    const long long nflips0 = nflips;
     int status = 0;
 #ifdef FS_RELAX_PROFILE
     long long prof[12] = {0};
@@ -669,7 +696,9 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     int pf_row = -1, pf_done = -1;                      // prefetch engines: candidate whose row / state is in flight
     constexpr int PF_W0 = NW / 2;                       // warps PF_W0.. are prefetch engines at the top of every iteration
     const int nsteps = T > 0 ? T : 1;
+    int st_last = 0;
     for (int st = 0; st < nsteps; ++st) {
+    st_last = st;
     const long long nflips_before = nflips;
     if (T > 0) {
         // ---- A4-A7 inside the CTA (sweep mode): one warp per leaf, same arithmetic as k_scan
@@ -716,7 +745,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             k = lane < nsup ? sidx[lane] : 0x7fffffff;
             warp_argmax_key(v, k);
             bool stop = !(v > KEY_ONE);                 // no switchable spin left
-            if (!stop && max_flips > 0 && nflips >= max_flips) { stop = true; status = 1; }
+            if (!stop && max_flips > 0 && nflips - nflips0 >= max_flips) { stop = true; status = 1; }
             if (stop) k = -1;
             if (lane == 0) { sh_k = k; sh_stop = stop ? 1 + status : 0; sh_ntouched = 0; }
         } else if (warp >= PF_W0 && one_warp) {         // (with K + 1 > 32 every warp is needed for the update itself)
@@ -767,9 +796,6 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
                 const int t = t0 + lane;
                 int i = -1;
                 if (t <= Kp) i = (t == Kp) ? k : rowk[t];        // entry Kp is the flipped spin itself
-#ifdef FS_RELAX_PROFILE
-                int isum = __reduce_add_sync(0xffffffffu, i + s_old); FS_PROF_T(u1); FS_PROF_ADD(6, c1, u1); if (isum == 0x7fffffff) printf("");
-#endif
                 int blk = -1;
                 if (i >= 0) {
                     double2 hd = hdip[i], hf = hfix[i];
@@ -781,13 +807,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
                         hd.y -= two_s * wt.y;
                         hdip[i] = hd;
                     }
-#ifdef FS_RELAX_PROFILE
-                    if (hd.x + hf.x + si + ih == 1e300) printf(""); FS_PROF_T(u2b); FS_PROF_ADD(7, u1, u2b);
-#endif
                     double m = margin(hd.x + hf.x, hd.y + hf.y, si, ih, ast);
-#ifdef FS_RELAX_PROFILE
-                    if (m == 1e300) printf(""); FS_PROF_T(u3); FS_PROF_ADD(8, u2b, u3);
-#endif
                     M[i] = m;
                     blk = i >> LBshift;
                     // the leaf maximum can only change if i was its arg-max or reaches its value
@@ -864,11 +884,16 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     if (status) break;                                  // max_flips reached
     __syncthreads();                                    // the next step's scan rewrites the hierarchy
     }   // steps
-    if (T > 0 && tid == 0) hext_all[r] = sweep_fields[min(T - 1, nsteps - 1)];
+    // a sweep stopped by max_flips leaves the fields of the step it actually reached (hfix, M and the spins
+    // belong to that step) and zero flips for the steps it never ran
+    if (T > 0 && tid == 0) hext_all[r] = sweep_fields[st_last];
+    if (T > 0 && flips_per_step)
+        for (int t = st_last + 1 + tid; t < T; t += RELAX_THREADS) flips_per_step[(int64_t)r * T + t] = 0;
     if (tid == 0) {
         ctr[r].total_flips += nflips;
         ctr[r].last_flips = nflips;
         ctr[r].status = status;
+        ctr[r].last_step = st_last;
 #ifdef FS_RELAX_PROFILE
         for (int q = 0; q < 12; ++q) atomicAdd((unsigned long long*)&g_relax_prof[q], (unsigned long long)prof[q]);
         atomicAdd((unsigned long long*)&g_relax_prof[15], (unsigned long long)nflips);
@@ -925,6 +950,7 @@ struct fs_sim {
     Astroid ast{};
     Grid grid{};
     cudaStream_t stream = nullptr;
+    int device = 0;                 // the device current at fs_create; every entry point switches to it
     int sm_count = 148;
     // geometry
     double2 *pos = nullptr, *cs = nullptr, *w = nullptr, *wT = nullptr;
@@ -955,6 +981,8 @@ struct fs_sim {
     unsigned long long st_id = 0;   // identity for the ownership of the constant-memory table
     double st_maxdev = 0.0, st_wmax = 0.0;
     long long st_slots = 0;         // stencil slots present (sum over sublattice pairs)
+    // exact batched flips (batch.cuh); library-owned scratch, freed by fs_destroy
+    void* bt_mem = nullptr; BatchArgs bt{}; bool bt_ok = false; int bt_P = 0, bt_seq = 64, bt_grid = 0;
 };
 
 namespace {
@@ -1112,6 +1140,8 @@ int do_gather_stencil(fs_sim* sim) {
     if (sim->st_ct) {
         // the constant-memory table is shared by all simulations of the process: take it over if needed
         std::lock_guard<std::mutex> lock(g_ct_mutex);
+        unsigned long long& g_ct_owner = g_ct_owner_dev[sim->device];
+        cudaEvent_t& g_ct_event = g_ct_event_dev[sim->device];
         if (g_ct_owner != sim->st_id) {
             if (g_ct_event) CUDA_TRY(cudaStreamWaitEvent(sim->stream, g_ct_event, 0));   // previous owner's kernels first
             CUDA_TRY(cudaMemcpyToSymbolAsync(c_T, sim->T, 16 * (size_t)g.nsub * g.nsub * g.W * g.H, 0,
@@ -1140,8 +1170,7 @@ int do_gather_stencil(fs_sim* sim) {
 struct StencilShape { int nw, rs, pv, ov; size_t smem; };
 
 bool stencil_ct(const LatGrid& g) {
-    return (int64_t)g.nsub * g.nsub * g.W * g.H <= CT_MAX && g.nsub * g.nsub * g.W <= CR_MAX &&
-           env_int("FS_STENCIL_NO_CT", 0) == 0;
+    return (int64_t)g.nsub * g.nsub * g.W * g.H <= CT_MAX && g.nsub * g.nsub * g.W <= CR_MAX;
 }
 
 size_t stencil_smem(const LatGrid& g, int nw, int rs, int ov, int* pv_out) {
@@ -1324,11 +1353,6 @@ int detect_lattice(fs_sim* sim) {
     int wh = g.W * g.H;
     StencilShape shp{};
     if (!plan_stencil(sim, g, &shp)) return lattice_fail(sim, FS_LATTICE_STENCIL_TOO_WIDE);
-    if (env_int("FS_STENCIL_NW", 0) > 0) {                           // tuning override
-        shp.nw = env_int("FS_STENCIL_NW", 0); shp.rs = std::max(1, env_int("FS_STENCIL_RS", 1));
-        shp.ov = ST_OV;
-        shp.smem = stencil_smem(g, shp.nw, shp.rs, shp.ov, &shp.pv);
-    }
     sim->st_nw = shp.nw; sim->st_rs = shp.rs; sim->st_pv = shp.pv; sim->st_ov = shp.ov; sim->st_smem = shp.smem;
     sim->st_ct = stencil_ct(g);
     sim->st_id = ++g_ct_next_id;
@@ -1372,14 +1396,10 @@ int detect_lattice(fs_sim* sim) {
     if (flags & 4) return lattice_fail(sim, FS_LATTICE_NOT_PERIODIC);
     if ((long long)res64[2] != (long long)sim->n_inter) return lattice_fail(sim, FS_LATTICE_REACH_MISMATCH);
     if (!(sim->st_maxdev * (double)sim->K <= 2e-13 * sim->st_wmax)) return lattice_fail(sim, FS_LATTICE_WEIGHT_MISMATCH);
-    if (sim->st_smem > 48 * 1024) {
-        int b = (int)sim->st_smem;
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, true, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<128, 7, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
-        CUDA_TRY(cudaFuncSetAttribute(k_gather_stencil<256, 3, false, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
-
-    }
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8>, sim->st_smem));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8>, sim->st_smem));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, false, 8>, sim->st_smem));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, false, 8>, sim->st_smem));
     sim->lg = g;
     sim->stencil_ok = true; sim->stencil_reason = 0;
     // the build-only arrays (sub, cu, cv) are no longer needed
@@ -1416,7 +1436,7 @@ int fetch_counters(fs_sim* sim) {
 
 // T == 0: relax at the field set by fs_set_field (k_scan first); T > 0: whole protocol in one launch
 int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_dev, uint32_t step0, long long* per_step_dev,
-                 const double* sigma_dev = nullptr) {
+                 const double* sigma_dev = nullptr, int use_base = 0) {
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
     FieldSpec fsp{sim->sigma, sim->seed, T > 0 ? step0 : sim->step};
     // ensembles of small systems: when there are more replicas than SMs and the whole update fits one warp,
@@ -1427,10 +1447,10 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr, \
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid, \
         sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0, \
-        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev
+        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev, use_base
     if (small_cta && sim->R > 8 * sim->sm_count) k_relax<64><<<sim->R, 64, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else if (small_cta) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
-    else if (sim->Kp + 1 > 512 && env_int("FS_RELAX_1024", 1)) k_relax<1024><<<sim->R, 1024, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+    else if (sim->Kp + 1 > 512) k_relax<1024><<<sim->R, 1024, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else k_relax<512><<<sim->R, 512, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
 #undef FS_RELAX_ARGS
     LAUNCHED();
@@ -1438,10 +1458,60 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
     return FS_OK;
 }
 
+// Exact batched flips (batch.cuh) for one large system: a cooperative kernel on all SMs commits the long prefixes of
+// the flip sequence that big avalanches allow; k_relax then finishes the tail from the rebuilt leaf maxima.
+int launch_batch(fs_sim* sim) {
+    BatchArgs a = sim->bt;
+    a.cellidx = sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr;
+    a.P = sim->bt_P; a.seq_threshold = sim->bt_seq;
+    CUDA_TRY(cudaMemsetAsync(a.ctl, 0, sizeof(BatchCtl), sim->stream));
+    CUDA_TRY(cudaMemsetAsync(a.owner, 0xff, 4 * (size_t)sim->N, sim->stream));
+    void* args[] = {&a};
+    CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_relax_batch, dim3((unsigned)sim->bt_grid), dim3(BT_THREADS), args, 0, sim->stream));
+    LAUNCHED();
+    return FS_OK;
+}
+
 int do_relax(fs_sim* sim, int64_t max_flips) {
     int rc = do_scan(sim, false);
     if (rc) return rc;
-    return launch_relax(sim, max_flips, 0, nullptr, 0, nullptr);
+    const bool batch = sim->bt_ok && sim->bt_P > 0 && max_flips <= 0;
+    if (batch) { rc = launch_batch(sim); if (rc) return rc; }
+    return launch_relax(sim, max_flips, 0, nullptr, 0, nullptr, nullptr, batch ? 1 : 0);
+}
+
+// scratch of k_relax_batch; never fails the creation (no scratch = sequential relax only)
+int setup_batch(fs_sim* sim) {
+    sim->bt_ok = false;
+    if (sim->R != 1 || sim->K < 1 || sim->K > 64 || sim->N < 16384) return FS_OK;
+    int coop = 0, occ = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sim->device);
+    if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_relax_batch, BT_THREADS, 0) != cudaSuccess || occ < 1) {
+        cudaGetLastError(); return FS_OK;
+    }
+    const int64_t pc = sim->N / (8 * (int64_t)(sim->K + 1));
+    const int P = (int)std::max<int64_t>(64, std::min<int64_t>(BT_PMAX, pc));
+    const size_t und = sizeof(BatchUndo) * (size_t)P * BT_LMAX * (size_t)(sim->Kp + 1);
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    const size_t o_ctl = take(sizeof(BatchCtl)), o_owner = take(4 * (size_t)sim->N), o_seeds = take(sizeof(BatchSeed) * BT_PMAX),
+                 o_edges = take(2 * (size_t)BT_PMAX * BT_EMAX), o_ecount = take(BT_PMAX), o_npos = take(4 * (size_t)BT_PMAX),
+                 o_elems = take(sizeof(BatchElem) * (size_t)P * BT_LMAX), o_undo = take(und),
+                 o_blocks = take(sizeof(BatchBlock) * BT_PMAX), o_clist = take(sizeof(BatchCommit) * (size_t)P * BT_LMAX);
+    if (cudaMalloc(&sim->bt_mem, o) != cudaSuccess) { cudaGetLastError(); sim->bt_mem = nullptr; return FS_OK; }
+    unsigned char* b = (unsigned char*)sim->bt_mem;
+    int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
+    BatchArgs& a = sim->bt;
+    a.N = sim->N; a.Kp = sim->Kp; a.LBshift = lb_shift; a.nblk = sim->nblk; a.ast = sim->ast; a.log_cap = sim->log_cap;
+    a.nbr = sim->nbr; a.wT = sim->wT; a.ihc = sim->hc; a.s = sim->s; a.hdip = sim->hdip; a.hfix = sim->hfix; a.M = sim->M;
+    a.bval = sim->bval; a.bidx = sim->bidx; a.flog = sim->flog; a.ctr = sim->ctr;
+    a.cellidx = nullptr; a.sgrid = sim->sgrid;
+    a.ctl = (BatchCtl*)(b + o_ctl); a.owner = (unsigned*)(b + o_owner); a.seeds = (BatchSeed*)(b + o_seeds);
+    a.edges = (unsigned short*)(b + o_edges); a.ecount = b + o_ecount; a.npos = (int*)(b + o_npos);
+    a.elems = (BatchElem*)(b + o_elems); a.undo = (BatchUndo*)(b + o_undo); a.blocks = (BatchBlock*)(b + o_blocks);
+    a.clist = (BatchCommit*)(b + o_clist);
+    sim->bt_P = P; sim->bt_seq = 64; sim->bt_grid = sim->sm_count; sim->bt_ok = true;
+    return FS_OK;
 }
 
 }  // namespace
@@ -1517,6 +1587,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     auto kind = [](double denom) { return denom == 3.0 ? 1 : (denom == 2.0 ? 2 : (denom == 1.0 ? 3 : 0)); };
     sim->ast = Astroid{1.0 / p->b, 1.0 / p->c, 2.0 / p->gamma, 2.0 / p->beta, kind(p->gamma), kind(p->beta)};
     int dev = 0; cudaGetDevice(&dev);
+    sim->device = dev;
     cudaDeviceGetAttribute(&sim->sm_count, cudaDevAttrMultiProcessorCount, dev);
     sim->pos = (double2*)(base + L.pos); sim->cs = (double2*)(base + L.cs);
     sim->nbr = (int*)(base + L.nbr); sim->w = (double2*)(base + L.w); sim->wT = (double2*)(base + L.wT);
@@ -1557,7 +1628,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     {
         int warps = 4;
         size_t smem = (size_t)warps * Kp2 * sizeof(int);
-        CREATE_TRY(cudaFuncSetAttribute(k_fill_neighbors, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CREATE_TRY(raise_smem_limit(k_fill_neighbors, smem));
         int64_t blocks = std::min<int64_t>((N + warps - 1) / warps, (int64_t)sim->sm_count * 16);
         k_fill_neighbors<<<(unsigned)blocks, warps * 32, smem, st>>>(N, gp.g, gp.cut2, Kp, Kp2, sim->pos,
                                                                       (int*)(base + L.cell_start), (int*)(base + L.items), sim->nbr);
@@ -1570,10 +1641,10 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
         LAUNCHED();
     }
     sim->relax_smem = ((size_t)nblk + (size_t)(nblk + 31) / 32 + 8) * 12 + (size_t)(Kp + 1) * 4 + 32;
-    CREATE_TRY(cudaFuncSetAttribute(k_relax<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
-    CREATE_TRY(cudaFuncSetAttribute(k_relax<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
-    CREATE_TRY(cudaFuncSetAttribute(k_relax<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
-    CREATE_TRY(cudaFuncSetAttribute(k_relax<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sim->relax_smem));
+    CREATE_TRY(raise_smem_limit(k_relax<512>, sim->relax_smem));
+    CREATE_TRY(raise_smem_limit(k_relax<128>, sim->relax_smem));
+    CREATE_TRY(raise_smem_limit(k_relax<64>, sim->relax_smem));
+    CREATE_TRY(raise_smem_limit(k_relax<1024>, sim->relax_smem));
     int hflags = 0;
     CREATE_TRY(cudaMemcpyAsync(&hflags, scr + 8, sizeof(int), cudaMemcpyDeviceToHost, st));
     CREATE_TRY(cudaStreamSynchronize(st));
@@ -1582,6 +1653,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     if (hflags & 1) { fs_destroy(sim); return fail(FS_ERR_ARG, "hc must be finite and > 0, angle finite"); }
     rc = detect_lattice(sim);
     if (rc) { fs_destroy(sim); return rc; }
+    setup_batch(sim);
     sim->fields_dirty = true;
     *out = sim;
     return FS_OK;
@@ -1594,17 +1666,21 @@ int fs_create(fs_sim** out, int64_t N, const double* pos_dev, const double* angl
 
 int fs_destroy(fs_sim* sim) {
     if (!sim) return FS_OK;
+    DeviceGuard guard_(sim->device);
+    cudaStreamSynchronize(sim->stream);                  // kernels in flight may still read the pinned staging buffers
     if (sim->hext_host) cudaFreeHost(sim->hext_host);
     if (sim->ctr_host) cudaFreeHost(sim->ctr_host);
     if (sim->hloc) cudaFree(sim->hloc);
     if (sim->lat_mem) cudaFree(sim->lat_mem);
     if (sim->st_mem) cudaFree(sim->st_mem);
+    if (sim->bt_mem) cudaFree(sim->bt_mem);
     delete sim;
     return FS_OK;
 }
 
 int fs_get_info(const fs_sim* sim, int64_t* N, int32_t* R, int32_t* K, int64_t* n_interactions) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     if (N) *N = sim->N;
     if (R) *R = sim->R;
     if (K) *K = sim->K;
@@ -1614,6 +1690,7 @@ int fs_get_info(const fs_sim* sim, int64_t* N, int32_t* R, int32_t* K, int64_t* 
 
 int fs_set_spins(fs_sim* sim, const int8_t* s_dev) {
     if (!sim || !s_dev) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     CUDA_TRY(cudaMemcpyAsync(sim->s, s_dev, (size_t)sim->R * sim->N, cudaMemcpyDeviceToDevice, sim->stream));
     sim->fields_dirty = true; sim->sgrid_valid = false;
     return FS_OK;
@@ -1621,12 +1698,14 @@ int fs_set_spins(fs_sim* sim, const int8_t* s_dev) {
 
 int fs_get_spins(fs_sim* sim, int8_t* s_dev_out) {
     if (!sim || !s_dev_out) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     CUDA_TRY(cudaMemcpyAsync(s_dev_out, sim->s, (size_t)sim->R * sim->N, cudaMemcpyDeviceToDevice, sim->stream));
     return FS_OK;
 }
 
 int fs_set_thermal(fs_sim* sim, double sigma_th, uint64_t seed) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     if (!(sigma_th >= 0.0)) return fail(FS_ERR_ARG, "sigma_th must be >= 0");
     sim->sigma = sigma_th; sim->seed = seed;
     return FS_OK;
@@ -1634,6 +1713,7 @@ int fs_set_thermal(fs_sim* sim, double sigma_th, uint64_t seed) {
 
 int fs_set_field(fs_sim* sim, double hx, double hy, uint32_t step) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     sim->step = step;
     k_set_field<<<(sim->R + 127) / 128, 128, 0, sim->stream>>>(sim->R, hx, hy, sim->hext); LAUNCHED();   // by value: no host sync
     CUDA_TRY(cudaGetLastError());
@@ -1642,6 +1722,7 @@ int fs_set_field(fs_sim* sim, double hx, double hy, uint32_t step) {
 
 int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step) {
     if (!sim || !h_host) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     CUDA_TRY(cudaStreamSynchronize(sim->stream));
     for (int r = 0; r < sim->R; ++r) sim->hext_host[r] = make_double2(h_host[2 * r], h_host[2 * r + 1]);
     sim->step = step;
@@ -1650,6 +1731,7 @@ int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step) {
 
 int fs_set_local_field(fs_sim* sim, const double* h_dev) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     if (!h_dev) {
         if (sim->hloc) { CUDA_TRY(cudaStreamSynchronize(sim->stream)); cudaFree(sim->hloc); sim->hloc = nullptr; }
         return FS_OK;
@@ -1661,6 +1743,7 @@ int fs_set_local_field(fs_sim* sim, const double* h_dev) {
 
 int fs_set_gather_variant(fs_sim* sim, int variant) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     if (variant < 0 || variant > 2) return fail(FS_ERR_ARG, "unknown gather variant %d", variant);
     if (variant == FS_GATHER_STENCIL && !sim->stencil_ok)
         return fail(FS_ERR_ARG, "stencil gather unavailable for this geometry (FS_LATTICE reason %d)", sim->stencil_reason);
@@ -1670,6 +1753,7 @@ int fs_set_gather_variant(fs_sim* sim, int variant) {
 
 int fs_get_lattice(const fs_sim* sim, int32_t* info, double* dinfo) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     if (info) {
         const LatGrid& g = sim->lg;
         int32_t v[10] = {sim->stencil_ok ? 1 : 0, sim->stencil_reason, g.nsub, g.U, g.V, g.Ru, g.Rv,
@@ -1716,13 +1800,40 @@ int fs_debug_relax_profile(long long* out16, int reset) {
 }
 #endif
 
+int fs_set_batch(fs_sim* sim, int32_t max_seeds, int32_t seq_threshold) {
+    if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    if (max_seeds < 0 || max_seeds > BT_PMAX || seq_threshold < 0) return fail(FS_ERR_ARG, "max_seeds must be in [0, %d], seq_threshold >= 0", BT_PMAX);
+    if (max_seeds > 0 && !sim->bt_ok) return fail(FS_ERR_ARG, "batched flips unavailable for this simulation (needs R = 1, 1 <= K <= 64, N >= 16384)");
+    if (sim->bt_ok) {
+        const int64_t cap = sim->N / (8 * (int64_t)(sim->K + 1));
+        const int alloc = (int)std::max<int64_t>(64, std::min<int64_t>(BT_PMAX, cap));
+        sim->bt_P = std::min<int>(max_seeds, alloc);
+        sim->bt_seq = seq_threshold;
+    }
+    return FS_OK;
+}
+
+int fs_get_batch_stats(fs_sim* sim, int64_t* out4) {
+    if (!sim || !out4) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
+    int rc = fetch_counters(sim);
+    if (rc) return rc;
+    out4[0] = sim->bt_ok ? sim->bt_P : 0;
+    out4[1] = sim->ctr_host[0].batch_total;
+    out4[2] = sim->ctr_host[0].batch_rounds;
+    out4[3] = sim->bt_seq;
+    return FS_OK;
+}
+
 int fs_update_fields(fs_sim* sim) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     return do_gather(sim);
 }
 
 int fs_scan_ensemble(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, double* best_L) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     int rc = do_scan(sim, true);
     if (rc) return rc;
     if (!n_switchable && !best_index && !best_L) return FS_OK;
@@ -1738,6 +1849,7 @@ int fs_scan_ensemble(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, do
 
 int fs_scan(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, double* best_L) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     if (sim->R == 1) return fs_scan_ensemble(sim, n_switchable, best_index, best_L);
     int rc = fs_scan_ensemble(sim, nullptr, nullptr, nullptr);
     if (rc) return rc;
@@ -1752,6 +1864,7 @@ int fs_scan(fs_sim* sim, int64_t* n_switchable, int64_t* best_index, double* bes
 
 int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     int rc = do_relax(sim, max_flips);
     if (rc) return rc;
     if (!n_flips_out) return FS_OK;
@@ -1764,6 +1877,7 @@ int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
 
 int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     int rc = do_relax(sim, max_flips);
     if (rc) return rc;
     if (!n_flips_out) return FS_OK;
@@ -1778,6 +1892,7 @@ int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
 int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_dev, int32_t T, uint32_t step0,
                     int64_t* flips_per_step_dev, int64_t max_flips, int64_t* n_flips_out) {
     if (!sim || !fields_dev) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     if (T <= 0) return fail(FS_ERR_ARG, "T=%d must be positive", (int)T);
     int rc = ensure_fields(sim);
     if (rc) return rc;
@@ -1790,6 +1905,7 @@ int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_d
     if (rc) return rc;
     int capped = 0;
     for (int r = 0; r < sim->R; ++r) { n_flips_out[r] = sim->ctr_host[r].last_flips; capped |= sim->ctr_host[r].status; }
+    if (capped) sim->step = step0 + (uint32_t)sim->ctr_host[0].last_step;      // replica 0's last step (see flatspin.h)
     return capped ? fail(FS_ERR_MAXFLIPS, "sweep stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
 }
 
@@ -1800,6 +1916,7 @@ int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, i
 
 int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     int rc = fetch_counters(sim);
     if (rc) return rc;
     for (int r = 0; r < sim->R; ++r) {
@@ -1812,6 +1929,7 @@ int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips
 
 int fs_get_fields(fs_sim* sim, int which, double* h_dev_out) {
     if (!sim || !h_dev_out) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     if (which < 0 || which > 3) return fail(FS_ERR_ARG, "unknown field selector %d", which);
     if (which == FS_FIELD_TOTAL || which == FS_FIELD_DIP) { int rc = ensure_fields(sim); if (rc) return rc; }
     dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
@@ -1824,6 +1942,7 @@ int fs_get_fields(fs_sim* sim, int which, double* h_dev_out) {
 
 int fs_get_flip_log(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out) {
     if (!sim || !n_out) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     if (replica < 0 || replica >= sim->R) return fail(FS_ERR_ARG, "replica out of range");
     int rc = fetch_counters(sim);
     if (rc) return rc;
@@ -1840,6 +1959,7 @@ int fs_get_flip_log(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t 
 
 int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
+    DeviceGuard guard_(sim->device);
     if (K_out) *K_out = sim->K;
     if (idx_dev_out && sim->K > 0)
         CUDA_TRY(cudaMemcpy2DAsync(idx_dev_out, 4 * (size_t)sim->K, sim->nbr, 4 * (size_t)sim->Kp, 4 * (size_t)sim->K,
@@ -1850,6 +1970,7 @@ int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out) {
 int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t* n_switchable, int64_t* best_index,
                  double* best_L) {
     if (!sim || !s_host || !h_host_out) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     size_t rn = (size_t)sim->R * sim->N;
     CUDA_TRY(cudaMemcpyAsync(sim->s, s_host, rn, cudaMemcpyHostToDevice, sim->stream));
     sim->fields_dirty = true; sim->sgrid_valid = false;
@@ -1873,6 +1994,7 @@ int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t*
 
 int fs_relax_host(fs_sim* sim, double hx, double hy, uint32_t step, int8_t* s_host_out, int64_t* n_flips_out) {
     if (!sim || !s_host_out) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
     int rc = fs_set_field(sim, hx, hy, step);
     if (rc) return rc;
     rc = do_relax(sim, 0);

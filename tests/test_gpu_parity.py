@@ -145,7 +145,7 @@ def test_stencil_other_geometries(B, geom):
     sim = B.Sim(pos, ang, hc, p); sim.set_spins(spins)
     orc = Oracle(pos, ang, hc, p, spins=spins)
     assert sim.lattice()["active"], sim.lattice()
-    assert sim.n_interactions == orc.num_interactions or orc.build_neighbors() >= 0
+    assert sim.n_interactions == orc.num_interactions and sim.K == orc.build_neighbors()
     for variant in (B.GATHER_STENCIL, B.GATHER_ELL_F64):
         sim.set_gather_variant(variant)
         sim.update_fields()
@@ -400,13 +400,13 @@ def test_config2_full_size_protocol(B):
 
 @pytest.mark.slow
 def test_config2b_full_size_protocol(B):
-    total, w, _, _ = _full_protocol(B, "2b", stride=2)
+    total, w, _, _ = _full_protocol(B, "2b")
     assert w.N == 14979 and total > w.N
 
 
 @pytest.mark.slow
 def test_config3_full_size_protocol(B):
-    total, w, _, _ = _full_protocol(B, "3", stride=4)      # every 4th of the 2001 field values
+    total, w, _, _ = _full_protocol(B, "3")                # all 2001 field values
     assert w.N == 80400 and total > w.N
 
 
@@ -579,6 +579,9 @@ def test_sweep_max_flips_cap(B):
         if sum(len(r) for r in ref) >= 100:
             break
     assert np.array_equal(sim.get_flip_log().cpu().numpy()[:100], np.concatenate(ref)[:100])
+    # the state left behind is the one of the step actually reached (t), not of the protocol's last step
+    assert int(ps[0, :t].sum().item()) + int(ps[0, t].item()) == 100 and int(ps[0, t + 1:].sum().item()) == 0
+    assert field_err(sim.get_fields(2).cpu().numpy(), orc.fields(2)) < FIELD_TOL
 
 
 def test_many_replicas_more_than_sms(B):
@@ -598,6 +601,86 @@ def test_many_replicas_more_than_sms(B):
         no, log = o.relax_B()
         assert n[r] == no and np.array_equal(sim.get_flip_log(replica=r).cpu().numpy(), log)
         assert np.array_equal(s[r], o.spins())
+
+
+def test_relax_64_thread_variant_many_replicas(B):
+    """R = 1,300 replicas (> 8 per SM): the 64-thread relax CTA (k_relax<64>), the variant bench.py's ensemble
+    figure runs.  Stepwise relax and the one-launch sweep, sampled replicas incl. first / last / around 8 x SMs."""
+    from oracle import Oracle
+    pos, ang = W.square_closed(4)
+    N = len(ang); R = 1300
+    p = dict(alpha=0.002, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    hc = W.coercive_fields(N, seed=70, replicas=R)
+    fields = W.ramp(0.2, -0.2, 40, 45.0, legs=2)
+    sample = (0, 1, 147, 148, 1183, 1184, 1185, 1298, 1299)
+    # stepwise
+    sim = B.Sim(pos, ang, hc, p); sim.set_thermal(0.006, 5)
+    orcs = {r: Oracle(pos, ang, hc[r], p) for r in sample}
+    for r, o in orcs.items():
+        o.set_thermal(0.006, 5 + r)
+    tot = 0
+    for t, (hx, hy) in enumerate(fields):
+        sim.set_field(hx, hy, t)
+        n = sim.relax_ensemble()
+        for r, o in orcs.items():
+            o.set_field(hx, hy, t)
+            no, log = o.relax_B()
+            assert n[r] == no, (t, r)
+            assert np.array_equal(sim.get_flip_log(replica=r).cpu().numpy(), log), (t, r)
+            tot += no
+    assert tot > len(sample) * N
+    s = sim.get_spins().cpu().numpy(); h = sim.get_fields(0).cpu().numpy()
+    for r, o in orcs.items():
+        assert np.array_equal(s[r], o.spins()) and field_err(h[r], o.fields(0)) < FIELD_TOL
+    # one launch
+    sim = B.Sim(pos, ang, hc, p); sim.set_thermal(0.006, 5)
+    n, ps = sim.sweep(fields, step0=0)
+    ps = ps.cpu().numpy(); s = sim.get_spins().cpu().numpy()
+    for r in sample:
+        o = Oracle(pos, ang, hc[r], p); o.set_thermal(0.006, 5 + r)
+        cnt, logs = [], []
+        for t, (hx, hy) in enumerate(fields):
+            o.set_field(hx, hy, t); c, log = o.relax_B(); cnt.append(c); logs.append(log)
+        assert np.array_equal(ps[r], np.array(cnt)) and n[r] == sum(cnt)
+        assert np.array_equal(sim.get_flip_log(replica=r).cpu().numpy()[: n[r]], np.concatenate(logs))
+        assert np.array_equal(s[r], o.spins())
+
+
+def test_stencil_shared_memory_table_variant(B):
+    """A coupling table too large for the 56 KB constant bank (square ASI, neighbor distance 15: 4 x 31 x 31 =
+    3,844 entries): k_gather_stencil reads the table from shared memory instead.  Fields against the oracle."""
+    from oracle import Oracle
+    pos, ang = W.square_closed(40)
+    N = len(ang)
+    p = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=15.0)
+    hc = W.coercive_fields(N, seed=3); spins = W.random_spins(N, seed=12)
+    sim = B.Sim(pos, ang, hc, p); sim.set_spins(spins)
+    lat = sim.lattice()
+    assert lat["active"] and (lat["Ru"], lat["Rv"]) == (15, 15) and lat["nsub"] ** 2 * 31 * 31 > 3584, lat
+    orc = Oracle(pos, ang, hc, p, spins=spins)
+    sim.set_gather_variant(B.GATHER_STENCIL); sim.update_fields()
+    a = sim.get_fields(1).cpu().numpy()
+    assert field_err(a, orc.fields(1)) < FIELD_TOL
+    sim.set_gather_variant(B.GATHER_ELL_F64); sim.update_fields()
+    assert field_err(sim.get_fields(1).cpu().numpy(), a) < FIELD_TOL
+
+
+def test_two_sims_of_different_size_stay_usable(B):
+    """The dynamic shared-memory limit of a kernel belongs to the function, not to a simulation: creating a
+    small simulation after a large one must not break the large one's relax / stencil gather."""
+    w3 = W.config("3", scale=200)                     # 80,400 spins: ~10k leaf blocks worth of relax shared memory
+    simA, orcA = mk(B, w3)
+    w1 = W.config("1")
+    simB, orcB = mk(B, w1)                            # created afterwards, far smaller
+    hx, hy = w3.fields[1000]
+    simA.set_field(hx, hy, 1000); orcA.set_field(hx, hy, 1000)
+    n = simA.relax(); no, log = orcA.relax_B()
+    assert n == no and n > 0 and np.array_equal(simA.get_flip_log().cpu().numpy(), log)
+    simA.set_gather_variant(B.GATHER_STENCIL); simA.update_fields()
+    assert field_err(simA.get_fields(1).cpu().numpy(), orcA.fields(1)) < FIELD_TOL
+    hx, hy = w1.fields[250]
+    simB.set_field(hx, hy, 250); orcB.set_field(hx, hy, 250)
+    assert simB.relax() == orcB.relax_B()[0]
 
 
 def test_annealing_sweep_matches_oracle(B):

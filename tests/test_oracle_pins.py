@@ -33,11 +33,11 @@ def gold_lines(name):
 def test_paper_magnet_counts():
     gen = dict(kagome=W.kagome, pinwheel_diamond=W.pinwheel_diamond)
     for name, n, count, cmp in gold_lines("paper_counts.txt"):
-        if int(n) > 100:   # closed form 2 n^2 without building a 1e6 array twice
-            N = 2 * int(n) ** 2
-            assert len(W.pinwheel_diamond(8)[1]) == 2 * 64
-        else:
-            N = len(gen[name](int(n))[1])
+        pos, ang = gen[name](int(n))           # the 708 x 708 diamond is built too (1,002,528 magnets)
+        N = len(ang)
+        assert pos.shape == (N, 2)
+        if name == "pinwheel_diamond":
+            assert N == 2 * int(n) ** 2
         assert (N == int(count)) if cmp == "eq" else (N > int(count))
 
 
@@ -250,6 +250,45 @@ def test_philox_known_answers():
     for row in gold_lines("philox_kat.txt"):
         v = [int(x, 16) for x in row]
         assert list(oracle.philox4x32_10(v[0:4], v[4:6])) == v[6:10]
+
+
+def test_unit_normals_known_answer():
+    """Reading C-11: counter = (spin, step, 0, 0), key = (seed_lo, seed_hi); u = ((hi*2^32 + lo) >> 12
+    + 0.5) * 2^-52 from the word pairs (x0,x1) and (x2,x3); z0 = sqrt(-2 ln u1) cos(2 pi u2), z1 = ... sin.
+    Derived here by hand from the published Philox known-answer rows (golden/philox_kat.txt), with Python
+    integers and `math` only: a swapped cos/sin, u1 <-> u2, >>11 for >>12, or a different counter/key layout
+    changes the expected numbers."""
+    rows = [[int(x, 16) for x in r] for r in gold_lines("philox_kat.txt")]
+
+    def expect(x):
+        a = ((x[0] << 32) | x[1]) >> 12
+        b = ((x[2] << 32) | x[3]) >> 12
+        u1 = (a + 0.5) / 4503599627370496.0
+        u2 = (b + 0.5) / 4503599627370496.0
+        r = math.sqrt(-2.0 * math.log(u1))
+        return r * math.cos(2.0 * math.pi * u2), r * math.sin(2.0 * math.pi * u2)
+
+    # row 0: ctr = 0, key = 0  <=>  seed 0, step 0, spin 0
+    z = oracle.unit_normals(0, 0, 0)
+    e = expect(rows[0][6:10])
+    assert abs(z[0] - e[0]) < 1e-15 and abs(z[1] - e[1]) < 1e-15
+    # the same row spelled out: u1 = 0x6627e8d5e169c >> 0 ... as decimals (guards the fixture reader itself)
+    assert rows[0][6:10] == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
+    a = 0x6627e8d5e169c58d >> 12; b = 0xbc57ac4c9b00dbd8 >> 12
+    assert a == 0x6627e8d5e169c and b == 0xbc57ac4c9b00d
+    assert abs((a + 0.5) / 2.0 ** 52 - 0.3990464708489646) < 1e-15 and abs((b + 0.5) / 2.0 ** 52 - 0.7357127844834425) < 1e-15
+    assert abs(z[0] - (-0.12151797595308224)) < 1e-14 and abs(z[1] - (-1.350032659857655)) < 1e-14
+    # row 2 has ctr2 = 0x13198a2e, ctr3 != 0, which the thermal stream never uses; rows 0 and 1 only.
+    # row 1 (all ones) cannot be reached either (ctr2 = ctr3 = 0 always): its words still pin the u -> z map
+    # through the oracle's philox + the formula above on a reachable counter:
+    x = oracle.philox4x32_10([5, 3, 0, 0], [7, 0])            # spin 5, step 3, seed 7
+    e = expect([int(v) for v in x])
+    z = oracle.unit_normals(7, 3, 5)
+    assert abs(z[0] - e[0]) < 1e-15 and abs(z[1] - e[1]) < 1e-15
+    x = oracle.philox4x32_10([9, 2, 0, 0], [0x89abcdef, 0x01234567])   # 64-bit seed split lo, hi
+    e = expect([int(v) for v in x])
+    z = oracle.unit_normals(0x0123456789abcdef, 2, 9)
+    assert abs(z[0] - e[0]) < 1e-15 and abs(z[1] - e[1]) < 1e-15
 
 
 def test_thermal_moments_and_determinism():
