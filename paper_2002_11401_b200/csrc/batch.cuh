@@ -60,7 +60,7 @@ struct BatchArgs {
     // scratch
     BatchCtl* ctl; unsigned* owner; BatchSeed* seeds; unsigned short* edges; unsigned char* ecount;
     int* npos; BatchElem* elems; BatchUndo* undo; BatchBlock* blocks; BatchCommit* clist;
-    int P, seq_threshold;
+    int P, seq_threshold, min_commit;
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -119,6 +119,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     int rot = 0;                                        // rotating counter slot of this round
     unsigned npass = 0;                                 // histogram passes so far (buffer = npass % 3)
     bool any_flip = false;
+    int lean = 0;                                       // consecutive rounds that committed fewer than min_commit flips
 
     for (;; ++rounds) {
         const unsigned tag = 0xFFFFFu - (unsigned)rounds;            // newer rounds win an atomicMin on the claim word
@@ -460,6 +461,10 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         nflips += nc;
         any_flip |= nc > 0;
         rot = (rot + 1) & 3;
+        // a round costs about as much as a few dozen sequential flips: when avalanches are dominoes (every flip
+        // triggers the next one) the prefixes stay short and the one-flip-at-a-time loop is faster
+        lean = nc < a.min_commit ? lean + 1 : 0;
+        if (lean >= 3) { ++rounds; break; }
         // (no barrier: the next round's first pass only reads M, which phase 7 finished before the last barrier;
         //  clist is rewritten only after three more barriers)
     }

@@ -27,6 +27,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <new>
 #include <algorithm>
@@ -68,18 +69,18 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 // it is only ever raised, so that simulations of different sizes can coexist in one process.
 constexpr int MAX_DEVICES = 64;
 std::mutex g_smem_mutex;
+std::map<std::pair<const void*, int>, size_t> g_smem_limit;   // (kernel, device) -> limit set so far
 template <typename F>
 cudaError_t raise_smem_limit(F* func, size_t bytes) {
-    static size_t current[MAX_DEVICES] = {0};          // one table per kernel instantiation
     if (bytes <= 48 * 1024) return cudaSuccess;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     std::lock_guard<std::mutex> lock(g_smem_mutex);
-    if (dev < 0 || dev >= MAX_DEVICES) return cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (bytes <= current[dev]) return cudaSuccess;
+    size_t& cur = g_smem_limit[std::make_pair((const void*)func, dev)];
+    if (bytes <= cur) return cudaSuccess;
     e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e == cudaSuccess) current[dev] = bytes;
+    if (e == cudaSuccess) cur = bytes;
     return e;
 }
 
@@ -982,7 +983,7 @@ struct fs_sim {
     double st_maxdev = 0.0, st_wmax = 0.0;
     long long st_slots = 0;         // stencil slots present (sum over sublattice pairs)
     // exact batched flips (batch.cuh); library-owned scratch, freed by fs_destroy
-    void* bt_mem = nullptr; BatchArgs bt{}; bool bt_ok = false; int bt_P = 0, bt_seq = 64, bt_grid = 0;
+    void* bt_mem = nullptr; BatchArgs bt{}; bool bt_ok = false; int bt_P = 0, bt_seq = 64, bt_min_commit = 32, bt_grid = 0;
 };
 
 namespace {
@@ -1463,7 +1464,7 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
 int launch_batch(fs_sim* sim) {
     BatchArgs a = sim->bt;
     a.cellidx = sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr;
-    a.P = sim->bt_P; a.seq_threshold = sim->bt_seq;
+    a.P = sim->bt_P; a.seq_threshold = sim->bt_seq; a.min_commit = sim->bt_min_commit;
     CUDA_TRY(cudaMemsetAsync(a.ctl, 0, sizeof(BatchCtl), sim->stream));
     CUDA_TRY(cudaMemsetAsync(a.owner, 0xff, 4 * (size_t)sim->N, sim->stream));
     void* args[] = {&a};

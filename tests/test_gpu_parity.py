@@ -668,12 +668,12 @@ def test_stencil_shared_memory_table_variant(B):
 def test_two_sims_of_different_size_stay_usable(B):
     """The dynamic shared-memory limit of a kernel belongs to the function, not to a simulation: creating a
     small simulation after a large one must not break the large one's relax / stencil gather."""
-    w3 = W.config("3", scale=200)                     # 80,400 spins: ~10k leaf blocks worth of relax shared memory
+    w3 = W.config("4", scale=200)                     # 80,400 spins: ~100 KB of relax shared memory (leaf hierarchy)
     simA, orcA = mk(B, w3)
     w1 = W.config("1")
     simB, orcB = mk(B, w1)                            # created afterwards, far smaller
-    hx, hy = w3.fields[1000]
-    simA.set_field(hx, hy, 1000); orcA.set_field(hx, hy, 1000)
+    hx, hy = w3.fields[160]
+    simA.set_field(hx, hy, 160); orcA.set_field(hx, hy, 160)
     n = simA.relax(); no, log = orcA.relax_B()
     assert n == no and n > 0 and np.array_equal(simA.get_flip_log().cpu().numpy(), log)
     simA.set_gather_variant(B.GATHER_STENCIL); simA.update_fields()
@@ -751,3 +751,115 @@ def test_paper_kagome_dirac_string_parameters(B):
     assert w.N == 2638
     total, sim, orc = run_parity(B, w, stride=2)
     assert total > w.N // 4
+
+
+# ------------------------------------------------------------------ f1: exact batched flips (k_relax_batch)
+def _protocol_vs_oracle(B, w, steps, hc=None, expect_batched=True):
+    """Relax at the given protocol steps with the batched kernel active; flip logs against the Tier B oracle."""
+    from oracle import Oracle
+    hc = w.hc if hc is None else hc
+    sim = B.Sim(w.pos, w.angle, hc, w.params); sim.set_spins(w.spins)
+    orc = Oracle(w.pos, w.angle, hc, w.params, spins=w.spins)
+    if w.sigma_th:
+        sim.set_thermal(w.sigma_th, w.thermal_seed); orc.set_thermal(w.sigma_th, w.thermal_seed)
+    assert sim.batch_stats()["max_seeds"] > 0, "batched flips should be available for this size"
+    total = 0
+    for t in steps:
+        hx, hy = w.fields[t]
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        n = sim.relax(); no, log = orc.relax_B()
+        assert n == no, (t, n, no)
+        if n:
+            assert np.array_equal(sim.get_flip_log().cpu().numpy(), log), f"flip order differs at step {t}"
+        total += n
+    st = sim.batch_stats()
+    if expect_batched:
+        assert st["flips"] > total // 2 and st["rounds"] > 0, st      # the batched kernel did most of the work
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    assert field_err(sim.get_fields(1).cpu().numpy(), orc.fields(1)) < FIELD_TOL     # incremental h_dip incl. undone rounds
+    assert orc.monitor()[0] == 0 and sim.scan()[0] == 0
+    return total, st, sim
+
+
+def test_batched_flips_config4_bit_exact(B):
+    w = W.config("4", scale=120)                       # 29,040 spins, thermal ramp: every spin reverses
+    total, st, sim = _protocol_vs_oracle(B, w, range(len(w.fields)))
+    assert total == w.N
+    # the stencil spin grid followed the committed flips only (undone ones never reach it)
+    sim.set_gather_variant(B.GATHER_STENCIL); sim.update_fields(); a = sim.get_fields(1).cpu().numpy()
+    sim.set_gather_variant(B.GATHER_ELL_F64); sim.update_fields(); b = sim.get_fields(1).cpu().numpy()
+    assert field_err(a, b) < 1e-13
+
+
+def test_batched_flips_one_giant_avalanche_refines_threshold(B):
+    """A single field jump makes every spin switchable at once with margins inside a few histogram bins: the
+    threshold search must split a bin (linear refinement pass) and the whole array reverses in one relax."""
+    w = W.config("4", scale=100)                       # 20,200 spins
+    w.fields = np.array([[-0.25 * math.cos(math.pi / 4), -0.25 * math.sin(math.pi / 4)]])
+    total, st, _ = _protocol_vs_oracle(B, w, [0], expect_batched=False)   # (it hands over to k_relax once rounds run lean)
+    assert total == w.N and st["rounds"] > 10 and st["flips"] > 1000
+
+
+@pytest.mark.parametrize("which,scale,stride", [("3", 100, 4), ("2", 80, 2)])
+def test_batched_flips_other_lattices(B, which, scale, stride):
+    """K = 60 (two chunks of neighbours per flip, domino avalanches: the kernel hands over to k_relax when its
+    prefixes stay short) and the kagome lattice (K = 14, three sublattices)."""
+    w = W.config(which, scale=scale)
+    assert w.N >= 16384
+    total, st, _ = _protocol_vs_oracle(B, w, range(0, len(w.fields), stride), expect_batched=False)
+    assert total > w.N // 2
+
+
+def test_batched_equals_sequential_with_exact_ties(B):
+    """Uniform h_c and a symmetric start: whole classes of spins have bit-identical margins, so the order among
+    them is decided by the index alone.  The batched kernel (threshold search over identical keys, bail-out when a
+    single key value exceeds the round's capacity) must give the sequential kernel's log bit for bit."""
+    pos, ang = W.square_closed(100)
+    N = len(ang)
+    p = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    hc = np.full(N, 0.2)
+    fields = W.ramp(0.0, -0.25, 25, 45.0, legs=1)
+    logs = {}
+    for mode in ("batch", "seq"):
+        sim = B.Sim(pos, ang, hc, p)
+        if mode == "seq":
+            sim.set_batch(0)
+        out = []
+        for t, (hx, hy) in enumerate(fields):
+            sim.set_field(hx, hy, t)
+            if sim.relax():
+                out.append(sim.get_flip_log().cpu().numpy().copy())
+        logs[mode] = (np.concatenate(out), sim.get_spins().cpu().numpy(), sim.get_fields(0).cpu().numpy())
+    assert len(logs["seq"][0]) == N
+    assert np.array_equal(logs["batch"][0], logs["seq"][0])
+    assert np.array_equal(logs["batch"][1], logs["seq"][1]) and np.array_equal(logs["batch"][2], logs["seq"][2])
+    # no coupling at all: every spin of a sublattice ties exactly; lowest index first (reading C-7)
+    pos, ang = W.ising(20000, 1)
+    sim = B.Sim(pos, ang, np.full(20000, 0.1), dict(p, alpha=0.0))
+    assert sim.batch_stats()["max_seeds"] > 0
+    sim.set_field(-0.2, 0.05, 0)
+    assert sim.relax() == 20000
+    assert np.array_equal(sim.get_flip_log().cpu().numpy(), np.arange(20000))
+
+
+@pytest.mark.slow
+def test_batched_equals_sequential_config4_full_size(B):
+    """2,002,000 spins: batched against the one-flip-at-a-time kernel (which the oracle checks in
+    test_config4_full_size_protocol), whole protocol, log of every step."""
+    w = W.config("4")
+    logs = {}
+    for mode in ("batch", "seq"):
+        sim = B.Sim(w.pos, w.angle, w.hc, w.params); sim.set_thermal(w.sigma_th, w.thermal_seed)
+        if mode == "seq":
+            sim.set_batch(0)
+        out = []
+        for t, (hx, hy) in enumerate(w.fields):
+            sim.set_field(hx, hy, t)
+            if sim.relax():
+                out.append(sim.get_flip_log().cpu().numpy().copy())
+        logs[mode] = (np.concatenate(out), sim.get_fields(1).cpu().numpy(), sim.batch_stats())
+        sim.close()
+    assert np.array_equal(logs["batch"][0], logs["seq"][0]) and np.array_equal(logs["batch"][1], logs["seq"][1])
+    st = logs["batch"][2]
+    assert st["flips"] > 1_900_000 and st["flips"] / st["rounds"] > 100, st
