@@ -64,6 +64,8 @@ def lib():
         L.orc_cached_hdip.argtypes = [vp, vp]
         L.orc_gather_cached.argtypes = [vp]
         L.orc_monitor.argtypes = [vp, P(i64), P(dbl), P(dbl), i32]
+        L.orc_spin_correlation.argtypes = [vp, dbl, i64, vp, vp]
+        L.orc_vertex_populations.argtypes = [vp, vp, i64, vp]
         L.orc_energy.restype = dbl
         L.orc_energy.argtypes = [vp]
         L.orc_astroid_L.restype = dbl
@@ -189,3 +191,16 @@ class Oracle:
         return n.value, g.value, t.value
 
     def energy(self): return float(self.L.orc_energy(self.h))
+
+    def spin_correlation(self, bin_width, nbins):
+        """(sum of c_ij, number of pairs) per separation bin floor(|r_ij| / bin_width)."""
+        sm = np.zeros(nbins, np.int64); cnt = np.zeros(nbins, np.int64)
+        self.L.orc_spin_correlation(self.h, float(bin_width), int(nbins), sm.ctypes.data, cnt.ctypes.data)
+        return sm, cnt
+
+    def vertex_populations(self, vertices):
+        """Counts of Type I, II, III, IV vertices; vertices [V,4] spin indices."""
+        v = np.ascontiguousarray(vertices, np.int32); assert v.ndim == 2 and v.shape[1] == 4
+        out = np.zeros(4, np.int64)
+        self.L.orc_vertex_populations(self.h, v.ctypes.data, int(v.shape[0]), out.ctypes.data)
+        return out

@@ -15,7 +15,8 @@
 //
 // Pins (tests/test_oracle_pins.py, -m "not gpu"): two-dipole closed forms, lattice sums, astroid
 // special cases, Philox known answers, brute-force neighbours, exhaustive <=12-spin flip orders,
-// energy descent, global spin-flip symmetry, kagome 29x29 = 2638 magnets.
+// energy descent, global spin-flip symmetry, kagome 29x29 = 2638 magnets; spin-spin correlation
+// and vertex populations on hand-countable states (polarised, ground state, one flipped spin).
 // Unpinned by the paper: full-config flip sequences (no published values exist); they are pinned only
 // through Tier A == Tier B on small sizes plus the invariants above ("parity unpinned" for those).
 //
@@ -367,6 +368,62 @@ struct Oracle {
         return n;
     }
 
+    // ---- analysis reductions of the annealed state (section IV.B)
+    // "the correlation of two spins is defined as +1 (-1) if their dipole interaction is minimized (maximized)".
+    // The dipole interaction energy of the pair is E_ij = -m_i . H_ij = -s_i s_j g_par,ij (Eq. 3; the parallel
+    // coupling is symmetric), so c_ij = +1 if s_i s_j g_par,ij > 0, -1 if < 0 (reading D-5).  Pairs whose
+    // parallel coupling vanishes (|g_par| d^3 < 1e-9: the orientation does not change the energy) get c_ij = 0
+    // and are not counted.  "as a function of their lateral separation": pairs are binned by
+    // floor(|r_ij| / bin_width); every unordered pair of the neighbourhood is visited once.
+    void spin_correlation(double bin_width, int64_t nbins, int64_t* sum, int64_t* count) {
+        build_neighbors();
+        for (int64_t b = 0; b < nbins; ++b) { sum[b] = 0; count[b] = 0; }
+        for (int64_t i = 0; i < N; ++i)
+            for (int32_t j : nbr[i]) {
+                if (j <= i) continue;
+                double dx = x[i] - x[j], dy = y[i] - y[j];
+                double d = std::sqrt(dx * dx + dy * dy);
+                int64_t b = (int64_t)std::floor(d / bin_width);
+                if (b >= nbins) continue;
+                double g[2]; coupling(i, j, g);
+                if (std::fabs(g[0]) * (d * d * d) < 1e-9) continue;
+                int c = ((double)s[i] * (double)s[j] * g[0] > 0.0) ? 1 : -1;
+                sum[b] += c; count[b] += 1;
+            }
+    }
+
+    // Vertex populations ("analysis of vertex populations"; Fig. 6: "Type I vertices"
+    // have zero net magnetization, "Type II or III" a non-zero one).  A vertex is a point where four magnets meet
+    // (square and pinwheel ASI); it is given by its four spin indices.  A moment points INTO the vertex if
+    // m_i . (r_v - r_i) > 0, r_v = mean of the four positions.  Types by the number of moments pointing in:
+    // 0 or 4 -> IV; 1 or 3 -> III; 2 -> I if the two in-pointing magnets sit on opposite sides of the vertex (the
+    // net moment cancels), II if they are adjacent (net moment non-zero)  (reading D-6).
+    void vertex_populations(const int32_t* vert, int64_t V, int64_t counts[4]) const {
+        for (int t = 0; t < 4; ++t) counts[t] = 0;
+        for (int64_t v = 0; v < V; ++v) {
+            const int32_t* q = vert + 4 * v;
+            double vx = 0.0, vy = 0.0;
+            for (int a = 0; a < 4; ++a) { vx += x[q[a]]; vy += y[q[a]]; }
+            vx *= 0.25; vy *= 0.25;
+            int nin = 0; double inx = 0.0, iny = 0.0; bool first = true; bool opposite = false;
+            for (int a = 0; a < 4; ++a) {
+                int64_t i = q[a];
+                double rx = vx - x[i], ry = vy - y[i];
+                double mx = s[i] * ct[i], my = s[i] * st[i];
+                if (mx * rx + my * ry > 0.0) {
+                    ++nin;
+                    if (first) { inx = rx; iny = ry; first = false; }
+                    else opposite = (inx * rx + iny * ry) < 0.0;      // meaningful when exactly two point in
+                }
+            }
+            int type;
+            if (nin == 0 || nin == 4) type = 3;
+            else if (nin == 1 || nin == 3) type = 2;
+            else type = opposite ? 0 : 1;
+            counts[type]++;
+        }
+    }
+
     // E = -1/2 sum_i m_i . h_dip,i - sum_i m_i . (h_ext + h_th)_i   (used by pin P-8 only; reading C-20)
     double energy() {
         double E = 0.0;
@@ -454,6 +511,12 @@ void orc_gather_cached(void* h) { ((Oracle*)h)->gather_cached(); }
 void orc_monitor(void* h, int64_t* n_events, double* min_gap, double* min_thr, int reset) {
     Oracle* o = (Oracle*)h; *n_events = o->n_events; *min_gap = o->min_gap; *min_thr = o->min_thr;
     if (reset) { o->n_events = 0; o->min_gap = 1e300; o->min_thr = 1e300; }
+}
+void orc_spin_correlation(void* h, double bin_width, int64_t nbins, int64_t* sum, int64_t* count) {
+    ((Oracle*)h)->spin_correlation(bin_width, nbins, sum, count);
+}
+void orc_vertex_populations(void* h, const int32_t* vert, int64_t V, int64_t* counts4) {
+    ((Oracle*)h)->vertex_populations(vert, V, counts4);
 }
 double orc_energy(void* h) { Oracle* o = (Oracle*)h; o->build_neighbors(); return o->energy(); }
 double orc_astroid_L(double hpar, double hperp, double hk, const orc_params* p) {

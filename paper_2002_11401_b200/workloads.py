@@ -114,6 +114,27 @@ def kagome(n: int):
     return np.ascontiguousarray(pos), np.ascontiguousarray(angle)
 
 
+def square_vertices(n: int):
+    """Interior vertices of `square_closed(n)`: the lattice points (x, y), 0 < x, y < n, where four magnets meet
+    (Fig. 6a "ASI vertices").  Returns [V,4] spin indices (left, right, below, above), V = (n-1)^2."""
+    y, x = np.meshgrid(np.arange(1, n), np.arange(1, n), indexing="ij")
+    x = x.ravel(); y = y.ravel()
+    nh = n * (n + 1)
+    left = y * n + (x - 1); right = y * n + x
+    below = nh + (y - 1) * (n + 1) + x; above = nh + y * (n + 1) + x
+    return np.ascontiguousarray(np.stack([left, right, below, above], axis=1).astype(np.int32))
+
+
+def square_ground_state(n: int):
+    """The antiferromagnetic ground state of `square_closed(n)` (every vertex Type I): horizontal
+    spins alternate with (i + j), vertical spins with (i + j + 1)."""
+    j, i = np.meshgrid(np.arange(n + 1), np.arange(n), indexing="ij")
+    sh = np.where((i + j) % 2 == 0, 1, -1).ravel()
+    j, i = np.meshgrid(np.arange(n), np.arange(n + 1), indexing="ij")
+    sv = np.where((i + j) % 2 == 0, -1, 1).ravel()
+    return np.concatenate([sh, sv]).astype(np.int8)
+
+
 # --------------------------------------------------------------------------- per-magnet inputs
 def coercive_fields(N: int, hk: float = 0.2, k_disorder: float = 0.05, seed: int = 0, replicas: int = 0):
     """h_k^(i) ~ N(h_k, (k_disorder h_k)^2), redrawn until positive.
@@ -153,6 +174,34 @@ def ramp(A: float, B: float, K: int, phi_deg: float, legs: int = 1):
         H = A + (B - A) * (1.0 - np.abs(1.0 - 2.0 * t / K))
     phi = math.radians(phi_deg)
     return np.ascontiguousarray(np.stack([H * math.cos(phi), H * math.sin(phi)], axis=1))
+
+
+def sinusoidal(amplitude: float, periods: float, steps_per_period: int, phi_deg: float, offset: float = 0.0):
+    """Input encoder "sinusoidal field": H_t = offset + A sin(2 pi t / steps_per_period) along
+    the fixed direction phi, t = 0 .. periods * steps_per_period.  Returns [T,2]."""
+    T = int(round(periods * steps_per_period)) + 1
+    t = np.arange(T, dtype=np.float64)
+    H = offset + amplitude * np.sin(2.0 * math.pi * t / steps_per_period)
+    phi = math.radians(phi_deg)
+    return np.ascontiguousarray(np.stack([H * math.cos(phi), H * math.sin(phi)], axis=1))
+
+
+def sawtooth(amplitude: float, periods: float, steps_per_period: int, phi_deg: float):
+    """Input encoder "sawtooth field": H_t rises linearly from -A to +A over one period, then jumps
+    back.  Returns [T,2]."""
+    T = int(round(periods * steps_per_period)) + 1
+    t = np.arange(T, dtype=np.float64)
+    H = amplitude * (2.0 * ((t / steps_per_period) % 1.0) - 1.0)
+    phi = math.radians(phi_deg)
+    return np.ascontiguousarray(np.stack([H * math.cos(phi), H * math.sin(phi)], axis=1))
+
+
+def rotating(amplitude: float, periods: float, steps_per_period: int, phi0_deg: float = 0.0):
+    """Input encoder "rotational field": constant magnitude A, direction phi0 + 2 pi t /
+    steps_per_period.  Returns [T,2]."""
+    T = int(round(periods * steps_per_period)) + 1
+    phi = math.radians(phi0_deg) + 2.0 * math.pi * np.arange(T, dtype=np.float64) / steps_per_period
+    return np.ascontiguousarray(np.stack([amplitude * np.cos(phi), amplitude * np.sin(phi)], axis=1))
 
 
 # --------------------------------------------------------------------------- the five configs
@@ -244,3 +293,21 @@ def paper_kagome_dirac_strings(n: int = 29, K: int = 400, amplitude: float = 0.1
     return Workload(f"paperIVA_kagome_{n}x{n}", pos, ang, coercive_fields(len(ang), hk=0.216, k_disorder=0.05, seed=0),
                     spins, _params(0.00103, 0.212, 1.0, 2.5, 3.0, SQRT3), ramp(0.0, amplitude, K, -3.6, legs=1),
                     sigma_th=0.002, thermal_seed=0, note="PAPER.md:182 parameters; neighbourhood and field range not given")
+
+
+def paper_square_anneal(n: int = 50, alpha: float = 0.0015, T: int = 200, sigma0: float = 0.1, decay: float = 40.0,
+                        replicas: int = 0, seed: int = 0) -> Workload:
+    """PAPER.md:196-206 (section IV.B): 50 x 50 square ASI (closed edges), annealed by a thermal protocol of
+    exponentially decreasing sigma_th; b = 0.4, c = 1, beta = gamma = 3, h_k = 0.186, k_disorder = 0.05, neighbor
+    distance 10; no external field.  The paper gives neither the map from the lattice constant a to alpha nor the
+    protocol constants: alpha, sigma0 and the decay (sigma_t = sigma0 exp(-t / decay), T steps) are this recipe's.
+    Spins start random.  `extra` carries sigma[T] and the interior vertices [V,4]; `replicas` > 0 draws that many
+    h_c disorder realisations [R,N] (an ensemble, "across the ensembles")."""
+    pos, ang = square_closed(n)
+    N = len(ang)
+    hc = coercive_fields(N, hk=0.186, k_disorder=0.05, seed=seed, replicas=replicas)
+    sigma = sigma0 * np.exp(-np.arange(T, dtype=np.float64) / decay)
+    return Workload(f"paperIVB_square_anneal_{n}x{n}", pos, ang, hc, random_spins(N, seed=seed + 1),
+                    _params(alpha, 0.4, 1.0, 3.0, 3.0, 10.0), np.zeros((T, 2)), sigma_th=float(sigma[0]), thermal_seed=seed,
+                    note="PAPER.md:202 parameters; alpha and the annealing schedule are not given in the paper",
+                    extra={"sigma": sigma, "vertices": square_vertices(n)})

@@ -518,3 +518,112 @@ def test_local_field_pins():
     one.set_field(0.0, 0.0, 0)
     one.set_local_field(np.array([[-0.1999, 0.0]])); assert one.relax_A()[0] == 0
     one.set_local_field(np.array([[-0.2001, 0.0]])); assert one.relax_A()[0] == 1 and one.spins()[0] == -1
+
+
+# ------------------------------------------------------------------ analysis reductions
+def _square(n, nd=1.0):
+    pos, ang = W.square_closed(n)
+    return Oracle(pos, ang, np.full(len(ang), 0.2), P(neighbor_distance=nd)), len(ang)
+
+
+@pytest.mark.parametrize("n", [4, 7])
+def test_vertex_populations_hand_counted_states(n):
+    """Polarised state: every vertex Type II; ground state: every vertex Type I (zero net
+    magnetisation); one flipped spin in the ground state: its two vertices become Type III; two spins turned so
+    that all four point into one vertex: that vertex is Type IV and its two neighbours Type III."""
+    o, N = _square(n)
+    V = W.square_vertices(n)
+    assert V.shape == ((n - 1) ** 2, 4)
+    nv = (n - 1) ** 2
+    assert list(o.vertex_populations(V)) == [0, nv, 0, 0]
+    o.set_spins(-np.ones(N, np.int8))
+    assert list(o.vertex_populations(V)) == [0, nv, 0, 0]
+    g = W.square_ground_state(n)
+    o.set_spins(g)
+    assert list(o.vertex_populations(V)) == [nv, 0, 0, 0]
+    o.set_spins(-g)
+    assert list(o.vertex_populations(V)) == [nv, 0, 0, 0]
+    s = g.copy(); k = V[0][1]          # the magnet right of the first interior vertex (1, 1): interior, two vertices
+    s[k] = -s[k]; o.set_spins(s)
+    assert list(o.vertex_populations(V)) == [nv - 2, 0, 2, 0]
+    s = np.ones(N, np.int8)            # all +1: left and below point in; turn right and above inwards as well
+    v = V[0]; s[v[1]] = -1; s[v[3]] = -1; o.set_spins(s)
+    assert list(o.vertex_populations(V)) == [0, nv - 3, 2, 1]
+    # the net moment of a Type I vertex vanishes and that of a Type II vertex does not (PAPER.md:214)
+    pos, ang = W.square_closed(n)
+    m = g[:, None] * np.stack([np.cos(ang), np.sin(ang)], 1)
+    assert np.abs(m[V].sum(axis=1)).max() < 1e-12
+    m = np.stack([np.cos(ang), np.sin(ang)], 1)
+    assert np.abs(m[V].sum(axis=1)).min() > 1.9
+
+
+@pytest.mark.parametrize("n", [4, 6])
+def test_spin_correlation_hand_counted_states(n):
+    """c_ij = +1 (-1) if the pair's dipole interaction is minimised (maximised).  Square ASI, nd = 1:
+    4 n^2 nearest pairs at 1/sqrt2 and 2 [(n-1)(n+1) + n^2] pairs at distance 1 (collinear + side by side).
+    Polarised state: head-to-tail collinear pairs are minimised (+1), parallel side-by-side pairs maximised (-1),
+    the nearest pairs split evenly.  Ground state: every nearest pair minimised."""
+    o, N = _square(n)
+    col, side = 2 * (n - 1) * (n + 1), 2 * n * n
+    sm, cnt = o.spin_correlation(0.25, 6)
+    assert list(cnt) == [0, 0, 4 * n * n, 0, col + side, 0]
+    assert list(sm) == [0, 0, 0, 0, col - side, 0]
+    g = W.square_ground_state(n); o.set_spins(g)
+    sm, cnt = o.spin_correlation(0.25, 6)
+    assert list(sm) == [0, 0, 4 * n * n, 0, side - col, 0]
+    s = g.copy(); k = W.square_vertices(n)[0][1]; s[k] = -s[k]; o.set_spins(s)      # an interior horizontal magnet:
+    sm2, _ = o.spin_correlation(0.25, 6)                                           # 4 nearest, 2 collinear, 2 side pairs
+    assert sm2[2] == 4 * n * n - 8 and sm2[4] == (side - col) - 2 * (2 - 2)
+    # global spin reversal leaves every pair energy unchanged
+    o.set_spins(-s)
+    assert np.array_equal(o.spin_correlation(0.25, 6)[0], sm2)
+    # pairs beyond the last bin are dropped, the bin of a pair is floor(d / width)
+    sm3, cnt3 = o.spin_correlation(0.5, 2)
+    assert list(cnt3) == [0, 4 * n * n]
+    # pinwheel: nearest neighbours have no parallel coupling at all in the point-dipole model (r is parallel to
+    # one moment and perpendicular to the other): they are not counted
+    pos, ang = W.rotated_square(n)
+    o = Oracle(pos, ang, np.full(len(ang), 0.2), P(neighbor_distance=1.0))
+    sm, cnt = o.spin_correlation(0.25, 6)
+    assert cnt[2] == 0 and cnt[4] == col + side
+
+
+def test_correlation_agrees_with_pair_energies_bruteforce():
+    """Independent restatement: E_ij = -s_i s_j g_par,ij from orc.coupling; c = -sign(E)."""
+    w = W.config("3", scale=5)
+    s = W.random_spins(w.N, seed=3)
+    o = Oracle(w.pos, w.angle, w.hc, w.params, spins=s)
+    nb = o.neighbors()
+    sm = np.zeros(8, np.int64); cnt = np.zeros(8, np.int64)
+    for i in range(w.N):
+        for j in nb[i]:
+            if j <= i:
+                continue
+            d = math.hypot(*(w.pos[i] - w.pos[j]))
+            gpar = o.coupling(i, j)[0]
+            if abs(gpar) * d ** 3 < 1e-9:
+                continue
+            E = -float(s[i]) * float(s[j]) * gpar
+            b = int(d // 0.5)
+            sm[b] += 1 if E < 0 else -1; cnt[b] += 1
+    a, c = o.spin_correlation(0.5, 8)
+    assert np.array_equal(a, sm) and np.array_equal(c, cnt) and cnt.sum() > 0
+
+
+def test_field_protocol_generators():
+    """Input encoders of PAPER.md:63, :156 (sinusoidal, sawtooth, rotational): closed forms."""
+    f = W.sinusoidal(0.1, 2, 8, 30.0)
+    assert f.shape == (17, 2)
+    H = f @ np.array([math.cos(math.radians(30)), math.sin(math.radians(30))])
+    assert np.allclose(H, 0.1 * np.sin(2 * math.pi * np.arange(17) / 8), atol=1e-15)
+    assert np.allclose(f[:, 0] * math.sin(math.radians(30)), f[:, 1] * math.cos(math.radians(30)), atol=1e-15)
+    f = W.sawtooth(0.2, 3, 10, 0.0)
+    assert f.shape == (31, 2) and np.allclose(f[:, 1], 0)
+    assert np.allclose(f[:10, 0], -0.2 + 0.04 * np.arange(10)) and np.allclose(f[10:20, 0], f[:10, 0])
+    f = W.rotating(0.15, 3, 12, 10.0)
+    assert f.shape == (37, 2) and np.allclose(np.hypot(f[:, 0], f[:, 1]), 0.15)
+    assert np.allclose(np.degrees(np.arctan2(f[3, 1], f[3, 0])), 10.0 + 90.0) and np.allclose(f[12], f[0])
+    w = W.paper_square_anneal(50)
+    assert w.N == 5100 and w.params["neighbor_distance"] == 10.0 and w.params["b"] == 0.4
+    sig = w.extra["sigma"]
+    assert np.all(np.diff(np.log(sig)) < 0) and np.allclose(np.diff(np.log(sig)), np.diff(np.log(sig))[0])   # exponential
