@@ -43,9 +43,11 @@ struct BatchUndo { double2 hd; double M; int idx; int pad; };
 struct BatchCommit { mkey_t nev; unsigned long long lo; int k; int pad; };   // sort key (~ev, ei << 32 | pos), ascending
 struct BatchBlock { mkey_t ev; int ei; int pos; };
 
-struct BatchCtl {                      // zeroed by the host before every launch
-    unsigned bar;                      // grid barrier counter (monotone)
-    unsigned bail;                     // 1 = exact ties defeat the threshold search: leave everything to k_relax
+struct BatchCtl {                      // zeroed once at creation; every launch leaves it clean for the next one
+    unsigned bar[2];                   // grid barrier counters (monotone within a launch), alternating between launches
+    unsigned bail;                     // 1 = exact ties defeated the threshold search in the last launch
+    unsigned round_base;               // rounds of all launches so far: the claim tag of a round is unique across launches
+    unsigned launch;                   // launches that used the barrier so far (their parity picks the counter)
     unsigned n_seeds[4], n_commit[4], n_block[4];      // rotating per-round counters
     unsigned long long n_cand[3];
     unsigned hist[3][BT_NB];           // rotating histograms (one per pass)
@@ -114,7 +116,21 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     const int64_t N = a.N;
     const int Kp = a.Kp;
     BatchCtl* g = a.ctl;
+    // k_scan (finalize) left the number of switchable spins: with only a few, k_relax does it alone (uniform exit,
+    // nothing touched)
+    if (__ldcg(&a.ctr[0].n_switchable) <= (long long)a.seq_threshold) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) a.ctr[0].batch_flips = 0;
+        return;
+    }
+    const unsigned parity = __ldcg(&g->launch) & 1u;
+    unsigned* const bar = &g->bar[parity];
     unsigned epoch = 0;
+    unsigned round_base = __ldcg(&g->round_base);
+    if (round_base > 0xF0000u) {                        // claim tags nearly used up: wipe the claim table
+        for (int64_t i = blockIdx.x * (int64_t)BT_THREADS + threadIdx.x; i < a.N; i += (int64_t)gridDim.x * BT_THREADS) a.owner[i] = 0xFFFFFFFFu;
+        grid_bar(bar, epoch);
+        round_base = 0;
+    }
     long long nflips = 0, rounds = 0, undone = 0, nblockers = 0;
     int rot = 0;                                        // rotating counter slot of this round
     unsigned npass = 0;                                 // histogram passes so far (buffer = npass % 3)
@@ -122,8 +138,8 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     int lean = 0;                                       // consecutive rounds that committed fewer than min_commit flips
 
     for (;; ++rounds) {
-        const unsigned tag = 0xFFFFFu - (unsigned)rounds;            // newer rounds win an atomicMin on the claim word
-        if (rounds >= 0xFFFF0) break;
+        const unsigned tag = 0xFFFFFu - (round_base + (unsigned)rounds);   // newer rounds win an atomicMin on the claim word
+        if (rounds >= 0xFFF0) break;
         // ================= phase 1: threshold theta such that <= P candidates have key > theta ==============
         // One pass over all margins builds a histogram of log-spaced bins of (key - 1); theta is the lower edge
         // of the lowest bin b* whose suffix count still fits P.  If that takes fewer than P/4 seeds although the
@@ -154,7 +170,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 my_cand = __reduce_add_sync(0xffffffffu, my_cand);
                 if (lane == 0 && my_cand) atomicAdd(&g->n_cand[hb], (unsigned long long)my_cand);
             }
-            grid_bar(&g->bar, epoch);
+            grid_bar(bar, epoch);
             if (blockIdx.x == 0) {                                   // the buffer of the previous pass: everyone has read it
                 const int zb = (hb + 2) % 3;
                 for (int b = tid; b < BT_NB; b += BT_THREADS) g->hist[zb][b] = 0;
@@ -224,7 +240,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 }
             }
         }
-        grid_bar(&g->bar, epoch);
+        grid_bar(bar, epoch);
         const int n_seeds = (int)min(__ldcg(&g->n_seeds[rot]), (unsigned)BT_PMAX);
         if (blockIdx.x == 0 && tid == 0) {                                       // counters two rounds ahead
             const int z = (rot + 2) & 3;
@@ -240,7 +256,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 if (i >= 0) atomicMin(a.owner + i, word);
             }
         }
-        grid_bar(&g->bar, epoch);
+        grid_bar(bar, epoch);
         // ================= phase 4: conflict edges (seed r shares a spin with the seed that owns it) ========
         for (int r = gwarp; r < n_seeds; r += nwarps) {
             const int k = seeds[r].idx;
@@ -262,7 +278,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             }
             if (lane == 0) a.ecount[r] = (unsigned char)(ne > BT_EMAX ? 0xFF : ne);
         }
-        grid_bar(&g->bar, epoch);
+        grid_bar(bar, epoch);
         // ================= phase 5: components (every CTA computes the same labels in shared memory) ========
         for (int r = tid; r < n_seeds; r += BT_THREADS) { sh_label[r] = r; sh_cnt[r] = 0; }
         __syncthreads();
@@ -398,7 +414,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 }
             }
         }
-        grid_bar(&g->bar, epoch);
+        grid_bar(bar, epoch);
         // ================= phase 7: the cut = earliest blocker (or theta); commit before it, undo after it ====
         mkey_t cv = theta; int ci = -1, cp = 0;
         {
@@ -445,7 +461,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             }
             if (lane == 0) undone += np - keep;
         }
-        grid_bar(&g->bar, epoch);
+        grid_bar(bar, epoch);
         // ================= phase 8: merged order -> flip log =================================================
         const int nc = (int)__ldcg(&g->n_commit[rot]);
         for (int q = gwarp; q < nc; q += nwarps) {
@@ -469,7 +485,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         //  clist is rewritten only after three more barriers)
     }
     // ================= tail: leaf maxima for k_relax, counters ===============================================
-    grid_bar(&g->bar, epoch);
+    grid_bar(bar, epoch);
     if (any_flip) {
         const int LB = 1 << a.LBshift;
         for (int b = gwarp; b < a.nblk; b += nwarps) {
@@ -491,6 +507,12 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     // per-warp statistics -> one atomic per warp
     undone = __reduce_add_sync(0xffffffffu, (unsigned)undone);
     if (lane == 0 && undone) atomicAdd((unsigned long long*)&g->undone, (unsigned long long)undone);
+    if (blockIdx.x == 0) {                              // leave the control block clean for the next launch
+        for (int b = tid; b < 3 * BT_NB; b += BT_THREADS) (&g->hist[0][0])[b] = 0;
+        if (tid < 4) { g->n_seeds[tid] = 0; g->n_commit[tid] = 0; g->n_block[tid] = 0; }
+        if (tid < 3) g->n_cand[tid] = 0;
+        if (tid == 0) { g->bar[parity ^ 1u] = 0; g->launch = g->launch + 1; g->round_base = round_base + (unsigned)rounds; }
+    }
     if (gtid == 0) {
         g->flips = nflips; g->rounds = rounds; g->blockers = nblockers;
         a.ctr[0].batch_flips = nflips;

@@ -1465,8 +1465,6 @@ int launch_batch(fs_sim* sim) {
     BatchArgs a = sim->bt;
     a.cellidx = sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr;
     a.P = sim->bt_P; a.seq_threshold = sim->bt_seq; a.min_commit = sim->bt_min_commit;
-    CUDA_TRY(cudaMemsetAsync(a.ctl, 0, sizeof(BatchCtl), sim->stream));
-    CUDA_TRY(cudaMemsetAsync(a.owner, 0xff, 4 * (size_t)sim->N, sim->stream));
     void* args[] = {&a};
     CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_relax_batch, dim3((unsigned)sim->bt_grid), dim3(BT_THREADS), args, 0, sim->stream));
     LAUNCHED();
@@ -1474,9 +1472,9 @@ int launch_batch(fs_sim* sim) {
 }
 
 int do_relax(fs_sim* sim, int64_t max_flips) {
-    int rc = do_scan(sim, false);
-    if (rc) return rc;
     const bool batch = sim->bt_ok && sim->bt_P > 0 && max_flips <= 0;
+    int rc = do_scan(sim, batch);                        // the batched kernel wants the number of switchable spins
+    if (rc) return rc;
     if (batch) { rc = launch_batch(sim); if (rc) return rc; }
     return launch_relax(sim, max_flips, 0, nullptr, 0, nullptr, nullptr, batch ? 1 : 0);
 }
@@ -1511,6 +1509,10 @@ int setup_batch(fs_sim* sim) {
     a.edges = (unsigned short*)(b + o_edges); a.ecount = b + o_ecount; a.npos = (int*)(b + o_npos);
     a.elems = (BatchElem*)(b + o_elems); a.undo = (BatchUndo*)(b + o_undo); a.blocks = (BatchBlock*)(b + o_blocks);
     a.clist = (BatchCommit*)(b + o_clist);
+    if (cudaMemsetAsync(a.ctl, 0, sizeof(BatchCtl), sim->stream) != cudaSuccess ||
+        cudaMemsetAsync(a.owner, 0xff, 4 * (size_t)sim->N, sim->stream) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(sim->bt_mem); sim->bt_mem = nullptr; return FS_OK;
+    }
     sim->bt_P = P; sim->bt_seq = 64; sim->bt_grid = sim->sm_count; sim->bt_ok = true;
     return FS_OK;
 }
