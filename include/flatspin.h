@@ -64,8 +64,11 @@ enum { FS_FIELD_TOTAL = 0, FS_FIELD_DIP = 1, FS_FIELD_EXT = 2, FS_FIELD_THERMAL 
  *   1 = ELL: neighbour indices + fp64 coupling pairs streamed from HBM (20 B / interaction; HBM-bound);
  *   2 = lattice stencil: dense per-sublattice spin grids correlated with the table
  *       T[sub_i][sub_j][du][dv] = alpha*g_ij held in shared memory (no per-interaction HBM traffic;
- *       FP64-pipe bound).  FS_ERR_ARG if the geometry is not a verified regular lattice. */
-enum { FS_GATHER_AUTO = 0, FS_GATHER_ELL_F64 = 1, FS_GATHER_STENCIL = 2 };
+ *       FP64-pipe bound).  FS_ERR_ARG if the geometry is not a verified regular lattice.  Where the table has an
+ *       exact inversion pairing (Eq. 3 is even in r_ij: T[d] == T[-d], bit for bit) the kernel adds the two
+ *       spins of a slot pair first: 3 FP64 operations per 2 interactions instead of 4;
+ *   3 = lattice stencil without the inversion pairing (one DFMA pair per interaction). */
+enum { FS_GATHER_AUTO = 0, FS_GATHER_ELL_F64 = 1, FS_GATHER_STENCIL = 2, FS_GATHER_STENCIL_PLAIN = 3 };
 
 /* Why the stencil is not available (fs_get_lattice info[1]); 0 = it is. */
 enum {
@@ -128,9 +131,9 @@ int fs_set_local_field(fs_sim* sim, const double* h_dev);
 int fs_set_gather_variant(fs_sim* sim, int variant);
 
 /* Result of the regular-lattice detection run by fs_create (flatspin geometries are
- * lattices with 1-3 sublattices, :146).  info HOST [10] int32: {stencil active, FS_LATTICE_* reason,
+ * lattices with 1-3 sublattices, :146).  info HOST [12] int32: {stencil active, FS_LATTICE_* reason,
  * sublattices, U, V (cells along the two lattice vectors), Ru, Rv (stencil half-extents), stencil
- * slots present, warps per CTA, shared-memory bytes per CTA}.  dinfo HOST [2]: {max |w_ELL - T| over
+ * slots present, warps per CTA, shared-memory bytes per CTA, inversion pairing active, row pairs}.  dinfo HOST [2]: {max |w_ELL - T| over
  * all interactions, max |w|}.  Either may be NULL.  No synchronise. */
 int fs_get_lattice(const fs_sim* sim, int32_t* info, double* dinfo);
 

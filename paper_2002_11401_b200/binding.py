@@ -16,7 +16,7 @@ from . import build as _build
 
 FS_OK, FS_ERR_ARG, FS_ERR_COINCIDENT, FS_ERR_WORKSPACE, FS_ERR_CUDA, FS_ERR_MAXFLIPS = 0, -1, -2, -3, -4, -5
 FIELD_TOTAL, FIELD_DIP, FIELD_EXT, FIELD_THERMAL = 0, 1, 2, 3
-GATHER_AUTO, GATHER_ELL_F64, GATHER_STENCIL = 0, 1, 2
+GATHER_AUTO, GATHER_ELL_F64, GATHER_STENCIL, GATHER_STENCIL_PLAIN = 0, 1, 2, 3
 
 EXPORTS = [
     "fs_workspace_bytes", "fs_create", "fs_create_ensemble", "fs_destroy", "fs_get_info", "fs_set_spins",
@@ -207,11 +207,11 @@ class Sim:
         return {"max_seeds": int(out[0]), "flips": int(out[1]), "rounds": int(out[2]), "seq_threshold": int(out[3])}
 
     def lattice(self) -> dict:
-        info = np.zeros(10, np.int32); d = np.zeros(2, np.float64)
+        info = np.zeros(12, np.int32); d = np.zeros(2, np.float64)
         _check(self.L, self.L.fs_get_lattice(self.h, info.ctypes.data, d.ctypes.data))
-        keys = ("active", "reason", "nsub", "U", "V", "Ru", "Rv", "slots", "warps_per_cta", "smem_bytes")
+        keys = ("active", "reason", "nsub", "U", "V", "Ru", "Rv", "slots", "warps_per_cta", "smem_bytes", "inversion_pairs", "row_pairs")
         out = {k: int(v) for k, v in zip(keys, info)}
-        out["active"] = bool(out["active"]); out["max_dev"] = float(d[0]); out["w_max"] = float(d[1])
+        out["active"] = bool(out["active"]); out["inversion_pairs"] = bool(out["inversion_pairs"]); out["max_dev"] = float(d[0]); out["w_max"] = float(d[1])
         return out
 
     # ---- compute

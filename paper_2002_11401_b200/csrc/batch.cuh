@@ -52,6 +52,7 @@ struct BatchCtl {                      // zeroed once at creation; every launch 
     unsigned long long n_cand[3];
     unsigned hist[3][BT_NB];           // rotating histograms (one per pass)
     long long flips, rounds, undone, blockers;         // results / statistics of this launch
+    long long prof[12];                // FS_BATCH_PROFILE: nanoseconds per phase (CTA 0), accumulated
 };
 
 struct BatchArgs {
@@ -101,6 +102,13 @@ __device__ __forceinline__ bool bt_before(mkey_t ev, int ei, int pos, mkey_t bv,
     return ev > bv || (ev == bv && (ei < bi || (ei == bi && pos < bp)));
 }
 
+#ifdef FS_BATCH_PROFILE
+__device__ __forceinline__ long long bt_now() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define BT_PROF(slot) do { if (gtid == 0) { const long long t_ = bt_now(); g->prof[slot] += t_ - tprof; tprof = t_; } } while (0)
+#else
+#define BT_PROF(slot)
+#endif
+
 __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     __shared__ unsigned sh_hist[BT_NB];
     __shared__ int sh_label[BT_PMAX];
@@ -137,6 +145,9 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     bool any_flip = false;
     int lean = 0;                                       // consecutive rounds that committed fewer than min_commit flips
 
+#ifdef FS_BATCH_PROFILE
+    long long tprof = bt_now();
+#endif
     for (;; ++rounds) {
         const unsigned tag = 0xFFFFFu - (round_base + (unsigned)rounds);   // newer rounds win an atomicMin on the claim word
         if (rounds >= 0xFFF0) break;
@@ -223,6 +234,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             if (ncand_total > (unsigned long long)a.seq_threshold && gtid == 0) g->bail = 1;       // exact ties defeat the search
             break;
         }
+        BT_PROF(0);
         // ================= phase 2: seeds = candidates with key > theta ====================================
         BatchSeed* seeds = a.seeds;
         for (int64_t i0 = (int64_t)gwarp * 32; i0 < N; i0 += (int64_t)nwarps * 32) {
@@ -246,6 +258,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             const int z = (rot + 2) & 3;
             g->n_seeds[z] = 0; g->n_commit[z] = 0; g->n_block[z] = 0;
         }
+        BT_PROF(1);
         // ================= phase 3: claims.  owner[t] = min over seeds claiming t of (tag, slot) ============
         for (int r = gwarp; r < n_seeds; r += nwarps) {
             const int k = seeds[r].idx;
@@ -257,6 +270,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             }
         }
         grid_bar(bar, epoch);
+        BT_PROF(2);
         // ================= phase 4: conflict edges (seed r shares a spin with the seed that owns it) ========
         for (int r = gwarp; r < n_seeds; r += nwarps) {
             const int k = seeds[r].idx;
@@ -279,6 +293,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             if (lane == 0) a.ecount[r] = (unsigned char)(ne > BT_EMAX ? 0xFF : ne);
         }
         grid_bar(bar, epoch);
+        BT_PROF(3);
         // ================= phase 5: components (every CTA computes the same labels in shared memory) ========
         for (int r = tid; r < n_seeds; r += BT_THREADS) { sh_label[r] = r; sh_cnt[r] = 0; }
         __syncthreads();
@@ -303,6 +318,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         }
         for (int r = tid; r < n_seeds; r += BT_THREADS) atomicAdd(&sh_cnt[sh_label[r]], 1u);     // members per component
         __syncthreads();
+        BT_PROF(4);
         // ================= phase 6: one warp per component runs the sequential rule locally ==================
         for (int r = gwarp; r < n_seeds; r += nwarps) {
             if (sh_label[r] != r) continue;                                      // not a leader
@@ -414,7 +430,9 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 }
             }
         }
+        BT_PROF(5);
         grid_bar(bar, epoch);
+        BT_PROF(6);
         // ================= phase 7: the cut = earliest blocker (or theta); commit before it, undo after it ====
         mkey_t cv = theta; int ci = -1, cp = 0;
         {
@@ -462,6 +480,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             if (lane == 0) undone += np - keep;
         }
         grid_bar(bar, epoch);
+        BT_PROF(7);
         // ================= phase 8: merged order -> flip log =================================================
         const int nc = (int)__ldcg(&g->n_commit[rot]);
         for (int q = gwarp; q < nc; q += nwarps) {
@@ -474,6 +493,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             rank = __reduce_add_sync(0xffffffffu, rank);
             if (lane == 0 && nflips + rank < a.log_cap) a.flog[nflips + rank] = me.k;
         }
+        BT_PROF(8);
         nflips += nc;
         any_flip |= nc > 0;
         rot = (rot + 1) & 3;

@@ -979,6 +979,8 @@ struct fs_sim {
     sgcell_t* sgrid = nullptr; int* cellidx = nullptr; bool sgrid_valid = false;
     int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
     int st_nw = 4, st_rs = 1, st_pv = 0, st_ov = ST_OV; size_t st_smem = 0; bool st_ct = false;
+    bool st_sym = false;            // inversion-paired stencil (c_prow / c_pstart tables below, host copies: they are tiny)
+    std::vector<int4> prow; std::vector<int2> pstart; std::vector<int> ptofs, rtofs;
     unsigned long long st_id = 0;   // identity for the ownership of the constant-memory table
     double st_maxdev = 0.0, st_wmax = 0.0;
     long long st_slots = 0;         // stencil slots present (sum over sublattice pairs)
@@ -1128,9 +1130,17 @@ int do_gather_stencil(fs_sim* sim) {
     }
     dim3 grid((unsigned)((g.U + ST_TU - 1) / ST_TU), (unsigned)((g.V + TV - 1) / TV), (unsigned)(g.nsub * sim->R));
     int threads = 32 * sim->st_nw * sim->st_rs;
-#define FS_LAUNCH_STENCIL1(MAXT, MINB, CTV, OVV)                                                    \
-    k_gather_stencil<MAXT, MINB, CTV, OVV><<<grid, threads, sim->st_smem, sim->stream>>>(           \
-        sim->N, g, sim->st_nw, sim->st_pv, sim->gidx, sim->sgrid, sim->T, sim->rowtab, sim->hdip)
+#define FS_STENCIL_ARGS sim->N, g, sim->st_nw, sim->st_pv, sim->gidx, sim->sgrid, sim->T, sim->rowtab, sim->hdip
+#define FS_LAUNCH_STENCIL1(MAXT, MINB, CTV, OVV)                                                                     \
+    do {                                                                                                             \
+        if (sim->st_pv == 64) k_gather_stencil<MAXT, MINB, CTV, OVV, false, 64><<<grid, threads, sim->st_smem, sim->stream>>>(FS_STENCIL_ARGS); \
+        else k_gather_stencil<MAXT, MINB, CTV, OVV, false, 128><<<grid, threads, sim->st_smem, sim->stream>>>(FS_STENCIL_ARGS);                  \
+    } while (0)
+#define FS_LAUNCH_STENCIL_SYM(MAXT, MINB)                                                                            \
+    do {                                                                                                             \
+        if (sim->st_pv == 64) k_gather_stencil<MAXT, MINB, true, 8, true, 64><<<grid, threads, sim->st_smem, sim->stream>>>(FS_STENCIL_ARGS); \
+        else k_gather_stencil<MAXT, MINB, true, 8, true, 128><<<grid, threads, sim->st_smem, sim->stream>>>(FS_STENCIL_ARGS);                  \
+    } while (0)
     // 8 outputs per thread: 72 (<= 128 threads) or 80 registers.  A 16-output variant (128 registers, half the
     // window set-ups per DFMA) was measured at 64.4 us against 63.3 us on config 5 and is not instantiated.
 #define FS_LAUNCH_STENCIL(CTV)                                                                      \
@@ -1149,8 +1159,17 @@ int do_gather_stencil(fs_sim* sim) {
                                              cudaMemcpyDeviceToDevice, sim->stream));
             CUDA_TRY(cudaMemcpyToSymbolAsync(c_rows, sim->rowtab, 8 * (size_t)g.nsub * g.nsub * g.W, 0,
                                              cudaMemcpyDeviceToDevice, sim->stream));
+            CUDA_TRY(cudaMemcpyToSymbolAsync(c_rtofs, sim->rtofs.data(), 4 * sim->rtofs.size(), 0, cudaMemcpyHostToDevice, sim->stream));
+            if (sim->st_sym) {
+                CUDA_TRY(cudaMemcpyToSymbolAsync(c_ptofs, sim->ptofs.data(), 4 * sim->ptofs.size(), 0, cudaMemcpyHostToDevice, sim->stream));
+                CUDA_TRY(cudaMemcpyToSymbolAsync(c_prow, sim->prow.data(), 16 * sim->prow.size(), 0, cudaMemcpyHostToDevice, sim->stream));
+                CUDA_TRY(cudaMemcpyToSymbolAsync(c_pstart, sim->pstart.data(), 8 * sim->pstart.size(), 0, cudaMemcpyHostToDevice, sim->stream));
+            }
             g_ct_owner = sim->st_id;
         }
+        if (sim->st_sym && sim->gather_variant != FS_GATHER_STENCIL_PLAIN) {
+            if (threads <= 128) FS_LAUNCH_STENCIL_SYM(128, 5); else FS_LAUNCH_STENCIL_SYM(256, 2);
+        } else
         FS_LAUNCH_STENCIL(true);
         if (!g_ct_event) CUDA_TRY(cudaEventCreateWithFlags(&g_ct_event, cudaEventDisableTiming));
         CUDA_TRY(cudaEventRecord(g_ct_event, sim->stream));
@@ -1158,6 +1177,8 @@ int do_gather_stencil(fs_sim* sim) {
         FS_LAUNCH_STENCIL(false);
     }
 #undef FS_LAUNCH_STENCIL
+#undef FS_LAUNCH_STENCIL_SYM
+#undef FS_STENCIL_ARGS
 #undef FS_LAUNCH_STENCIL1
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
@@ -1174,13 +1195,15 @@ bool stencil_ct(const LatGrid& g) {
     return (int64_t)g.nsub * g.nsub * g.W * g.H <= CT_MAX && g.nsub * g.nsub * g.W <= CR_MAX;
 }
 
+int stencil_pu(const LatGrid& g) { return ((ST_TU + 2 * g.Ru + 3) & ~3) <= 64 ? 64 : 128; }   // shared-memory row pitch (cells)
+
 size_t stencil_smem(const LatGrid& g, int nw, int rs, int ov, int* pv_out) {
-    int TV = ov * nw, SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv;
-    int pv = (SH + 1) | 1;                                           // odd row pitch (4-byte cells): lanes -> distinct banks
+    int TV = ov * nw, SH = TV + 2 * g.Rv, pu = stencil_pu(g);
     size_t tsm = stencil_ct(g) ? 0 : 16 * (size_t)g.nsub * g.W * g.H;
     size_t tables = (tsm + 8 * (size_t)g.nsub * g.W + 128 * (size_t)TV + 15) & ~(size_t)15;
-    size_t tiles = 4 * (size_t)g.nsub * SU * pv, red = (size_t)(rs - 1) * nw * 512 * ov;
-    if (pv_out) *pv_out = pv;
+    // one spare row in front and behind: the sliding windows read one cell past the last slot of a row
+    size_t tiles = 4 * (size_t)(g.nsub * SH + 1) * pu, red = (size_t)(rs - 1) * nw * 512 * ov;
+    if (pv_out) *pv_out = pu;
     return tables + std::max(tiles, red);
 }
 
@@ -1245,6 +1268,62 @@ int lattice_fail(fs_sim* sim, int reason) {
     if (sim->st_mem) { cudaFree(sim->st_mem); sim->st_mem = nullptr; }
     if (sim->lat_mem) { cudaFree(sim->lat_mem); sim->lat_mem = nullptr; }
     cudaGetLastError();
+    return FS_OK;
+}
+
+// Inversion pairing of the stencil slots (lattice.cuh, SYM variant).  Eq. 3 is even in r_ij, so on a lattice
+// with an inversion centre on the sites of sublattice si the slot (du, dv) of the pair (si, sj) has a partner
+// (-du - cu, -dv - cv) with the same coupling.  (cu, cv) is searched in [-2, 2]^2 and accepted only if every
+// present slot has a present partner whose table entry is BIT-IDENTICAL; otherwise the plain variant stays.
+int build_inversion_pairs(fs_sim* sim, const LatGrid& g, const std::vector<unsigned long long>& own) {
+    const int nsub = g.nsub, W = g.W, H = g.H, wh = W * H;
+    std::vector<double2> T((size_t)nsub * nsub * wh);
+    CUDA_TRY(cudaMemcpyAsync(T.data(), sim->T, 16 * T.size(), cudaMemcpyDeviceToHost, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    std::vector<int4> prow; std::vector<int> ptofs; std::vector<int2> pstart((size_t)NSUB_MAX * NSUB_MAX, make_int2(0, 0));
+    auto present = [&](int pair, int du, int dv) {
+        if (du < -g.Ru || du > g.Ru || dv < -g.Rv || dv > g.Rv) return false;
+        return own[(size_t)pair * wh + (size_t)(du + g.Ru) * H + (dv + g.Rv)] != ~0ull;
+    };
+    auto entry = [&](int pair, int du, int dv) { return T[(size_t)pair * wh + (size_t)(du + g.Ru) * H + (dv + g.Rv)]; };
+    for (int pair = 0; pair < nsub * nsub; ++pair) {
+        int fcu = 0, fcv = 0; bool found = false, any = false;
+        for (int du = -g.Ru; du <= g.Ru && !any; ++du) for (int dv = -g.Rv; dv <= g.Rv; ++dv) if (present(pair, du, dv)) { any = true; break; }
+        if (!any) { pstart[pair] = make_int2((int)prow.size(), 0); continue; }
+        for (int cu = -2; cu <= 2 && !found; ++cu)
+            for (int cv = -2; cv <= 2 && !found; ++cv) {
+                bool ok = true;
+                for (int du = -g.Ru; du <= g.Ru && ok; ++du)
+                    for (int dv = -g.Rv; dv <= g.Rv && ok; ++dv) {
+                        if (!present(pair, du, dv)) continue;
+                        const int pu = -du - cu, pv = -dv - cv;
+                        if (!present(pair, pu, pv) || (pu == du && pv == dv)) { ok = false; break; }
+                        const double2 a = entry(pair, du, dv), b = entry(pair, pu, pv);
+                        ok = a.x == b.x && a.y == b.y;               // equal values (+0 == -0: the products are the same)
+                    }
+                if (ok) { fcu = cu; fcv = cv; found = true; }
+            }
+        if (!found) return FS_OK;                        // no exact pairing: plain variant
+        const int first = (int)prow.size();
+        for (int du = g.Ru; du >= -g.Ru; --du) {
+            const int pu = -du - fcu;
+            if (pu > du) continue;                       // visited from the partner row
+            // slots of row du to visit: all present ones, or (row paired with itself) those with dv > -dv - cv
+            int a = 0, b = -1; bool anyrow = false;
+            for (int dv = -g.Rv; dv <= g.Rv; ++dv)
+                if (present(pair, du, dv) && (pu != du || 2 * dv > -fcv)) { if (!anyrow) a = dv; b = dv; anyrow = true; }
+            if (!anyrow) continue;
+            // holes inside [a, b] carry zero weight and must be holes in the mirrored row as well
+            for (int dv = a; dv <= b; ++dv)
+                if (present(pair, du, dv) != present(pair, pu, -dv - fcv)) return FS_OK;
+            if (-b - fcv < -g.Rv || -a - fcv > g.Rv) return FS_OK;
+            prow.push_back(make_int4((du + g.Ru) | ((pu + g.Ru) << 16), a, b, -a - fcv));
+            ptofs.push_back(pair * wh + (du + g.Ru) * H + (a + g.Rv));
+        }
+        pstart[pair] = make_int2(first, (int)prow.size() - first);
+    }
+    if (prow.size() > (size_t)CP_MAX) return FS_OK;
+    sim->prow = prow; sim->pstart = pstart; sim->ptofs = ptofs; sim->st_sym = true;
     return FS_OK;
 }
 
@@ -1359,7 +1438,7 @@ int detect_lattice(fs_sim* sim) {
     sim->st_id = ++g_ct_next_id;
     {
         int TV = sim->st_ov * sim->st_nw;
-        g.Upa = (g.U + ST_TU - 1) / ST_TU * ST_TU + 2 * g.Ru;           // whole tiles + halo: the prologue needs no bounds tests
+        g.Upa = ((g.U + ST_TU - 1) / ST_TU * ST_TU + 2 * g.Ru + 3) & ~3;  // whole tiles + halo (16-byte rows): the prologue needs no bounds tests
         g.Vpa = (g.V + TV - 1) / TV * TV + 2 * g.Rv;
     }
     const size_t sg_bytes = 4 * (size_t)sim->R * nsub * g.Vpa * g.Upa;
@@ -1397,11 +1476,31 @@ int detect_lattice(fs_sim* sim) {
     if (flags & 4) return lattice_fail(sim, FS_LATTICE_NOT_PERIODIC);
     if ((long long)res64[2] != (long long)sim->n_inter) return lattice_fail(sim, FS_LATTICE_REACH_MISMATCH);
     if (!(sim->st_maxdev * (double)sim->K <= 2e-13 * sim->st_wmax)) return lattice_fail(sim, FS_LATTICE_WEIGHT_MISMATCH);
-    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8>, sim->st_smem));
-    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8>, sim->st_smem));
-    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, false, 8>, sim->st_smem));
-    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, false, 8>, sim->st_smem));
+    const size_t stb = 200 * 1024;                       // the planner's cap: set once for every instantiation
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, false, 64>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, false, 64>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, false, 8, false, 64>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, false, 8, false, 64>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, false, 128>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, false, 128>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, false, 8, false, 128>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, false, 8, false, 128>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 5, true, 8, true, 64>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 2, true, 8, true, 64>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 5, true, 8, true, 128>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 2, true, 8, true, 128>, stb));
     sim->lg = g;
+    sim->st_sym = false;
+    if (sim->st_ct) {
+        std::vector<int2> rt((size_t)nsub * nsub * g.W);
+        CUDA_TRY(cudaMemcpyAsync(rt.data(), sim->rowtab, 8 * rt.size(), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        sim->rtofs.resize(rt.size());
+        for (size_t q = 0; q < rt.size(); ++q)
+            sim->rtofs[q] = (int)(q / g.W) * wh + (int)(q % g.W) * g.H + (rt[q].x + g.Rv);
+        int rc2 = build_inversion_pairs(sim, g, own);
+        if (rc2) return rc2;
+    }
     sim->stencil_ok = true; sim->stencil_reason = 0;
     // the build-only arrays (sub, cu, cv) are no longer needed
     cudaFree(sim->lat_mem); sim->lat_mem = nullptr; sim->lat_sub = nullptr; sim->lat_cu = sim->lat_cv = nullptr;
@@ -1747,8 +1846,8 @@ int fs_set_local_field(fs_sim* sim, const double* h_dev) {
 int fs_set_gather_variant(fs_sim* sim, int variant) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
     DeviceGuard guard_(sim->device);
-    if (variant < 0 || variant > 2) return fail(FS_ERR_ARG, "unknown gather variant %d", variant);
-    if (variant == FS_GATHER_STENCIL && !sim->stencil_ok)
+    if (variant < 0 || variant > 3) return fail(FS_ERR_ARG, "unknown gather variant %d", variant);
+    if ((variant == FS_GATHER_STENCIL || variant == FS_GATHER_STENCIL_PLAIN) && !sim->stencil_ok)
         return fail(FS_ERR_ARG, "stencil gather unavailable for this geometry (FS_LATTICE reason %d)", sim->stencil_reason);
     sim->gather_variant = variant;
     return FS_OK;
@@ -1759,9 +1858,10 @@ int fs_get_lattice(const fs_sim* sim, int32_t* info, double* dinfo) {
     DeviceGuard guard_(sim->device);
     if (info) {
         const LatGrid& g = sim->lg;
-        int32_t v[10] = {sim->stencil_ok ? 1 : 0, sim->stencil_reason, g.nsub, g.U, g.V, g.Ru, g.Rv,
-                         (int32_t)sim->st_slots, sim->st_nw * sim->st_rs, (int32_t)sim->st_smem};
-        for (int k = 0; k < 10; ++k) info[k] = v[k];
+        int32_t v[12] = {sim->stencil_ok ? 1 : 0, sim->stencil_reason, g.nsub, g.U, g.V, g.Ru, g.Rv,
+                         (int32_t)sim->st_slots, sim->st_nw * sim->st_rs, (int32_t)sim->st_smem,
+                         sim->stencil_ok && sim->st_sym ? 1 : 0, (int32_t)sim->prow.size()};
+        for (int k = 0; k < 12; ++k) info[k] = v[k];
     }
     if (dinfo) { dinfo[0] = sim->st_maxdev; dinfo[1] = sim->st_wmax; }
     return FS_OK;
@@ -1793,6 +1893,28 @@ int fs_measure_fp64_peak(double* dfma_per_s, void* stream) {
     *dfma_per_s = best;
     return FS_OK;
 }
+
+#ifdef FS_DEBUG_API
+// experiments only (never built into the shipped library): override the stencil kernel's CTA shape
+int fs_debug_stencil_shape(fs_sim* sim, int nw, int rs) {
+    if (!sim || !sim->stencil_ok) return -1;
+    LatGrid& g = sim->lg;
+    sim->st_nw = nw; sim->st_rs = rs;
+    sim->st_smem = stencil_smem(g, nw, rs, ST_OV, &sim->st_pv);
+    int TV = ST_OV * nw;
+    int Upa = ((g.U + ST_TU - 1) / ST_TU * ST_TU + 2 * g.Ru + 3) & ~3, Vpa = (g.V + TV - 1) / TV * TV + 2 * g.Rv;
+    if (Vpa > g.Vpa || Upa > g.Upa) return -2;          // spin grid allocation too small for this tile
+    return FS_OK;
+}
+#endif
+
+#ifdef FS_BATCH_PROFILE
+int fs_debug_batch_profile(fs_sim* sim, long long* out12) {
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpy(out12, sim->bt.ctl->prof, sizeof(long long) * 12, cudaMemcpyDeviceToHost));
+    return FS_OK;
+}
+#endif
 
 #ifdef FS_RELAX_PROFILE
 int fs_debug_relax_profile(long long* out16, int reset) {

@@ -35,7 +35,7 @@ struct LatFrame { double ox, oy, i11, i12, i21, i22; };   // (u, v) = Ainv (r - 
 
 struct LatGrid {
     int nsub, u0, v0, U, V, Ru, Rv, Up, Vp, W, H;         // W = 2Ru+1, H = 2Rv+1, Up = U+2Ru, Vp = V+2Rv
-    int Upa, Vpa;                                         // spin-grid allocation [Upa][Vpa]: whole tiles + halo, Vpa even
+    int Upa, Vpa;                                         // spin-grid allocation [Vpa][Upa] (u fastest): whole tiles + halo, Upa % 4 == 0
 };
 
 __device__ __forceinline__ void lat_uv(const LatFrame& f, double2 p, double& u, double& v) {
@@ -116,13 +116,13 @@ __device__ __forceinline__ int64_t lat_cell(const LatGrid& g, int sub, int cu, i
     return ((int64_t)sub * g.Vp + (cv - g.v0 + g.Rv)) * g.Up + (cu - g.u0 + g.Ru);
 }
 
-// flags bit 2: two spins in one cell.  cellidx[i] = position of spin i in one replica's spin grid sg[sub][Upa][Vpa].
+// flags bit 2: two spins in one cell.  cellidx[i] = position of spin i in one replica's spin grid sg[sub][Vpa][Upa].
 __global__ void k_lat_scatter(int64_t N, LatGrid g, const uint8_t* __restrict__ sub, const int* __restrict__ cu,
                               const int* __restrict__ cv, int* __restrict__ gidx, int* __restrict__ cellidx,
                               int* __restrict__ flags) {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= N) return;
-    cellidx[i] = (int)(((int64_t)sub[i] * g.Upa + (cu[i] - g.u0 + g.Ru)) * g.Vpa + (cv[i] - g.v0 + g.Rv));
+    cellidx[i] = (int)(((int64_t)sub[i] * g.Vpa + (cv[i] - g.v0 + g.Rv)) * g.Upa + (cu[i] - g.u0 + g.Ru));
     if (atomicCAS(&gidx[lat_cell(g, sub[i], cu[i], cv[i])], -1, (int)i) != -1) atomicOr(flags, 4);
 }
 
@@ -185,26 +185,18 @@ __global__ void k_stencil_count(int64_t N, LatGrid g, const uint8_t* __restrict_
     if ((threadIdx.x & 31) == 0 && n) atomicAdd(total, n);
 }
 
-// dense spin grids sg[rep][sub][Upa][Vpa] (v fastest), one sgcell_t per lattice site, rebuilt from s when
-// the spins were rewritten from outside (the relax loop keeps them in step with its own flips).  32 x 32 tiles are transposed through shared memory: gidx is read along u, sg written
-// along v, both coalesced.
+// dense spin grids sg[rep][sub][Vpa][Upa] (u fastest, like gidx), one sgcell_t per lattice site, rebuilt from s when
+// the spins were rewritten from outside (the relax loop keeps them in step with its own flips).
 __global__ void k_spin_grid(int64_t N, LatGrid g, int R, const int* __restrict__ gidx, const int8_t* __restrict__ s_all,
                             sgcell_t* __restrict__ sg) {
-    __shared__ int tile[32][33];
-    const int sub = blockIdx.z, gu0 = blockIdx.x * 32, gv0 = blockIdx.y * 32;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;           // 32 x 8 threads
-    for (int k = ty; k < 32; k += 8) {
-        int gu = gu0 + tx, gv = gv0 + k;
-        tile[k][tx] = (gu < g.Up && gv < g.Vp) ? gidx[((int64_t)sub * g.Vp + gv) * g.Up + gu] : -1;
-    }
-    __syncthreads();
-    for (int k = ty; k < 32; k += 8) {
-        int gu = gu0 + k, gv = gv0 + tx;
-        if (gu >= g.Up || gv >= g.Vp) continue;
-        int idx = tile[tx][k];
+    const int sub = blockIdx.z;
+    const int gu = blockIdx.x * 32 + (threadIdx.x & 31);
+    for (int gv = blockIdx.y * 32 + (threadIdx.x >> 5); gv < min(g.Vp, (int)(blockIdx.y + 1) * 32); gv += 8) {
+        if (gu >= g.Up) continue;
+        const int idx = gidx[((int64_t)sub * g.Vp + gv) * g.Up + gu];
         for (int r = 0; r < R; ++r) {
-            int sv = idx >= 0 ? (int)s_all[(int64_t)r * N + idx] : 0;
-            sg[(((int64_t)r * g.nsub + sub) * g.Upa + gu) * g.Vpa + gv] = (sv > 0 ? SG_UP : (sv < 0 ? SG_DOWN : 0u));
+            const int sv = idx >= 0 ? (int)s_all[(int64_t)r * N + idx] : 0;
+            sg[(((int64_t)r * g.nsub + sub) * g.Vpa + gv) * g.Upa + gu] = (sv > 0 ? SG_UP : (sv < 0 ? SG_DOWN : 0u));
         }
     }
 }
@@ -237,41 +229,60 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // k_gather_stencil: a warp-uniform weight read through the constant cache lands in a uniform register,
 // and DFMA R, R, UR, R reads only two vector-register pairs: 62 DFMA/clk/SM measured against 51 with
 // the weight in a vector register.  Re-uploaded when another simulation takes over.
-constexpr int CT_MAX = 3584;           // double2 entries (56 KB of the 64 KB constant bank)
+constexpr int CT_MAX = 2560;           // double2 entries (40 KB of the 64 KB constant bank)
 constexpr int CR_MAX = 960;            // row intervals (7.5 KB)
+constexpr int CP_MAX = 480;            // row pairs of the inversion-symmetric variant (7.5 KB)
 __constant__ double2 c_T[CT_MAX];
 __constant__ int2 c_rows[CR_MAX];
+// Inversion symmetry (Eq. 3, is even in r_ij): T[si][sj][du][dv] == T[si][sj][-du-cu][-dv-cv] for the
+// lattice's inversion offset (cu, cv) of that sublattice pair.  The SYM variant visits only one slot of every such
+// pair: x(+d) + x(-d) once (DADD), then one DFMA pair: 3 FP64 operations per 2 interactions instead of 4.
+// c_prow[e] = {row+ | row- << 16, first dv of row+, last dv of row+, offset of the mirrored window in row-};
+// c_pstart[pair] = {first entry, entries}.
+__constant__ int4 c_prow[CP_MAX];
+__constant__ int2 c_pstart[NSUB_MAX * NSUB_MAX];
+// Table offset of the first slot of every row (plain) / row pair (SYM), in arrays of their own: a value whose only
+// consumer is the index of c_T stays in the uniform datapath (LDCU -> UR -> LDCU.64 c_T[UR + imm] -> DFMA R, R, UR, R);
+// derived from a row entry that also feeds vector address arithmetic, ptxas loads it into a vector register and the
+// weights follow (LDC.64, DFMA with three vector operands: 51 instead of 62 DFMA/clk/SM).
+__constant__ int c_rtofs[CR_MAX];
+__constant__ int c_ptofs[CP_MAX];
 
-template <int MAXT, int MINB, bool CT, int OV>
+template <int MAXT, int MINB, bool CT, int OV, bool SYM, int PU>
 __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGrid g, int NW, int Pv,
                                                                const int* __restrict__ gidx, const sgcell_t* __restrict__ sg,
                                                                const double2* __restrict__ T, const int2* __restrict__ rowtab,
                                                                double2* __restrict__ hdip_all) {
     extern __shared__ __align__(16) unsigned char st_raw[];
     const int RS = (blockDim.x >> 5) / NW, TV = OV * NW;
-    const int SU = ST_TU + 2 * g.Ru, SH = TV + 2 * g.Rv, WH = g.W * g.H;
+    const int SUc = (ST_TU + 2 * g.Ru + 3) & ~3, SH = TV + 2 * g.Rv, WH = g.W * g.H;   // staged row: SUc cells, pitch PU
+    (void)Pv;
     double2* Tsm = reinterpret_cast<double2*>(st_raw);                      // [nsub][WH]
     const size_t tsm_n = CT ? 0 : (size_t)g.nsub * WH;                      // no shared copy of T in the CT variant
     int2* rows = reinterpret_cast<int2*>(Tsm + tsm_n);                      // [nsub][W]
     int* oidx = reinterpret_cast<int*>(rows + (size_t)g.nsub * g.W);        // [TV][32] spin index of every output
-    sgcell_t* S = reinterpret_cast<sgcell_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 15) & ~(size_t)15));   // [nsub][SU][Pv]
-    const int si = blockIdx.z % g.nsub, rep = blockIdx.z / g.nsub;
+    sgcell_t* S = reinterpret_cast<sgcell_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 15) & ~(size_t)15));   // [nsub][SH][PU]
+    const int si = __shfl_sync(0xffffffffu, (int)(blockIdx.z % g.nsub), 0), rep = __shfl_sync(0xffffffffu, (int)(blockIdx.z / g.nsub), 0);
     const int tu0 = blockIdx.x * ST_TU, tv0 = blockIdx.y * TV;       // tile origin, interior coordinates
     // the warp index via a shuffle from lane 0: the compiler then knows everything derived from it is
     // warp-uniform
     const int wid_u = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31, warp = wid_u % NW, rs = wid_u / NW;
 
-    // ---- prologue: everything this CTA reads, in flight at once
+    // ---- prologue: everything this CTA reads, in flight at once.  A staged row = SUc consecutive cells along u
+    // (contiguous in the spin grid and in shared memory): 16-byte cp.async, 16 or 32 lanes per row
     {
-        const sgcell_t* src = sg + (((int64_t)rep * g.nsub * g.Upa + tu0) * g.Vpa + tv0);
-        const int nwarps = blockDim.x >> 5, wid = threadIdx.x >> 5;
-        for (int sj = 0; sj < g.nsub; ++sj)
-            for (int ul = wid; ul < SU; ul += nwarps) {            // one tile row per warp: no index divisions
-                sgcell_t* drow = S + ((size_t)sj * SU + ul) * Pv;
-                const sgcell_t* srow = src + ((int64_t)sj * g.Upa + ul) * g.Vpa;
-                for (int c = lane; c < SH; c += 32) cp_async4(drow + c, srow + c);
+        const sgcell_t* src = sg + (((int64_t)rep * g.nsub * g.Vpa + tv0) * g.Upa + tu0);
+        constexpr int CPR = PU / 4;                                   // 16-byte chunks per shared-memory row
+        const int nch = SUc >> 2;
+        for (int sj = 0; sj < g.nsub; ++sj) {
+            sgcell_t* dst = S + (size_t)sj * SH * PU;
+            const sgcell_t* srcj = src + (int64_t)sj * g.Vpa * g.Upa;
+            for (int t = threadIdx.x; t < SH * CPR; t += blockDim.x) {
+                const int vl = t / CPR, ch = t % CPR;                 // CPR is a power of two
+                if (ch < nch) cp_async16(dst + (size_t)vl * PU + 4 * ch, srcj + (int64_t)vl * g.Upa + 4 * ch);
             }
+        }
     }
     if (!CT)
         for (int t = threadIdx.x; t < g.nsub * WH; t += blockDim.x) cp_async16(Tsm + t, T + (int64_t)si * g.nsub * WH + t);
@@ -287,10 +298,59 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     double ax[OV], ay[OV], x[OV];                      // all indices below are compile-time after unrolling: registers
 #pragma unroll
     for (int q = 0; q < OV; ++q) { ax[q] = 0.0; ay[q] = 0.0; }
-#define FS_ST_LD(K) __hiloint2double((int)sp[K], 0)
+#define FS_ST_LD(K) __hiloint2double((int)sp[(K) * PU], 0)
+#define FS_ST_LDM(K) __hiloint2double((int)sm[(K) * PU], 0)
 
+    if (SYM) {
+        // one slot of every inversion pair: window x slides forward along row+, window y backward along row-
+        double y[OV];
+        for (int sj = 0; sj < g.nsub; ++sj) {
+            const sgcell_t* Sj = S + ((size_t)sj * SH + warp * OV + g.Rv) * PU + lane;
+            const int2 ps = c_pstart[si * g.nsub + sj];
+            for (int e = 0; e < ps.y; ++e) {
+                if ((e & (RS - 1)) != rs) continue;
+                const int4 pr = c_prow[ps.x + e];
+                const int rp = pr.x & 0xffff, rm = pr.x >> 16;
+                int n = pr.z - pr.y + 1;
+                const sgcell_t* sp = Sj + rp + pr.y * PU;              // x[q] = S[.. + q + dv][lane + row+]
+                const sgcell_t* sm = Sj + rm + pr.w * PU;              // y[q] = S[.. + q - dv - cv][lane + row-]
+                int tofs = c_ptofs[ps.x + e];
+#pragma unroll
+                for (int q = 0; q < OV; ++q) { x[q] = FS_ST_LD(q); y[q] = FS_ST_LDM(q); }
+                for (; n >= OV; n -= OV, sp += OV * PU, sm -= OV * PU, tofs += OV) {
+#pragma unroll
+                    for (int K = 0; K < OV; ++K) {
+                        const double2 t = c_T[tofs + K];
+#pragma unroll
+                        for (int q = 0; q < OV; ++q) {
+                            const double z = x[(q + K) % OV] + y[(q - K + OV) % OV];
+                            ax[q] = fma(z, t.x, ax[q]);
+                            ay[q] = fma(z, t.y, ay[q]);
+                        }
+                        x[K] = FS_ST_LD(OV + K);
+                        y[OV - 1 - K] = FS_ST_LDM(-(K + 1));
+                    }
+                }
+                if (n > 0) {
+#pragma unroll
+                    for (int K = 0; K < OV - 1; ++K) {
+                        const double2 t = c_T[tofs + K];
+#pragma unroll
+                        for (int q = 0; q < OV; ++q) {
+                            const double z = x[(q + K) % OV] + y[(q - K + OV) % OV];
+                            ax[q] = fma(z, t.x, ax[q]);
+                            ay[q] = fma(z, t.y, ay[q]);
+                        }
+                        if (--n == 0) break;
+                        x[K] = FS_ST_LD(OV + K);
+                        y[OV - 1 - K] = FS_ST_LDM(-(K + 1));
+                    }
+                }
+            }
+        }
+    } else
     for (int sj = 0; sj < g.nsub; ++sj) {
-        const sgcell_t* Sj = S + ((size_t)sj * SU + lane) * Pv + warp * OV + g.Rv;
+        const sgcell_t* Sj = S + ((size_t)sj * SH + warp * OV + g.Rv) * PU + lane;
         const double2* Tj = Tsm + (CT ? 0 : (size_t)sj * WH + g.Rv);
         const int tj = (si * g.nsub + sj) * WH + g.Rv;
         // r = du + Ru is a uniform loop counter, so that the row interval and the weight offsets below live
@@ -300,14 +360,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
             const int2 rt = CT ? c_rows[(si * g.nsub + sj) * g.W + r] : rows[sj * g.W + r];
             int n = rt.y - rt.x + 1;
             if (n <= 0) continue;
-            // output (lane, warp*OV+q) at slot (du, dv) reads S[sj][lane + du + Ru][warp*OV + q + dv + Rv]
-            const sgcell_t* sp = Sj + (size_t)r * Pv + rt.x;
+            // output (lane, warp*OV+q) at slot (du, dv) reads S[sj][warp*OV + q + dv + Rv][lane + du + Ru]
+            const sgcell_t* sp = Sj + r + rt.x * PU;
             const double2* tp = Tj + (CT ? 0 : r * g.H + rt.x);
-            int tofs = tj + r * g.H + rt.x;
+            int tofs = CT ? c_rtofs[(si * g.nsub + sj) * g.W + r] : tj + r * g.H + rt.x;
 #pragma unroll
             for (int q = 0; q < OV; ++q) x[q] = FS_ST_LD(q);
             // full groups of OV slots (no exit test): slot K consumes the window and refills its oldest cell
-            for (; n >= OV; n -= OV, sp += OV, tp += OV, tofs += OV) {
+            for (; n >= OV; n -= OV, sp += OV * PU, tp += OV, tofs += OV) {
 #pragma unroll
                 for (int K = 0; K < OV; ++K) {
                     const double2 t = CT ? c_T[tofs + K] : tp[K];
@@ -335,6 +395,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
         }
     }
 #undef FS_ST_LD
+#undef FS_ST_LDM
     // ---- epilogue: add the row groups' partial sums (fixed order), scatter the OV outputs to their spins
     if (RS > 1) {
         __syncthreads();                               // everyone is done with the tiles
