@@ -182,7 +182,7 @@ int fs_get_batch_stats(fs_sim* sim, int64_t* out4);
  * multi-kernel path scans faster.  fields_dev DEVICE [T,2] (hx,hy), shared by all replicas;
  * flips_per_step_dev DEVICE [R,T] int64 or NULL; max_flips <= 0: unlimited (cap on the whole sweep);
  * n_flips_out HOST [R] (total flips of the sweep) or NULL = asynchronous.  The flip log
- * (fs_get_flip_log) then holds the flips of the whole sweep in order (first 4N+1024).
+ * (fs_get_flip_log) then holds the flips of the whole sweep in order (the last 4N+1024 of them).
  * If the cap stops a replica inside the protocol (FS_ERR_MAXFLIPS, reported only with n_flips_out != NULL) its
  * state is that of the step it reached: the global field is fields[that step], flips_per_step of the steps
  * never run is 0, and the thermal step key used by fs_get_fields becomes step0 + (the step replica 0 reached). */
@@ -196,6 +196,30 @@ int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, i
 int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_dev, int32_t T, uint32_t step0,
                     int64_t* flips_per_step_dev, int64_t max_flips, int64_t* n_flips_out);
 
+/* fs_sweep with time-dependent per-spin fields ("h_ext is a discrete time series of either local,
+ * global or spatial fields"): at step t the external field of spin i is
+ *     h_ext^(i)(t) = fields[t] + local_scale[t] * local_i + local_series[t][i]        (global x,y components)
+ * local_i = the static per-spin field of fs_set_local_field (its scale defaults to 1), local_scale_dev DEVICE [T] or
+ * NULL, local_series_dev DEVICE [T,N,2] or NULL (shared by all replicas), sigma_dev as fs_sweep_anneal.  Rounded as
+ * written: (scale * local) + series, then added to the global field, then rotated (reading D-4).
+ * After the call fs_get_fields(EXT/TOTAL) uses the static local field only. */
+int fs_sweep_ex(fs_sim* sim, const double* fields_dev, const double* sigma_dev, const double* local_scale_dev,
+                const double* local_series_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
+                int64_t max_flips, int64_t* n_flips_out);
+
+/* Analysis reductions of the current spin state (PAPER.md:204-206 section IV.B; :160 "analysis of vertex populations").
+ * fs_correlation: spin-spin correlation by separation.  c_ij = +1 (-1) if the dipole interaction of the pair is
+ * minimised (maximised): sign of s_i s_j g_par,ij; pairs whose parallel coupling vanishes (|g_par| d^3 < 1e-9) are
+ * skipped.  Every unordered pair of the neighbourhood once, bin = floor(|r_ij| / bin_width), pairs beyond nbins
+ * (<= 2048) dropped.  sum_dev DEVICE [R,nbins] int64 = sum of c_ij per replica, count_dev DEVICE [nbins] int64 =
+ * pairs per bin (geometry only); the correlation at a separation is sum / count (average over replicas for an
+ * ensemble).  Asynchronous.
+ * fs_vertex_populations: vertices_dev DEVICE [V,4] int32 = the four spins meeting at each vertex (square / pinwheel
+ * ASI); counts_dev DEVICE [R,4] int64 = number of Type I, II, III, IV vertices: moments pointing into the vertex
+ * 0 or 4 -> IV, 1 or 3 -> III, 2 -> I if they are opposite (zero net moment), II if adjacent. */
+int fs_correlation(fs_sim* sim, double bin_width, int32_t nbins, int64_t* sum_dev, int64_t* count_dev);
+int fs_vertex_populations(fs_sim* sim, const int32_t* vertices_dev, int64_t V, int64_t* counts_dev);
+
 /* Counters accumulated on the device since creation / the last reset: HOST [R] each (any may be
  * NULL).  Synchronises. */
 int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips, int reset);
@@ -203,10 +227,14 @@ int fs_get_counters(fs_sim* sim, int64_t* total_flips, int64_t* last_relax_flips
 /* h_dev_out DEVICE [R,N,2] (par, perp) in the fixed theta_i frame; `which` = FS_FIELD_*. */
 int fs_get_fields(fs_sim* sim, int which, double* h_dev_out);
 
-/* Flip log of the last fs_relax of replica `replica`: idx_dev_out DEVICE [cap] int32 in flip order;
- * n_out HOST = number of flips of that relax (may exceed what was logged: the internal log holds
- * 4N+1024 entries).  Synchronises. */
+/* Flip log of the last fs_relax / fs_sweep of replica `replica`: idx_dev_out DEVICE [cap] int32 in flip order;
+ * n_out HOST = number of flips of that call.  The internal log is a ring of 4N+1024 entries: when a long sweep
+ * (many field periods) makes more flips than that, the LAST 4N+1024 are kept.  The output starts at the oldest
+ * flip still held, number *first_out (HOST, may be NULL; 0 unless the ring wrapped), and holds
+ * min(cap, n - first) entries.  fs_get_flip_log is the same without first_out.  Synchronises. */
 int fs_get_flip_log(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out);
+int fs_get_flip_log_window(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out,
+                           int64_t* first_out);
 
 /* Neighbour table: idx_dev_out DEVICE [N,K] row-major int32, ascending, -1 padded; K_out HOST. */
 int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out);

@@ -24,7 +24,7 @@ EXPORTS = [
     "fs_update_fields", "fs_scan", "fs_scan_ensemble", "fs_relax", "fs_relax_ensemble", "fs_get_counters",
     "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
     "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep", "fs_sweep_anneal", "fs_set_local_field",
-    "fs_set_batch", "fs_get_batch_stats",
+    "fs_set_batch", "fs_get_batch_stats", "fs_sweep_ex", "fs_correlation", "fs_vertex_populations", "fs_get_flip_log_window",
 ]
 
 
@@ -81,6 +81,10 @@ def load_library(path: str | None = None):
         "fs_sweep_anneal": [vp, vp, vp, i32, C.c_uint32, vp, i64, vp],
         "fs_measure_fp64_peak": [P(dbl), vp],
         "fs_set_batch": [vp, i32, i32],
+        "fs_sweep_ex": [vp, vp, vp, vp, vp, i32, C.c_uint32, vp, i64, vp],
+        "fs_correlation": [vp, dbl, i32, vp, vp],
+        "fs_vertex_populations": [vp, vp, i64, vp],
+        "fs_get_flip_log_window": [vp, i32, vp, i64, P(i64), P(i64)],
         "fs_get_batch_stats": [vp, vp],
     }
     for name, args in sig.items():
@@ -239,21 +243,43 @@ class Sim:
         _check(self.L, self.L.fs_relax(self.h, int(max_flips), C.byref(n)), allow=(FS_ERR_MAXFLIPS,))
         return int(n.value)
 
-    def sweep(self, fields, step0=0, per_step=True, max_flips=0, sync=True, sigma=None):
-        """Whole protocol in one launch.  fields [T,2]; sigma [T] = thermal std per step (annealing) or None.
+    def sweep(self, fields, step0=0, per_step=True, max_flips=0, sync=True, sigma=None, local_scale=None, local_series=None):
+        """Whole protocol in one launch.  fields [T,2]; sigma [T] = thermal std per step (annealing) or None;
+        local_scale [T] scales the static per-spin field per step, local_series [T,N,2] adds a per-spin field per step.
         Returns (flips per replica [R] or None if not sync, flips per step tensor [R,T] on the device or None)."""
-        f = torch.as_tensor(np.ascontiguousarray(fields, np.float64)).to(self.device)
+        def dev(a):
+            return None if a is None else torch.as_tensor(np.ascontiguousarray(a, np.float64)).to(self.device)
+        f = dev(fields)
         T = int(f.shape[0])
-        sg = None if sigma is None else torch.as_tensor(np.ascontiguousarray(sigma, np.float64)).to(self.device)
+        sg, ls, lser = dev(sigma), dev(local_scale), dev(local_series)
         assert sg is None or sg.numel() == T
+        assert ls is None or ls.numel() == T
+        assert lser is None or tuple(lser.shape) == (T, self.N, 2)
         ps = torch.zeros((self.R, T), dtype=torch.int64, device=self.device) if per_step else None
         n = np.zeros(self.R, np.int64)
-        _check(self.L, self.L.fs_sweep_anneal(self.h, f.data_ptr(), None if sg is None else sg.data_ptr(), T, int(step0),
-                                              ps.data_ptr() if per_step else None, int(max_flips),
-                                              n.ctypes.data if sync else None), allow=(FS_ERR_MAXFLIPS,))
+        ptr = lambda t: None if t is None else t.data_ptr()
+        _check(self.L, self.L.fs_sweep_ex(self.h, f.data_ptr(), ptr(sg), ptr(ls), ptr(lser), T, int(step0),
+                                          ps.data_ptr() if per_step else None, int(max_flips),
+                                          n.ctypes.data if sync else None), allow=(FS_ERR_MAXFLIPS,))
         if not sync:
-            self._keep = (f, sg)                           # the kernel reads them asynchronously
+            self._keep = (f, sg, ls, lser)                 # the kernel reads them asynchronously
         return (n if sync else None), ps
+
+    def correlation(self, bin_width, nbins):
+        """Spin-spin correlation by separation: (sum of c_ij [R,nbins] or [nbins], pairs per bin [nbins])."""
+        sm = torch.zeros((self.R, int(nbins)), dtype=torch.int64, device=self.device)
+        cnt = torch.zeros(int(nbins), dtype=torch.int64, device=self.device)
+        _check(self.L, self.L.fs_correlation(self.h, float(bin_width), int(nbins), sm.data_ptr(), cnt.data_ptr()))
+        return (sm if self.R > 1 else sm[0]), cnt
+
+    def vertex_populations(self, vertices):
+        """Counts of Type I..IV vertices ([R,4] or [4]); vertices [V,4] spin indices."""
+        v = torch.as_tensor(np.ascontiguousarray(vertices, np.int32)).to(self.device)
+        assert v.dim() == 2 and v.shape[1] == 4
+        out = torch.zeros((self.R, 4), dtype=torch.int64, device=self.device)
+        _check(self.L, self.L.fs_vertex_populations(self.h, v.data_ptr(), int(v.shape[0]), out.data_ptr()))
+        self.stream.synchronize()                          # `v` may be a temporary
+        return out if self.R > 1 else out[0]
 
     def relax_ensemble(self, max_flips=0):
         n = np.zeros(self.R, np.int64)
@@ -275,9 +301,10 @@ class Sim:
         cap = int(cap if cap is not None else 4 * self.N + 1024)
         out = torch.empty(cap, dtype=torch.int32, device=self.device)
         n = C.c_int64()
-        _check(self.L, self.L.fs_get_flip_log(self.h, int(replica), out.data_ptr(), cap, C.byref(n)))
-        self.last_log_count = int(n.value)
-        return out[:min(int(n.value), cap)]
+        first = C.c_int64()
+        _check(self.L, self.L.fs_get_flip_log_window(self.h, int(replica), out.data_ptr(), cap, C.byref(n), C.byref(first)))
+        self.last_log_count = int(n.value); self.last_log_first = int(first.value)
+        return out[:min(int(n.value) - int(first.value), cap)]
 
     def get_neighbors(self) -> torch.Tensor:
         out = torch.empty((self.N, max(self.K, 1)), dtype=torch.int32, device=self.device)

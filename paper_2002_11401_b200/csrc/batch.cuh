@@ -491,7 +491,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 rank += (o.nev < me.nev || (o.nev == me.nev && o.lo < me.lo)) ? 1 : 0;
             }
             rank = __reduce_add_sync(0xffffffffu, rank);
-            if (lane == 0 && nflips + rank < a.log_cap) a.flog[nflips + rank] = me.k;
+            if (lane == 0) a.flog[(nflips + rank) % a.log_cap] = me.k;       // ring buffer, like k_relax
         }
         BT_PROF(8);
         nflips += nc;

@@ -67,7 +67,6 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 // The dynamic shared-memory limit is an attribute of the kernel function (per device), not of a simulation:
 // it is only ever raised, so that simulations of different sizes can coexist in one process.
-constexpr int MAX_DEVICES = 64;
 std::mutex g_smem_mutex;
 std::map<std::pair<const void*, int>, size_t> g_smem_limit;   // (kernel, device) -> limit set so far
 template <typename F>
@@ -662,6 +661,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         long long* __restrict__ flips_per_step /*[R,T] or NULL*/, double2* __restrict__ hext_all,
         const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/,
         const double* __restrict__ sweep_sigma /*[T] thermal std per step (annealing) or NULL*/,
+        const double* __restrict__ sweep_lscale /*[T] scale of the static per-spin field per step or NULL*/,
+        const double2* __restrict__ sweep_lseries /*[T,N] per-spin field per step or NULL*/,
         int use_base /*continue the flip count and log of k_relax_batch (ctr[r].batch_flips)*/) {
     // four-level arg-max hierarchy in shared memory:
     // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
@@ -711,8 +712,23 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             for (int q = lane; q < LB; q += 32) {
                 const int64_t i = ((int64_t)b << LBshift) + q;
                 if (i < N) {
+                    // h_ext^(i)(t) = global(t) + scale(t) * local_i + series(t, i)   (reading D-4)
                     double2 hei = he;
-                    if (hloc) { const double2 l = hloc[i]; hei = make_double2(he.x + l.x, he.y + l.y); }
+                    {
+                        double lx = 0.0, ly = 0.0; bool anyl = false;
+                        if (hloc) {
+                            const double2 l = hloc[i];
+                            if (sweep_lscale) { const double sc = sweep_lscale[st]; lx = __dmul_rn(sc, l.x); ly = __dmul_rn(sc, l.y); }
+                            else { lx = l.x; ly = l.y; }
+                            anyl = true;
+                        }
+                        if (sweep_lseries) {
+                            const double2 l2 = sweep_lseries[(int64_t)st * N + i];
+                            lx = anyl ? __dadd_rn(lx, l2.x) : l2.x; ly = anyl ? __dadd_rn(ly, l2.y) : l2.y;
+                            anyl = true;
+                        }
+                        if (anyl) hei = make_double2(he.x + lx, he.y + ly);
+                    }
                     const double2 hf = fixed_field(cs[i], hei, f2, r, (uint32_t)i);
                     hfix[i] = hf;
                     const double2 hd = hdip[i];
@@ -843,7 +859,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         if (sh_stop) { status = sh_stop - 1; break; }
         if (tid == 0) {
             s[sh_k] = (int8_t)(-sh_sold);
-            if (nflips < log_cap) flog[nflips] = sh_k;
+            flog[nflips % log_cap] = sh_k;                       // ring buffer: the last log_cap flips are kept
         }
         if (tid == RELAX_THREADS - 32 && cellidx)           // keep the stencil gather's spin grid in step (an idle warp)
             sgrid[(int64_t)r * sgrid_stride + cellidx[sh_k]] = (sh_sold > 0 ? SG_DOWN : SG_UP);
@@ -927,6 +943,85 @@ __global__ void k_fields_out(int64_t N, int which, FieldSpec fs, const double2* 
     else if (which == FS_FIELD_THERMAL) o = t;
     else o = make_double2(d.x + e.x + t.x, d.y + e.y + t.y);
     out_all[(int64_t)r * N + i] = o;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Analysis reductions of a (usually annealed) state.
+// ------------------------------------------------------------------------------------------------
+// Spin-spin correlation: "the correlation of two spins is defined as +1 (-1) if their dipole interaction is
+// minimized (maximized)", as a function of their separation.  The pair energy is -s_i s_j g_par,ij (Eq. 3), so
+// c_ij = sign(s_i s_j g_par,ij); pairs with |g_par| d^3 < 1e-9 (no parallel coupling) are skipped (reading D-5).
+// Every unordered neighbour pair once; bin = floor(d / bin_width) from IEEE operations without contraction, so the
+// integer bins equal the oracle's.  blockIdx.y = replica; counts by replica 0 only.
+constexpr int CORR_MAX_BINS = 2048;
+__global__ void __launch_bounds__(256) k_correlation(int64_t N, int Kp, double bin_width, int nbins, const double2* __restrict__ pos,
+                                                     const double2* __restrict__ cs, const int* __restrict__ nbr,
+                                                     const int8_t* __restrict__ s_all, long long* __restrict__ sum_all,
+                                                     long long* __restrict__ count) {
+    __shared__ int sh_sum[CORR_MAX_BINS];
+    __shared__ int sh_cnt[CORR_MAX_BINS];
+    const int r = blockIdx.y;
+    const int8_t* s = s_all + (int64_t)r * N;
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) { sh_sum[b] = 0; sh_cnt[b] = 0; }
+    __syncthreads();
+    const int64_t total = N * (int64_t)Kp;
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = t / Kp;
+        const int j = nbr[t];
+        if (j <= (int)i) continue;                       // padding (-1) and the mirrored entry
+        const double2 pi = pos[i], pj = pos[j];
+        const double dx = pi.x - pj.x, dy = pi.y - pj.y;
+        const double d = __dsqrt_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)));
+        const double fb = floor(__ddiv_rn(d, bin_width));
+        if (!(fb < (double)nbins)) continue;
+        const double2 g = coupling(pi, cs[i], pj, cs[j], 1.0);
+        if (fabs(g.x) * (d * d * d) < 1e-9) continue;
+        const int c = ((double)s[i] * (double)s[j] * g.x > 0.0) ? 1 : -1;
+        atomicAdd(&sh_sum[(int)fb], c);
+        if (r == 0) atomicAdd(&sh_cnt[(int)fb], 1);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) {
+        if (sh_sum[b]) atomicAdd((unsigned long long*)&sum_all[(int64_t)r * nbins + b], (unsigned long long)(long long)sh_sum[b]);
+        if (r == 0 && sh_cnt[b]) atomicAdd((unsigned long long*)&count[b], (unsigned long long)sh_cnt[b]);
+    }
+}
+
+// Vertex populations: a vertex = four magnets around a point (square / pinwheel ASI).  A moment points into the
+// vertex if m_i . (r_v - r_i) > 0, r_v = mean position.  0 or 4 in: Type IV; 1 or 3: Type III; 2: Type I if the
+// two in-pointing magnets are opposite (net moment zero), Type II if adjacent (reading D-6).
+__global__ void k_vertex_populations(int64_t N, int64_t V, const int* __restrict__ vert, const double2* __restrict__ pos,
+                                     const double2* __restrict__ cs, const int8_t* __restrict__ s_all,
+                                     long long* __restrict__ counts_all) {
+    __shared__ int sh[4];
+    const int r = blockIdx.y;
+    const int8_t* s = s_all + (int64_t)r * N;
+    if (threadIdx.x < 4) sh[threadIdx.x] = 0;
+    __syncthreads();
+    for (int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; v < V; v += (int64_t)gridDim.x * blockDim.x) {
+        int q[4]; double2 p[4];
+        double vx = 0.0, vy = 0.0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { q[a] = vert[4 * v + a]; p[a] = pos[q[a]]; vx += p[a].x; vy += p[a].y; }
+        vx *= 0.25; vy *= 0.25;
+        int nin = 0; double inx = 0.0, iny = 0.0; bool first = true, opposite = false;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const double rx = vx - p[a].x, ry = vy - p[a].y;
+            const double2 c = cs[q[a]];
+            const double si = (double)s[q[a]];
+            if (si * c.x * rx + si * c.y * ry > 0.0) {
+                ++nin;
+                if (first) { inx = rx; iny = ry; first = false; }
+                else opposite = (inx * rx + iny * ry) < 0.0;
+            }
+        }
+        const int type = (nin == 0 || nin == 4) ? 3 : ((nin == 1 || nin == 3) ? 2 : (opposite ? 0 : 1));
+        atomicAdd(&sh[type], 1);
+    }
+    __syncthreads();
+    if (threadIdx.x < 4 && sh[threadIdx.x])
+        atomicAdd((unsigned long long*)&counts_all[(int64_t)r * 4 + threadIdx.x], (unsigned long long)sh[threadIdx.x]);
 }
 
 __global__ void k_set_field(int R, double hx, double hy, double2* hext) {
@@ -1151,8 +1246,8 @@ int do_gather_stencil(fs_sim* sim) {
     if (sim->st_ct) {
         // the constant-memory table is shared by all simulations of the process: take it over if needed
         std::lock_guard<std::mutex> lock(g_ct_mutex);
-        unsigned long long& g_ct_owner = g_ct_owner_dev[sim->device];
-        cudaEvent_t& g_ct_event = g_ct_event_dev[sim->device];
+        unsigned long long& g_ct_owner = g_ct_owner_dev[sim->device & 63];
+        cudaEvent_t& g_ct_event = g_ct_event_dev[sim->device & 63];
         if (g_ct_owner != sim->st_id) {
             if (g_ct_event) CUDA_TRY(cudaStreamWaitEvent(sim->stream, g_ct_event, 0));   // previous owner's kernels first
             CUDA_TRY(cudaMemcpyToSymbolAsync(c_T, sim->T, 16 * (size_t)g.nsub * g.nsub * g.W * g.H, 0,
@@ -1536,7 +1631,8 @@ int fetch_counters(fs_sim* sim) {
 
 // T == 0: relax at the field set by fs_set_field (k_scan first); T > 0: whole protocol in one launch
 int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_dev, uint32_t step0, long long* per_step_dev,
-                 const double* sigma_dev = nullptr, int use_base = 0) {
+                 const double* sigma_dev = nullptr, int use_base = 0, const double* lscale_dev = nullptr,
+                 const double2* lseries_dev = nullptr) {
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
     FieldSpec fsp{sim->sigma, sim->seed, T > 0 ? step0 : sim->step};
     // ensembles of small systems: when there are more replicas than SMs and the whole update fits one warp,
@@ -1547,7 +1643,7 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr, \
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid, \
         sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0, \
-        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev, use_base
+        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev, lscale_dev, lseries_dev, use_base
     if (small_cta && sim->R > 8 * sim->sm_count) k_relax<64><<<sim->R, 64, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else if (small_cta) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else if (sim->Kp + 1 > 512) k_relax<1024><<<sim->R, 1024, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
@@ -2014,15 +2110,17 @@ int fs_relax(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out) {
     return capped ? fail(FS_ERR_MAXFLIPS, "relax stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
 }
 
-int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_dev, int32_t T, uint32_t step0,
-                    int64_t* flips_per_step_dev, int64_t max_flips, int64_t* n_flips_out) {
+int fs_sweep_ex(fs_sim* sim, const double* fields_dev, const double* sigma_dev, const double* local_scale_dev,
+                const double* local_series_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev, int64_t max_flips,
+                int64_t* n_flips_out) {
     if (!sim || !fields_dev) return fail(FS_ERR_ARG, "null pointer");
     DeviceGuard guard_(sim->device);
     if (T <= 0) return fail(FS_ERR_ARG, "T=%d must be positive", (int)T);
     int rc = ensure_fields(sim);
     if (rc) return rc;
     rc = launch_relax(sim, max_flips, T, reinterpret_cast<const double2*>(fields_dev), step0,
-                      reinterpret_cast<long long*>(flips_per_step_dev), sigma_dev);
+                      reinterpret_cast<long long*>(flips_per_step_dev), sigma_dev, 0, local_scale_dev,
+                      reinterpret_cast<const double2*>(local_series_dev));
     if (rc) return rc;
     sim->step = step0 + (uint32_t)(T - 1);
     if (!n_flips_out) return FS_OK;
@@ -2032,6 +2130,11 @@ int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_d
     for (int r = 0; r < sim->R; ++r) { n_flips_out[r] = sim->ctr_host[r].last_flips; capped |= sim->ctr_host[r].status; }
     if (capped) sim->step = step0 + (uint32_t)sim->ctr_host[0].last_step;      // replica 0's last step (see flatspin.h)
     return capped ? fail(FS_ERR_MAXFLIPS, "sweep stopped at max_flips=%lld", (long long)max_flips) : FS_OK;
+}
+
+int fs_sweep_anneal(fs_sim* sim, const double* fields_dev, const double* sigma_dev, int32_t T, uint32_t step0,
+                    int64_t* flips_per_step_dev, int64_t max_flips, int64_t* n_flips_out) {
+    return fs_sweep_ex(sim, fields_dev, sigma_dev, nullptr, nullptr, T, step0, flips_per_step_dev, max_flips, n_flips_out);
 }
 
 int fs_sweep(fs_sim* sim, const double* fields_dev, int32_t T, uint32_t step0, int64_t* flips_per_step_dev,
@@ -2065,21 +2168,30 @@ int fs_get_fields(fs_sim* sim, int which, double* h_dev_out) {
     return FS_OK;
 }
 
-int fs_get_flip_log(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out) {
+int fs_get_flip_log_window(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out, int64_t* first_out) {
     if (!sim || !n_out) return fail(FS_ERR_ARG, "null pointer");
     DeviceGuard guard_(sim->device);
     if (replica < 0 || replica >= sim->R) return fail(FS_ERR_ARG, "replica out of range");
     int rc = fetch_counters(sim);
     if (rc) return rc;
-    int64_t n = sim->ctr_host[replica].last_flips;
+    const int64_t n = sim->ctr_host[replica].last_flips, L = sim->log_cap;
+    const int64_t first = std::max<int64_t>(0, n - L);           // oldest flip still in the ring
     *n_out = n;
-    int64_t ncopy = std::min(std::min(n, cap), sim->log_cap);
+    if (first_out) *first_out = first;
+    const int64_t ncopy = std::min(cap, n - first);
     if (ncopy > 0) {
         if (!idx_dev_out) return fail(FS_ERR_ARG, "null output buffer");
-        CUDA_TRY(cudaMemcpyAsync(idx_dev_out, sim->flog + (int64_t)replica * sim->log_cap, 4 * (size_t)ncopy,
-                                 cudaMemcpyDeviceToDevice, sim->stream));
+        const int32_t* base = sim->flog + (int64_t)replica * L;
+        const int64_t p0 = first % L, n1 = std::min(ncopy, L - p0);          // flip number q sits at q % L
+        CUDA_TRY(cudaMemcpyAsync(idx_dev_out, base + p0, 4 * (size_t)n1, cudaMemcpyDeviceToDevice, sim->stream));
+        if (ncopy > n1)
+            CUDA_TRY(cudaMemcpyAsync(idx_dev_out + n1, base, 4 * (size_t)(ncopy - n1), cudaMemcpyDeviceToDevice, sim->stream));
     }
     return FS_OK;
+}
+
+int fs_get_flip_log(fs_sim* sim, int32_t replica, int32_t* idx_dev_out, int64_t cap, int64_t* n_out) {
+    return fs_get_flip_log_window(sim, replica, idx_dev_out, cap, n_out, nullptr);
 }
 
 int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out) {
@@ -2089,6 +2201,36 @@ int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out) {
     if (idx_dev_out && sim->K > 0)
         CUDA_TRY(cudaMemcpy2DAsync(idx_dev_out, 4 * (size_t)sim->K, sim->nbr, 4 * (size_t)sim->Kp, 4 * (size_t)sim->K,
                                    (size_t)sim->N, cudaMemcpyDeviceToDevice, sim->stream));
+    return FS_OK;
+}
+
+int fs_correlation(fs_sim* sim, double bin_width, int32_t nbins, int64_t* sum_dev, int64_t* count_dev) {
+    if (!sim || !sum_dev || !count_dev) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
+    if (!(bin_width > 0.0) || nbins <= 0 || nbins > CORR_MAX_BINS) return fail(FS_ERR_ARG, "bin_width must be > 0 and 0 < nbins <= %d", CORR_MAX_BINS);
+    CUDA_TRY(cudaMemsetAsync(sum_dev, 0, 8 * (size_t)sim->R * nbins, sim->stream));
+    CUDA_TRY(cudaMemsetAsync(count_dev, 0, 8 * (size_t)nbins, sim->stream));
+    if (sim->K == 0) return FS_OK;
+    const int64_t total = sim->N * (int64_t)sim->Kp;
+    const unsigned nb = (unsigned)std::min<int64_t>((total + 255) / 256, (int64_t)sim->sm_count * 8);
+    k_correlation<<<dim3(nb, (unsigned)sim->R), 256, 0, sim->stream>>>(sim->N, sim->Kp, bin_width, nbins, sim->pos, sim->cs, sim->nbr,
+                                                                          sim->s, (long long*)sum_dev, (long long*)count_dev);
+    LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    return FS_OK;
+}
+
+int fs_vertex_populations(fs_sim* sim, const int32_t* vertices_dev, int64_t V, int64_t* counts_dev) {
+    if (!sim || !counts_dev || (V > 0 && !vertices_dev)) return fail(FS_ERR_ARG, "null pointer");
+    DeviceGuard guard_(sim->device);
+    if (V < 0) return fail(FS_ERR_ARG, "V must be >= 0");
+    CUDA_TRY(cudaMemsetAsync(counts_dev, 0, 8 * (size_t)sim->R * 4, sim->stream));
+    if (V == 0) return FS_OK;
+    const unsigned nb = (unsigned)std::min<int64_t>((V + 255) / 256, (int64_t)sim->sm_count * 8);
+    k_vertex_populations<<<dim3(nb, (unsigned)sim->R), 256, 0, sim->stream>>>(sim->N, V, vertices_dev, sim->pos, sim->cs, sim->s,
+                                                                                 (long long*)counts_dev);
+    LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
     return FS_OK;
 }
 

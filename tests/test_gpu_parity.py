@@ -863,3 +863,171 @@ def test_batched_equals_sequential_config4_full_size(B):
     assert np.array_equal(logs["batch"][0], logs["seq"][0]) and np.array_equal(logs["batch"][1], logs["seq"][1])
     st = logs["batch"][2]
     assert st["flips"] > 1_900_000 and st["flips"] / st["rounds"] > 100, st
+
+
+# ------------------------------------------------------------------ f2: time-dependent protocols, local field series
+def _oracle_protocol(orc, fields, local=None):
+    counts, logs = [], []
+    for t, (hx, hy) in enumerate(fields):
+        if local is not None:
+            orc.set_local_field(local[t])
+        orc.set_field(hx, hy, t)
+        n, log = orc.relax_B()
+        counts.append(n); logs.append(log)
+    return np.array(counts), (np.concatenate(logs) if logs else np.zeros(0, np.int32))
+
+
+@pytest.mark.parametrize("kind", ["rotating", "sinusoidal", "sawtooth"])
+def test_periodic_field_protocols_one_launch(B, kind):
+    """Input encoders of PAPER.md:63 / :156: spins flip back and forth over several periods.  One launch (fs_sweep)
+    and the stepwise path against the Tier B oracle; a run that makes more flips than the ring log holds must
+    return the LAST 4N+1024 flips."""
+    from oracle import Oracle
+    pos, ang = W.square_closed(16)
+    N = len(ang)
+    p = dict(alpha=0.001, b=0.4, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.5)
+    hc = W.coercive_fields(N, seed=8)
+    if kind == "rotating":
+        fields = W.rotating(0.13, 5, 48, 20.0)
+    elif kind == "sinusoidal":
+        fields = W.sinusoidal(0.16, 3, 40, 35.0)
+    else:
+        fields = W.sawtooth(0.16, 3, 40, 35.0)
+    orc = Oracle(pos, ang, hc, p)
+    counts, ref = _oracle_protocol(orc, fields)
+    assert counts.sum() > 2 * N and orc.monitor()[0] == 0            # every spin reverses more than once
+    sim = B.Sim(pos, ang, hc, p)
+    n, ps = sim.sweep(fields, step0=0)
+    assert np.array_equal(ps.cpu().numpy()[0], counts) and n[0] == counts.sum()
+    cap = 4 * N + 1024
+    glog = sim.get_flip_log().cpu().numpy()
+    if counts.sum() > cap:
+        assert sim.last_log_first == counts.sum() - cap and len(glog) == cap
+        assert np.array_equal(glog, ref[-cap:])
+        small = sim.get_flip_log(cap=100).cpu().numpy()             # a short buffer gets the oldest retained flips
+        assert np.array_equal(small, ref[-cap:][:100])
+    else:
+        assert sim.last_log_first == 0 and np.array_equal(glog, ref)
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    # stepwise
+    sim2 = B.Sim(pos, ang, hc, p)
+    got = []
+    for t, (hx, hy) in enumerate(fields):
+        sim2.set_field(hx, hy, t); got.append(sim2.relax())
+    assert np.array_equal(np.array(got), counts)
+    assert np.array_equal(sim2.get_spins().cpu().numpy(), orc.spins())
+
+
+def test_sweep_local_scale_and_series(B):
+    """h_ext^(i)(t) = global(t) + scale(t) * local_i + series(t, i): one launch against the oracle
+    stepping the same per-spin field (composed on the host in the same order of operations)."""
+    from oracle import Oracle
+    w = W.config("4", scale=16)
+    T = 60
+    fields = W.ramp(0.05, -0.12, T - 1, 45.0)
+    loc = 0.04 * np.stack([np.sin(0.5 * w.pos[:, 0]), np.cos(0.4 * w.pos[:, 1])], axis=1)
+    scale = np.linspace(0.0, 1.5, T)
+    rng = np.random.default_rng(5)
+    series = 0.01 * rng.standard_normal((T, w.N, 2))
+    cases = {"scale": (loc, scale, None), "series": (None, None, series), "both": (loc, scale, series), "static": (loc, None, None)}
+    for name, (l, sc, ser) in cases.items():
+        local = []
+        for t in range(T):
+            tot = np.zeros((w.N, 2))
+            if l is not None:
+                tot = (sc[t] * l) if sc is not None else l.copy()
+            if ser is not None:
+                tot = (tot + ser[t]) if l is not None else ser[t].copy()
+            local.append(tot)
+        orc = Oracle(w.pos, w.angle, w.hc, w.params); orc.set_thermal(w.sigma_th, 3)
+        counts, ref = _oracle_protocol(orc, fields, local)
+        sim = B.Sim(w.pos, w.angle, w.hc, w.params); sim.set_thermal(w.sigma_th, 3)
+        if l is not None:
+            sim.set_local_field(l)
+        n, ps = sim.sweep(fields, step0=0, local_scale=sc, local_series=ser)
+        assert np.array_equal(ps.cpu().numpy()[0], counts), name
+        assert counts.sum() > w.N // 4 and np.array_equal(sim.get_flip_log().cpu().numpy(), ref), name
+        assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins()), name
+
+
+# ------------------------------------------------------------------ f4: analysis reductions, the IV.B annealing workload
+@pytest.mark.parametrize("geom", ["square_nd3", "rotated_nd2", "kagome"])
+def test_spin_correlation_matches_oracle(B, geom):
+    from oracle import Oracle
+    if geom == "square_nd3":
+        pos, ang = W.square_closed(13); nd = 3.0
+    elif geom == "rotated_nd2":
+        pos, ang = W.rotated_square(11); nd = 2.0
+    else:
+        pos, ang = W.kagome(9); nd = 2.0
+    N = len(ang)
+    p = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=nd)
+    R = 3
+    hc = W.coercive_fields(N, seed=2, replicas=R)
+    spins = np.stack([W.random_spins(N, seed=30 + r) for r in range(R)])
+    sim = B.Sim(pos, ang, hc, p); sim.set_spins(spins)
+    for width, nbins in ((0.25, 16), (0.4, 5), (1.0, 3)):
+        sm, cnt = sim.correlation(width, nbins)
+        sm = sm.cpu().numpy(); cnt = cnt.cpu().numpy()
+        for r in range(R):
+            o = Oracle(pos, ang, hc[r], p, spins=spins[r])
+            osm, ocnt = o.spin_correlation(width, nbins)
+            assert np.array_equal(sm[r], osm) and np.array_equal(cnt, ocnt), (geom, width, r)
+        assert cnt.sum() > 0
+
+
+def test_vertex_populations_match_oracle(B):
+    from oracle import Oracle
+    n = 14
+    pos, ang = W.square_closed(n)
+    N = len(ang); V = W.square_vertices(n)
+    p = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=1.0)
+    states = [np.ones(N, np.int8), W.square_ground_state(n), W.random_spins(N, seed=1), W.random_spins(N, seed=2)]
+    g = W.square_ground_state(n).copy(); g[V[5][1]] *= -1; states.append(g)
+    hc = np.full((len(states), N), 0.2)
+    sim = B.Sim(pos, ang, hc, p); sim.set_spins(np.stack(states))
+    got = sim.vertex_populations(V).cpu().numpy()
+    for r, s in enumerate(states):
+        o = Oracle(pos, ang, hc[r], p, spins=s)
+        assert list(got[r]) == list(o.vertex_populations(V)), r
+    assert list(got[0]) == [0, (n - 1) ** 2, 0, 0] and list(got[1]) == [(n - 1) ** 2, 0, 0, 0]
+    assert list(got[4]) == [(n - 1) ** 2 - 2, 0, 2, 0] and got[2].sum() == (n - 1) ** 2
+    # pinwheel: the same vertices of the rotated lattice
+    pos, ang = W.rotated_square(n)
+    s = W.random_spins(N, seed=7)
+    sim = B.Sim(pos, ang, np.full(N, 0.2), p); sim.set_spins(s)
+    o = Oracle(pos, ang, np.full(N, 0.2), p, spins=s)
+    assert list(sim.vertex_populations(V).cpu().numpy()) == list(o.vertex_populations(V))
+
+
+def test_paper_square_anneal_ensemble(B):
+    """PAPER.md:196-206 (IV.B) scaled down: an ensemble of square ASIs annealed by an exponentially decreasing thermal
+    field in one launch; annealed spins, spin-spin correlation and vertex populations of every replica against
+    independent oracles."""
+    from oracle import Oracle
+    R = 4
+    w = W.paper_square_anneal(12, alpha=0.004, T=50, sigma0=0.12, decay=10.0, replicas=R)
+    w.params["neighbor_distance"] = 3.0
+    sigma, V = w.extra["sigma"], w.extra["vertices"]
+    sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+    sim.set_spins(np.tile(w.spins, (R, 1))); sim.set_thermal(0.0, 11)
+    n, _ = sim.sweep(w.fields, step0=0, sigma=sigma)
+    s = sim.get_spins().cpu().numpy()
+    sm, cnt = sim.correlation(0.5, 8); sm = sm.cpu().numpy(); cnt = cnt.cpu().numpy()
+    vp = sim.vertex_populations(V).cpu().numpy()
+    total = 0
+    for r in range(R):
+        o = Oracle(w.pos, w.angle, w.hc[r], w.params, spins=w.spins)
+        for t in range(len(sigma)):
+            o.set_thermal(float(sigma[t]), 11 + r); o.set_field(0.0, 0.0, t)
+            total += o.relax_B()[0]
+        assert np.array_equal(s[r], o.spins()), r
+        osm, ocnt = o.spin_correlation(0.5, 8)
+        assert np.array_equal(sm[r], osm) and np.array_equal(cnt, ocnt)
+        assert list(vp[r]) == list(o.vertex_populations(V))
+        assert o.monitor()[0] == 0
+    assert total == int(n.sum()) and total > R * w.N // 2
+    # annealing lowers the dipolar energy: more minimised nearest-neighbour pairs than in the random start
+    o0 = Oracle(w.pos, w.angle, w.hc[0], w.params, spins=w.spins)
+    assert sm[0][1] > o0.spin_correlation(0.5, 8)[0][1]
