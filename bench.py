@@ -43,6 +43,29 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def kernel_source_hash():
+    """sha256 of the CUDA sources: measured ncu figures stored under profiles/ are tied to the code they were taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2002_11401_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def stored_traffic(kernel, N, K):
+    """dram__bytes_read + dram__bytes_write per launch from the committed ncu capture (profiles/traffic.json), or None
+    if the capture was taken on other kernel sources or another workload size (a stale figure is not reported)."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None, "no capture"
+    d = json.load(open(path))
+    e = d.get(kernel)
+    if not e or e.get("source_hash") != kernel_source_hash() or (e.get("N"), e.get("K")) != (N, K):
+        return None, "capture is stale for these sources / this size (see profiles/traffic.json)"
+    return e["traffic_bytes"], e.get("source", "profiles/traffic.json")
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks / throttle reasons during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -83,8 +106,8 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------------------------ CPU oracle legs
 def oracle_field_sample(w, budget_s=12.0, chunk=256, seed=123):
-    """The oracle as it stands (Tier A direct evaluation of Eq. 3 + Eq. 5/6 per spin) on a bounded random
-    sample of the workload's spins.  Returns (interactions/s, n_spins, n_interactions, seconds)."""
+    """Tier A as it stands (direct evaluation of Eq. 3 per pair + Eq. 5/6 per spin, nothing cached) on a bounded
+    random sample of the workload's spins.  Returns (interactions/s, n_spins, n_interactions, seconds)."""
     from oracle import Oracle
     orc = Oracle(w.pos, w.angle, w.hc, w.params, spins=w.spins)
     hx, hy = w.fields[0]
@@ -100,6 +123,35 @@ def oracle_field_sample(w, budget_s=12.0, chunk=256, seed=123):
             n_sp += 1
     dt = time.perf_counter() - t0
     return n_int / dt, n_sp, n_int, dt
+
+
+def oracle_cached_legs(scale=160, budget_s=6.0):
+    """The oracle's precomputed-neighbour-list field pass and switching scan (SURVEY.md 8(d) legs (i), (ii)): couplings
+    built once (untimed), then gather_cached (h_dip = sum_j s_j w_ij over the list) + scan_cached (Eq. 2, 5, 6 per spin,
+    arg-max), timed single-threaded and with OpenMP over spins on all host cores.  Bounded sample: the config-5 recipe
+    (square ASI, neighbor distance 10, random spins) at scale x scale."""
+    from oracle import Oracle
+    w = W.config("5", scale=scale)
+    orc = Oracle(w.pos, w.angle, w.hc, w.params, spins=w.spins)
+    hx, hy = w.fields[0]
+    orc.set_field(hx, hy, 0)
+    t0 = time.perf_counter(); orc.build_weights(); t_build = time.perf_counter() - t0
+    I = orc.num_interactions
+    cores = os.cpu_count() or 1
+    out = {"sample": f"config 5 recipe at {scale}x{scale} ({w.N} spins, {I} interactions), couplings precomputed "
+                     f"(untimed, {t_build:.1f} s); each repetition = gather over the list + switching scan",
+           "N": w.N, "interactions": I, "host_cores": cores}
+    for label, nt in (("threads_1", 1), ("threads_all", cores)):
+        orc.set_threads(nt)
+        orc.gather_cached(); orc.scan_cached()
+        reps = 0; tg = ts = 0.0
+        t_end = time.perf_counter() + budget_s
+        while time.perf_counter() < t_end or reps < 2:
+            a = time.perf_counter(); orc.gather_cached(); b = time.perf_counter(); orc.scan_cached(); c = time.perf_counter()
+            tg += b - a; ts += c - b; reps += 1
+        out[label] = {"threads": nt, "repetitions": reps, "interactions_per_s": I * reps / (tg + ts),
+                      "gather_interactions_per_s": I * reps / tg, "scan_spins_per_s": w.N * reps / ts}
+    return out
 
 
 def oracle_relax_sample(scale=400):
@@ -119,63 +171,129 @@ def oracle_relax_sample(scale=400):
 
 
 def run_reference(args, rank, world):
+    """The oracle as it stands on the host cores: the precomputed-list gather + scan with OpenMP over all cores (the
+    stronger of its two field tiers), on a bounded sample of config 5; each step = one bounded run."""
     if rank != 0:
         return
-    w = W.config("5")
-    budget = 3.0
-    for _ in range(args.warmup):
-        oracle_field_sample(w, budget_s=0.5)
-    vals = []; t0 = time.perf_counter()
+    w5 = W.config("5", scale=64)
+    for _ in range(min(args.warmup, 1)):
+        oracle_cached_legs(scale=96, budget_s=0.5)
+    tot_i = tot_t = 0.0; last = None
     for k in range(args.steps):
-        v, n_sp, n_int, dt = oracle_field_sample(w, budget_s=budget, seed=1000 + k)
-        vals.append((n_int, dt))
-    tot_int = sum(a for a, _ in vals); tot_t = sum(b for _, b in vals)
-    value = tot_int / tot_t
+        r = oracle_cached_legs(scale=160, budget_s=max(1.0, 20.0 / max(args.steps, 1)))
+        a = r["threads_all"]
+        tot_i += r["interactions"] * a["repetitions"]; tot_t += r["interactions"] * a["repetitions"] / a["interactions_per_s"]
+        last = r
+    value = tot_i / tot_t
+    full = W.config("5")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "N": w.N, "neighbor_distance": 10.0},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
-                             "sample": f"each step: {budget:.0f} s of random spins of config 5, direct Eq. 3 + Eq. 5/6 per spin"},
+            "config": {"workload": full.name, "N": full.N, "neighbor_distance": 10.0},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": last["host_cores"], "kind": "oracle",
+                             "sample": last["sample"], "threads_1": last["threads_1"], "threads_all": last["threads_all"]},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
 
 # ------------------------------------------------------------------------------------------------ GPU arm
-def relax_sweep(B, torch, which="4", scale=None):
-    """Whole-sweep wall time and flips/s of config 4 (2,002,000 spins, thermal ramp, 201 steps)."""
+def relax_sweep(B, torch, which="4", scale=None, sequential=False):
+    """Whole-sweep wall time and flips/s of config 4 (2,002,000 spins, thermal ramp, 201 steps).  Pass 1 (timed as the
+    headline): every step enqueued without a host round trip.  Pass 2 (statistics): the same sweep with the flip count
+    read back after every step, for the per-step us/flip distribution."""
     w = W.config(which, scale=scale)
     t0 = time.perf_counter()
     sim = B.Sim(w.pos, w.angle, w.hc, w.params)
     torch.cuda.synchronize(); t_create = time.perf_counter() - t0
-    sim.set_spins(w.spins)
-    if w.sigma_th:
-        sim.set_thermal(w.sigma_th, w.thermal_seed)
-    sim.update_fields()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(len(w.fields) + 1)]
+    if sequential:
+        sim.set_batch(0)
+
+    def reset():
+        sim.set_spins(w.spins)
+        if w.sigma_th:
+            sim.set_thermal(w.sigma_th, w.thermal_seed)
+        sim.update_fields(); sim.counters(reset=True); torch.cuda.synchronize()
+
+    reset()
     l0 = B.kernel_launches()
-    torch.cuda.synchronize()
     t0 = time.perf_counter()
-    ev[0].record()
     for t, (hx, hy) in enumerate(w.fields):
         sim.set_field(hx, hy, t)
         sim.relax(sync=False)                      # no host round trip per step
-        ev[t + 1].record()
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
     launches = B.kernel_launches() - l0
     total, _ = sim.counters()
     flips = int(total.sum())
-    step_ms = np.array([ev[t].elapsed_time(ev[t + 1]) for t in range(len(w.fields))])
     s = sim.get_spins()
+    st = sim.batch_stats()
     out = {"workload": w.name, "N": w.N, "steps": len(w.fields), "flips": flips, "sweep_wall_s": wall,
-           "flips_per_s": flips / wall, "create_s": t_create, "gpu_launches": launches,
-           "all_reversed": bool((s == -1).all().item()), "max_step_ms": float(step_ms.max()),
-           "quiet_step_ms_median": float(np.median(step_ms))}
-    busy = step_ms > 4 * np.median(step_ms)
-    if busy.any() and flips:
-        # per-flip latency inside the avalanches: time of the busy steps beyond a quiet step / flips
-        out["us_per_flip"] = float(1e3 * (step_ms[busy] - np.median(step_ms)).sum() / flips)
+           "flips_per_s": flips / wall, "us_per_flip_whole_sweep": 1e6 * wall / max(flips, 1), "create_s": t_create,
+           "gpu_launches": launches, "all_reversed": bool((s == -1).all().item()),
+           "mode": "one flip per dependent chain (k_relax only)" if sequential else
+                   "exact batched flips (k_relax_batch on all SMs) + k_relax for the tails",
+           "batched": {"max_seeds": st["max_seeds"], "flips_committed": st["flips"], "rounds": st["rounds"],
+                       "mean_committed_prefix": st["flips"] / max(st["rounds"], 1), "seq_threshold": st["seq_threshold"]}}
+    # pass 2: per-step flips and device time
+    reset()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(len(w.fields) + 1)]
+    per = []
+    ev[0].record()
+    for t, (hx, hy) in enumerate(w.fields):
+        sim.set_field(hx, hy, t)
+        per.append(sim.relax())
+        ev[t + 1].record()
+    torch.cuda.synchronize()
+    per = np.array(per); step_ms = np.array([ev[t].elapsed_time(ev[t + 1]) for t in range(len(w.fields))])
+    quiet = float(np.median(step_ms[per == 0])) if (per == 0).any() else float(step_ms.min())
+    busy = per >= 100
+    out["quiet_step_ms_median"] = quiet
+    out["max_step_ms"] = float(step_ms.max()); out["max_step_flips"] = int(per.max())
+    if busy.any():
+        upf = 1e3 * np.maximum(step_ms[busy] - quiet, 0.0) / per[busy]
+        out["us_per_flip_mean"] = float(1e3 * np.maximum(step_ms[busy] - quiet, 0.0).sum() / per[busy].sum())
+        out["us_per_flip_median_over_steps"] = float(np.median(upf))
+        out["us_per_flip_p10_p90_over_steps"] = [float(np.percentile(upf, 10)), float(np.percentile(upf, 90))]
+        out["steps_with_100_or_more_flips"] = int(busy.sum())
+    # scan share: the fused scan alone at this size (thermal field included), times the number of steps
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    sim.scan_async(); torch.cuda.synchronize()
+    e0.record()
+    for _ in range(20):
+        sim.scan_async()
+    e1.record(); torch.cuda.synchronize()
+    scan_ms = e0.elapsed_time(e1) / 20
+    out["scan_ms"] = scan_ms
+    out["scan_share_of_sweep"] = scan_ms * 1e-3 * len(w.fields) / wall
+    out["flip_loop_share_of_sweep"] = 1.0 - out["scan_share_of_sweep"]
+    sim.close()
+    return out
+
+
+def anneal_ensemble(B, torch, R=592):
+    """PAPER.md:196-206 (IV.B): R replicas of the 50 x 50 square ASI (neighbor distance 10, b = 0.4, h_k = 0.186)
+    annealed by an exponentially decreasing thermal field, whole protocol in one launch (one CTA per replica), then the
+    spin-spin correlation by separation and the vertex populations of every replica on the device."""
+    w = W.paper_square_anneal(50, replicas=R)
+    sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+    out = {"workload": w.name, "replicas": R, "N": w.N, "K": sim.K, "steps": len(w.fields)}
+    for _ in range(2):
+        sim.set_spins(np.tile(w.spins, (R, 1))); sim.set_thermal(0.0, w.thermal_seed); sim.update_fields(); sim.counters(reset=True)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        sim.sweep(w.fields, step0=0, per_step=False, sync=False, sigma=w.extra["sigma"])
+        torch.cuda.synchronize(); dt = time.perf_counter() - t0
+    flips = int(sim.counters()[0].sum())
+    t0 = time.perf_counter()
+    sm, cnt = sim.correlation(0.5, 24)
+    vp = sim.vertex_populations(w.extra["vertices"])
+    torch.cuda.synchronize(); dt_red = time.perf_counter() - t0
+    cnt = cnt.cpu().numpy().astype(np.float64); sm = sm.cpu().numpy().astype(np.float64).mean(axis=0)
+    corr = np.where(cnt > 0, sm / np.maximum(cnt, 1), 0.0)
+    vp = vp.cpu().numpy().astype(np.float64).mean(axis=0)
+    out.update({"anneal_wall_s": dt, "flips": flips, "flips_per_s": flips / dt, "replica_anneals_per_s": R / dt,
+                "reductions_wall_s": dt_red,
+                "correlation_by_separation": {f"{0.5 * b:.1f}": round(float(corr[b]), 4) for b in range(24) if cnt[b] > 0},
+                "vertex_fractions_I_II_III_IV": [round(float(x / vp.sum()), 4) for x in vp]})
     sim.close()
     return out
 
@@ -367,11 +485,11 @@ def run_ours(args, rank, world, local_rank):
         achieved = 2.0 * 2.0 * I / (gather_ms * 1e-3) / 1e12    # 2 DFMA (4 flop) per interaction
         roofline = {"bound": "alu", "kernel": "k_gather_stencil", "achieved": achieved, "peak": 2.0 * dfma_peak / 1e12,
                     "unit": "TFLOP/s", "frac": achieved / (2.0 * dfma_peak / 1e12),
-                    # dram__bytes_read+write of one launch at full config-5 size, from the committed ncu capture
-                    "traffic": 3310848 if (N, K) == (501000, 632) else None, "traffic_source": "profiles/r01_ncu_full.md",
+                    "traffic": stored_traffic("k_gather_stencil", N, K)[0], "traffic_source": stored_traffic("k_gather_stencil", N, K)[1],
+                    "inversion_pairs": bool(lat.get("inversion_pairs")),
                     "peak_source": "fp64 DFMA-chain kernel (fs_measure_fp64_peak) measured in this run; "
                                    "nominal 148 SM x 64 DFMA/clk x 1.965 GHz = 37.2 TFLOP/s",
-                    "algorithmic_flops_per_launch": 4.0 * I, "kernel_ms": gather_ms,
+                    "algorithmic_flops_per_launch": 4.0 * I, "kernel_ms": gather_ms, "source_hash": kernel_source_hash(),
                     "share_of_step": gather_ms / (ms / args.steps)}
     else:
         achieved = ell_bytes / (gather_ms * 1e-3) / 1e9
@@ -384,7 +502,8 @@ def run_ours(args, rank, world, local_rank):
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "N": N, "K": K, "interactions": I, "neighbor_distance": w.params["neighbor_distance"],
-                   "step": "fs_update_fields + fs_scan", "gather": "lattice stencil" if use_stencil else "ELL fp64",
+                   "step": "fs_update_fields + fs_scan",
+                   "gather": ("lattice stencil" + (", inversion-paired" if lat.get("inversion_pairs") and args.gather != 3 else "")) if use_stencil else "ELL fp64",
                    "lattice": lat,
                    "l2": "flushed before every timed step (256 MiB fill, untimed); step time = sum of per-step CUDA-event intervals",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "create_s": t_create,
@@ -401,18 +520,24 @@ def run_ours(args, rank, world, local_rank):
         a = ell_bytes / (ell * 1e-3) / 1e9
         line["roofline_ell"] = {"bound": "hbm", "kernel": "k_gather (general-geometry ELL path, same workload)",
                                 "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak,
-                                "traffic": 6271733000 if (N, K) == (501000, 632) else None,
-                                "traffic_source": "profiles/r01_ncu_full.md",
+                                "traffic": stored_traffic("k_gather", N, K)[0], "traffic_source": stored_traffic("k_gather", N, K)[1],
                                 "peak_source": peak_src, "algorithmic_bytes_per_launch": ell_bytes, "kernel_ms": ell,
                                 "interactions_per_s": I / (ell * 1e-3)}
     sim.close()
     if rank == 0 and not args.no_cpu:
-        v, n_sp, n_int, dt = oracle_field_sample(w, budget_s=args.cpu_budget)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"{n_sp} random spins of {w.name} ({n_int} interactions, {dt:.1f} s): direct Eq. 3 + Eq. 5/6 per spin"}
+        legs = oracle_cached_legs(scale=160, budget_s=args.cpu_budget / 2)
+        v, n_sp, n_int, dt = oracle_field_sample(w, budget_s=min(args.cpu_budget, 6.0))
+        line["cpu_baseline"] = {"value": legs["threads_all"]["interactions_per_s"], "unit": UNIT, "cores": legs["host_cores"],
+                                "kind": "oracle", "sample": legs["sample"],
+                                "threads_1": legs["threads_1"], "threads_all": legs["threads_all"],
+                                "tier_a_direct": {"interactions_per_s": v, "cores": 1,
+                                                  "sample": f"{n_sp} random spins of {w.name} ({n_int} interactions, {dt:.1f} s): "
+                                                            "direct Eq. 3 per pair + Eq. 5/6 per spin, nothing cached"}}
     if rank == 0 and not args.no_relax:
         try:
             line["relax"] = relax_sweep(B, torch, "4", scale=args.relax_scale)
+            line["relax_sequential"] = relax_sweep(B, torch, "4", scale=args.relax_scale, sequential=True)
+            line["relax"]["speedup_over_sequential"] = line["relax_sequential"]["sweep_wall_s"] / line["relax"]["sweep_wall_s"]
             if not args.no_cpu:
                 line["relax"]["cpu_baseline"] = oracle_relax_sample()
         except Exception as e:   # never lose the headline line
@@ -421,6 +546,10 @@ def run_ours(args, rank, world, local_rank):
             line["sweeps"], line["ensemble"] = protocol_sweeps(B, torch, cpu=not args.no_cpu)
         except Exception as e:
             line["sweeps"] = {"error": repr(e)}
+        try:
+            line["anneal_ensemble"] = anneal_ensemble(B, torch)
+        except Exception as e:
+            line["anneal_ensemble"] = {"error": repr(e)}
         try:
             line["paper_workloads"] = paper_workloads(B, torch)
         except Exception as e:
@@ -438,7 +567,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--gather", type=int, default=0, help="FS_GATHER_* variant (0 auto, 1 ELL fp64, 2 lattice stencil)")
+    ap.add_argument("--gather", type=int, default=0, help="FS_GATHER_* variant (0 auto, 1 ELL fp64, 2 lattice stencil, 3 stencil without inversion pairing)")
     ap.add_argument("--no-ell", action="store_true", help="skip the side measurement of the ELL gather")
     ap.add_argument("--scale", type=int, default=None, help="debug: lattice size override for config 5")
     ap.add_argument("--relax-scale", type=int, default=None, help="debug: lattice size override for config 4")

@@ -20,7 +20,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 def build(force: bool = False) -> str:
     """Compile the oracle with g++ (fp64, no FMA contraction so it rounds like the formulas read)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC",
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-shared", "-fPIC",
                                _SRC, "-o", _LIB])
     return _LIB
 
@@ -63,6 +63,9 @@ def lib():
             getattr(L, name).argtypes = [vp, i64, vp, i64]
         L.orc_cached_hdip.argtypes = [vp, vp]
         L.orc_gather_cached.argtypes = [vp]
+        L.orc_set_threads.argtypes = [vp, i32]
+        L.orc_build_weights.argtypes = [vp]
+        L.orc_scan_cached.argtypes = [vp, P(i64), P(i64), P(dbl)]
         L.orc_monitor.argtypes = [vp, P(i64), P(dbl), P(dbl), i32]
         L.orc_spin_correlation.argtypes = [vp, dbl, i64, vp, vp]
         L.orc_vertex_populations.argtypes = [vp, vp, i64, vp]
@@ -184,6 +187,13 @@ class Oracle:
         h = np.zeros((self.N, 2)); self.L.orc_cached_hdip(self.h, h.ctypes.data); return h
 
     def gather_cached(self): self.L.orc_gather_cached(self.h)
+    def build_weights(self): self.L.orc_build_weights(self.h)
+    def set_threads(self, n): self.L.orc_set_threads(self.h, int(n))
+
+    def scan_cached(self):
+        n, b, l = C.c_int64(), C.c_int64(), C.c_double()
+        self.L.orc_scan_cached(self.h, C.byref(n), C.byref(b), C.byref(l))
+        return n.value, b.value, l.value
 
     def monitor(self, reset=False):
         n, g, t = C.c_int64(), C.c_double(), C.c_double()

@@ -20,7 +20,8 @@
 // Unpinned by the paper: full-config flip sequences (no published values exist); they are pinned only
 // through Tier A == Tier B on small sizes plus the invariants above ("parity unpinned" for those).
 //
-// Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC flatspin_oracle.cpp -o liboracle.so
+// Build: g++ -O2 -ffp-contract=off -fopenmp -std=c++17 -shared -fPIC flatspin_oracle.cpp -o liboracle.so
+// (OpenMP only splits the per-spin loops of the two timing legs gather_cached / scan_cached over host threads.)
 
 #include <algorithm>
 #include <cmath>
@@ -293,9 +294,12 @@ struct Oracle {
         }
         have_w = true;
     }
+    // (timing legs only: the loop over spins may be split over host threads; every spin's sum is unchanged)
+    int nthreads = 1;
     void gather_cached() {
         build_weights();
         hd_par.assign(N, 0.0); hd_perp.assign(N, 0.0);
+#pragma omp parallel for num_threads(nthreads) schedule(static)
         for (int64_t i = 0; i < N; ++i) {
             double a = 0.0, b = 0.0;
             for (size_t k = 0; k < nbr[i].size(); ++k) {
@@ -305,6 +309,27 @@ struct Oracle {
         }
         hd_valid = true;
     }
+    // Switching scan over the cached h_dip (Eq. 2 + Eqs. 5, 6 per spin): number of switchable spins and the arg-max,
+    // lowest index among ties (C-7).  Same decisions as orc_scan, which recomputes Eq. 3 per pair instead.
+    void scan_cached(int64_t* n_switchable, int64_t* best_index, double* best_L) {
+        if (!hd_valid) gather_cached();
+        const int T = nthreads > 0 ? nthreads : 1;
+        std::vector<int64_t> cn(T, 0), cb(T, -1); std::vector<double> cl(T, NEG_INF);
+#pragma omp parallel for num_threads(T) schedule(static, 1)
+        for (int t = 0; t < T; ++t) {
+            const int64_t i0 = N * t / T, i1 = N * (t + 1) / T;
+            for (int64_t i = i0; i < i1; ++i) {
+                double h[2]; const double d[2] = {hd_par[i], hd_perp[i]};
+                total_from_dip(i, d, h);
+                const double k = key_of(i, h);
+                if (k > 1.0) { ++cn[t]; if (k > cl[t]) { cl[t] = k; cb[t] = i; } }
+            }
+        }
+        int64_t n = 0, best = -1; double L1 = NEG_INF;
+        for (int t = 0; t < T; ++t) { n += cn[t]; if (cl[t] > L1) { L1 = cl[t]; best = cb[t]; } }
+        *n_switchable = n; *best_index = best; *best_L = best >= 0 ? L1 : NEG_INF;
+    }
+
     bool better(int32_t a, int32_t b) const {               // key desc, index asc
         if (a < 0) return false;
         if (b < 0) return true;
@@ -508,6 +533,11 @@ void orc_cached_hdip(void* h, double* out) {
     for (int64_t i = 0; i < o->N; ++i) { out[2 * i] = o->hd_par[i]; out[2 * i + 1] = o->hd_perp[i]; }
 }
 void orc_gather_cached(void* h) { ((Oracle*)h)->gather_cached(); }
+void orc_set_threads(void* h, int n) { ((Oracle*)h)->nthreads = n > 0 ? n : 1; }
+void orc_build_weights(void* h) { ((Oracle*)h)->build_weights(); }
+void orc_scan_cached(void* h, int64_t* n_switchable, int64_t* best_index, double* best_L) {
+    ((Oracle*)h)->scan_cached(n_switchable, best_index, best_L);
+}
 void orc_monitor(void* h, int64_t* n_events, double* min_gap, double* min_thr, int reset) {
     Oracle* o = (Oracle*)h; *n_events = o->n_events; *min_gap = o->min_gap; *min_thr = o->min_thr;
     if (reset) { o->n_events = 0; o->min_gap = 1e300; o->min_thr = 1e300; }

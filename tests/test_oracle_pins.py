@@ -627,3 +627,23 @@ def test_field_protocol_generators():
     assert w.N == 5100 and w.params["neighbor_distance"] == 10.0 and w.params["b"] == 0.4
     sig = w.extra["sigma"]
     assert np.all(np.diff(np.log(sig)) < 0) and np.allclose(np.diff(np.log(sig)), np.diff(np.log(sig))[0])   # exponential
+
+
+def test_cached_scan_and_threaded_gather_equal_the_direct_tier():
+    """The two legs bench.py times on the host (cached-coupling gather, scan over the cached h_dip, optionally split
+    over threads) make the same decisions as the direct Tier A evaluation and do not depend on the thread count."""
+    w = W.config("3", scale=12)
+    s = W.random_spins(w.N, seed=4)
+    o = Oracle(w.pos, w.angle, w.hc, w.params, spins=s)
+    o.set_thermal(0.01, 5); o.set_field(0.05, -0.06, 7)
+    ref = o.scan()
+    hd = None
+    for nt in (1, 3, 8):
+        o.set_threads(nt); o.set_spins(s)
+        o.gather_cached()
+        h = o.cached_hdip()
+        assert hd is None or np.array_equal(h, hd)
+        hd = h
+        got = o.scan_cached()
+        assert got[:2] == ref[:2] and abs(got[2] - ref[2]) <= 1e-13 * abs(ref[2])
+    assert np.abs(hd - o.fields(1)).max() <= 1e-13 * np.abs(hd).max()
