@@ -80,7 +80,7 @@ enum {
     FS_LATTICE_STENCIL_TOO_WIDE = 5,      /* half-extent > 40 cells or shared memory exceeded */
     FS_LATTICE_TOO_SPARSE = 6,            /* dense grids would exceed 8N + 2^20 cells */
     FS_LATTICE_REACH_MISMATCH = 7,        /* stencil would reach a different set of pairs than the ELL */
-    FS_LATTICE_WEIGHT_MISMATCH = 8        /* couplings of equal offsets differ by more than 2e-13/K relative */
+    FS_LATTICE_WEIGHT_MISMATCH = 8        /* couplings of equal offsets differ by more than 5e-13/K relative to max|w| */
 };
 
 /* Bytes of workspace fs_create[_ensemble] needs for this geometry (runs the cell-grid neighbour count,

@@ -466,10 +466,7 @@ __device__ __forceinline__ double2 fixed_field(double2 c, double2 he, const Fiel
 
 struct ScanGroup { double v; int idx; unsigned cnt; };  // result of one group of 32 scan CTAs
 // uint32 words of scan scratch per replica: per-CTA counts, group tickets, group results
-__host__ __device__ inline size_t scan_aux_stride(int ncta) {
-    int ngroups = (ncta + 31) >> 5;
-    return (size_t)((ncta + ngroups + 3) & ~3) + 4 * (size_t)ngroups;
-}
+__host__ __device__ inline size_t scan_aux_stride(int ncta) { return 4 * (size_t)ncta + 4; }   // one ScanGroup per CTA
 
 constexpr int SCAN_SPB = 1024;                          // consecutive spins per CTA = 1024 / LB leaves
 
@@ -530,50 +527,38 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
         }
     }
     if (!finalize) return;
-    // A7 top level (fs_scan only), two-level "last one out" reduction so that no CTA has a long serial tail:
-    // CTAs form groups of 32; the last CTA of a group to finish reduces the group's leaf maxima and
-    // switchable counts; the last group to finish reduces the <= 64 group results.  One ticket atomic per
-    // CTA and one per group; everything else is plain stores + fences.
+    // A7 top level (fs_scan, and the hand-over count for k_relax_batch): every CTA publishes (its arg-max, its number
+    // of switchable spins) and takes a ticket; the last CTA to finish reduces the <= N/1024 entries.  One dependent
+    // round trip after the CTA's own work (a two-level version cost two).
     __shared__ unsigned wcnt[32];
-    __shared__ unsigned long long wc[32];
-    const int ncta = gridDim.x, ngroups = (ncta + 31) >> 5, g = blockIdx.x >> 5;
-    unsigned* scnt = scnt_all + (int64_t)r * scan_aux_stride(ncta);           // [ncta] per-CTA counts
-    unsigned* gticket = scnt + ncta;                                           // [ngroups]
-    ScanGroup* gres = reinterpret_cast<ScanGroup*>(scnt + ((ncta + ngroups + 3) & ~3));   // [ngroups], 16-byte aligned
+    const int ncta = gridDim.x;
+    ScanGroup* cres = reinterpret_cast<ScanGroup*>(scnt_all + (int64_t)r * scan_aux_stride(ncta));   // [ncta]
     if (lane == 0) wcnt[w] = (unsigned)nsw;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned c = 0;
-        for (int k = 0; k < SCAN_THREADS / 32; ++k) c += wcnt[k];
-        scnt[blockIdx.x] = c;
-        __threadfence();
-        is_last = (atomicAdd(&gticket[g], 1u) == (unsigned)(min(32, ncta - 32 * g) - 1));
+    if (w == 0) {
+        double v = wv[lane]; int bi = wi[lane];              // 32 slots of 32 spins
+        warp_argmax_margin(v, bi);
+        unsigned c = lane < SCAN_THREADS / 32 ? wcnt[lane] : 0u;
+        c = __reduce_add_sync(0xffffffffu, c);
+        if (lane == 0) {
+            cres[blockIdx.x].v = v; cres[blockIdx.x].idx = bi; cres[blockIdx.x].cnt = c;
+            __threadfence();
+            is_last = (atomicAdd(&ctr[r].ticket, 1u) == (unsigned)(ncta - 1));
+        }
     }
     __syncthreads();
     if (!is_last) return;
     __threadfence();
     double v = -CUDART_INF; int bi = 0x7fffffff;
     unsigned long long cnt = 0;
-    {
-        const int nleaf = SCAN_SPB / LB;
-        const int b0 = 32 * g * nleaf, b1 = min(nblk, 32 * (g + 1) * nleaf);
-        const double* bval = bval_all + (int64_t)r * nblk;
-        const int* bidx = bidx_all + (int64_t)r * nblk;
-        for (int t0 = b0 + threadIdx.x; t0 < b1; t0 += 4 * SCAN_THREADS) {     // <= 1024 leaves: one batch of 4 loads
-            double tv[4]; int ti[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                int t = t0 + u * SCAN_THREADS;
-                tv[u] = t < b1 ? __ldcg(bval + t) : -CUDART_INF;
-                ti[u] = t < b1 ? __ldcg(bidx + t) : 0x7fffffff;
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) if (better(tv[u], ti[u], v, bi)) { v = tv[u]; bi = ti[u]; }
-        }
-        if (threadIdx.x < 32 && 32 * g + (int)threadIdx.x < ncta) cnt = __ldcg(scnt + 32 * g + threadIdx.x);
+    for (int t = threadIdx.x; t < ncta; t += SCAN_THREADS) {
+        const double tv = __ldcg(&cres[t].v); const int ti = __ldcg(&cres[t].idx);
+        cnt += __ldcg(&cres[t].cnt);
+        if (better(tv, ti, v, bi)) { v = tv; bi = ti; }
     }
     warp_argmax_margin(v, bi);
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    __shared__ unsigned long long wc[32];
     __syncthreads();                                     // wv/wi are reused
     if (lane == 0) { wv[w] = v; wi[w] = bi; wc[w] = cnt; }
     __syncthreads();
@@ -582,24 +567,7 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
             if (better(wv[k], wi[k], v, bi)) { v = wv[k]; bi = wi[k]; }
             cnt += wc[k];
         }
-        gres[g].v = v; gres[g].idx = bi; gres[g].cnt = (unsigned)cnt;
-        gticket[g] = 0u;
-        __threadfence();
-        is_last = (atomicAdd(&ctr[r].ticket, 1u) == (unsigned)(ngroups - 1));
-    }
-    __syncthreads();
-    if (!is_last || threadIdx.x >= 32) return;
-    __threadfence();
-    v = -CUDART_INF; bi = 0x7fffffff; cnt = 0;
-    for (int t = lane; t < ngroups; t += 32) {
-        double tv = __ldcg(&gres[t].v); int ti = __ldcg(&gres[t].idx);
-        cnt += __ldcg(&gres[t].cnt);
-        if (better(tv, ti, v, bi)) { v = tv; bi = ti; }
-    }
-    warp_argmax_margin(v, bi);
-    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
-    if (lane == 0) {
-        bool any = v > 1.0;
+        const bool any = v > 1.0;
         ctr[r].best_index = any ? bi : -1;
         ctr[r].best_L = any ? v : -CUDART_INF;
         ctr[r].n_switchable = (long long)cnt;
@@ -1570,7 +1538,12 @@ int detect_lattice(fs_sim* sim) {
     for (unsigned long long o : own) sim->st_slots += (o != ~0ull);
     if (flags & 4) return lattice_fail(sim, FS_LATTICE_NOT_PERIODIC);
     if ((long long)res64[2] != (long long)sim->n_inter) return lattice_fail(sim, FS_LATTICE_REACH_MISMATCH);
-    if (!(sim->st_maxdev * (double)sim->K <= 2e-13 * sim->st_wmax)) return lattice_fail(sim, FS_LATTICE_WEIGHT_MISMATCH);
+    // Acceptance (i): the stencil field differs from the per-pair (ELL) field by at most sum_j |w_ij - T| <= K * maxdev
+    // at every spin.  On lattices with irrational coordinates (kagome: y = p * sqrt3 / 4, rounded per spin) couplings
+    // of equal offsets differ by the rounding of the positions, ~3 ulp(coordinate) / d relative, so maxdev is not 0;
+    // K * maxdev <= 5e-13 max|w| keeps the stencil field within 1e-12 of the per-pair field relative to max|h| for
+    // every state with max|h| >= max|w| / 2.  Exact lattices (square, pinwheel) have maxdev == 0.
+    if (!(sim->st_maxdev * (double)sim->K <= 5e-13 * sim->st_wmax)) return lattice_fail(sim, FS_LATTICE_WEIGHT_MISMATCH);
     const size_t stb = 200 * 1024;                       // the planner's cap: set once for every instantiation
     CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, false, 64>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, false, 64>, stb));

@@ -11,7 +11,7 @@
 //
 // Nothing is assumed about the input: the lattice is *detected* from raw pos/angle, the table is
 // filled from the ELL couplings already computed from the actual positions (k_weights), and the
-// result is accepted only if (i) every ELL entry equals its table entry to <= 2e-13/K relative and
+// result is accepted only if (i) every ELL entry equals its table entry to <= 5e-13/K relative to max|w| and
 // (ii) the stencil reaches exactly the ELL's interactions.  Otherwise the ELL gather is used.
 //
 //   k_lat_assign        sublattice + integer cell of every spin, one pass per sublattice

@@ -77,6 +77,16 @@ def test_config2_full_neighbor_count(B):
     w = W.config("2")
     sim = B.Sim(w.pos, w.angle, w.hc, w.params)
     assert (sim.N, sim.K, sim.n_interactions) == (7699, 14, 105476)
+    # full size, stencil (the auto choice) against the oracle's direct evaluation on random spins
+    from oracle import Oracle
+    for which in ("2", "2b"):
+        w = W.config(which)
+        spins = W.random_spins(w.N, seed=17)
+        sim = B.Sim(w.pos, w.angle, w.hc, w.params); sim.set_spins(spins)
+        assert sim.lattice()["active"] and sim.lattice()["nsub"] == 3
+        orc = Oracle(w.pos, w.angle, w.hc, w.params, spins=spins)
+        sim.update_fields()
+        assert field_err(sim.get_fields(1).cpu().numpy(), orc.fields(1)) < FIELD_TOL
 
 
 # ------------------------------------------------------------------ A3: full gather (ELL and lattice stencil)
@@ -97,11 +107,7 @@ def test_full_gather_fields(B, which, scale, variant):
     sim, orc = mk(B, w, spins=spins)
     lat = sim.lattice()
     if variant == "stencil":
-        if not lat["active"]:
-            # only the kagome lattice (irrational coordinates: couplings of equal offsets differ in the
-            # last bits) may decline the stencil; the square-based configs must take it
-            assert which == "2" and lat["reason"] == 8, lat
-            pytest.skip("stencil declined: couplings of equal offsets differ beyond 2e-13/K")
+        assert lat["active"], lat                 # every BASELINE geometry is a detected lattice (kagome: 3 sublattices)
         sim.set_gather_variant(B.GATHER_STENCIL)
     else:
         sim.set_gather_variant(B.GATHER_ELL_F64)
@@ -124,7 +130,8 @@ def test_lattice_detection_tables(B):
     assert lat["active"] and lat["nsub"] == 2 and lat["slots"] == 16, lat       # 4 same + 4 cross, per sublattice
     w = W.config("2", scale=12)
     lat = B.Sim(w.pos, w.angle, w.hc, w.params).lattice()
-    assert lat["nsub"] == 3 and lat["reason"] in (0, 8), lat
+    assert lat["active"] and lat["nsub"] == 3 and not lat["inversion_pairs"], lat    # irrational coordinates: T[d] != T[-d] bit for bit
+    assert 0 < lat["max_dev"] * 14 < 5e-13 * lat["w_max"]
 
 
 @pytest.mark.parametrize("geom", ["square_open", "pinwheel_diamond", "ising", "ising_chain"])
