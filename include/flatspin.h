@@ -167,7 +167,9 @@ int fs_relax_ensemble(fs_sim* sim, int64_t max_flips, int64_t* n_flips_out /*HOS
  * candidates, joined into components where their closed neighbourhoods overlap, each relaxed locally by one warp,
  * merged by effective key, cut at the first conflict (batch.cuh has the argument).  The flip log, spins and fields
  * are identical to the one-flip-at-a-time loop, which still finishes the tail once fewer than `seq_threshold`
- * spins are switchable.  max_seeds = 0 switches the batched kernel off; the default is min(4096, N / (8 (K+1))).
+ * spins are switchable.  max_seeds = 0 switches the batched kernel off; the default is about 4 sqrt(N / (K+1)) (the
+ * measured optimum: commits per round grow with the seeds, collisions between regions with their square), the
+ * maximum twice that (at most 4096).
  * fs_get_batch_stats: out4 HOST [4] = {max_seeds in use (0 = off), flips committed by the batched kernel, its
  * rounds (mean committed prefix = flips / rounds), seq_threshold} since creation / the last counter reset.
  * Synchronises. */

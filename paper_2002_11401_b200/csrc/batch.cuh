@@ -48,6 +48,7 @@ struct BatchCtl {                      // zeroed once at creation; every launch 
     unsigned bail;                     // 1 = exact ties defeated the threshold search in the last launch
     unsigned round_base;               // rounds of all launches so far: the claim tag of a round is unique across launches
     unsigned launch;                   // launches that used the barrier so far (their parity picks the counter)
+    unsigned n_list;                   // entries of the candidate list (this launch)
     unsigned n_seeds[4], n_commit[4], n_block[4];      // rotating per-round counters
     unsigned long long n_cand[3];
     unsigned hist[3][BT_NB];           // rotating histograms (one per pass)
@@ -63,7 +64,8 @@ struct BatchArgs {
     // scratch
     BatchCtl* ctl; unsigned* owner; BatchSeed* seeds; unsigned short* edges; unsigned char* ecount;
     int* npos; BatchElem* elems; BatchUndo* undo; BatchBlock* blocks; BatchCommit* clist;
-    int P, seq_threshold, min_commit;
+    int* cand; unsigned* cbits;        // candidate list: every spin with margin > 1 is in it (dead entries stay), bit = listed
+    int P, seq_threshold, min_commit, max_chain;
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -145,6 +147,25 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     bool any_flip = false;
     int lean = 0;                                       // consecutive rounds that committed fewer than min_commit flips
 
+    // ---- candidate list: every spin with margin > 1 (one pass over M per launch; the rounds then touch only the list).
+    // Invariant at the start of every round: {i : M_i > 1} is a subset of the list.  Spins whose margin falls to <= 1
+    // stay as dead entries (skipped by their margin); spins that become switchable are appended when a round
+    // commits the flip that touched them.
+    for (int64_t wd = gtid; wd < (N + 31) / 32; wd += nthreads) a.cbits[wd] = 0u;
+    if (gtid == 0) g->n_list = 0u;
+    grid_bar(bar, epoch);
+    for (int64_t i0 = (int64_t)gwarp * 32; i0 < N; i0 += (int64_t)nwarps * 32) {
+        const int64_t i = i0 + lane;
+        const bool c = i < N && __ldcg(a.M + i) > 1.0;
+        const unsigned m = __ballot_sync(0xffffffffu, c);
+        if (m) {
+            unsigned base = 0;
+            if (lane == 0) { base = atomicAdd(&g->n_list, (unsigned)__popc(m)); a.cbits[i0 >> 5] = m; }   // word i0/32 is this warp's
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (c) a.cand[base + __popc(m & ((1u << lane) - 1u))] = (int)i;
+        }
+    }
+    grid_bar(bar, epoch);
 #ifdef FS_BATCH_PROFILE
     long long tprof = bt_now();
 #endif
@@ -161,13 +182,14 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         unsigned long long ncand_total = 0;
         bool have_theta = false, quit = false;
         const unsigned P = (unsigned)a.P;
+        const int nl = (int)__ldcg(&g->n_list);
         for (int refine = 0; refine < 8 && !have_theta; ++refine, ++npass) {
             const int hb = (int)(npass % 3);
             for (int b = tid; b < BT_NB; b += BT_THREADS) sh_hist[b] = 0;
             __syncthreads();
             unsigned my_cand = 0;
-            for (int64_t i = gtid; i < N; i += nthreads) {
-                const mkey_t key = margin_key(__ldcg(a.M + i));
+            for (int j = gtid; j < nl; j += nthreads) {
+                const mkey_t key = margin_key(__ldcg(a.M + a.cand[j]));
                 if (key > KEY_ONE) {
                     ++my_cand;
                     if (shift < 0) atomicAdd(&sh_hist[log_bin(key - KEY_ONE - 1)], 1u);
@@ -237,9 +259,10 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         BT_PROF(0);
         // ================= phase 2: seeds = candidates with key > theta ====================================
         BatchSeed* seeds = a.seeds;
-        for (int64_t i0 = (int64_t)gwarp * 32; i0 < N; i0 += (int64_t)nwarps * 32) {
-            const int64_t i = i0 + lane;
-            const mkey_t key = i < N ? margin_key(__ldcg(a.M + i)) : 0ull;
+        for (int j0 = gwarp * 32; j0 < nl; j0 += nwarps * 32) {
+            const int j = j0 + lane;
+            const int i = j < nl ? a.cand[j] : -1;
+            const mkey_t key = i >= 0 ? margin_key(__ldcg(a.M + i)) : 0ull;
             const bool sel = key > theta;
             const unsigned m = __ballot_sync(0xffffffffu, sel);
             if (m) {
@@ -248,7 +271,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 base = __shfl_sync(0xffffffffu, base, 0);
                 if (sel) {
                     const unsigned slot = base + __popc(m & ((1u << lane) - 1u));
-                    if (slot < BT_PMAX) seeds[slot] = BatchSeed{key, (int)i, 0};
+                    if (slot < BT_PMAX) seeds[slot] = BatchSeed{key, i, 0};
                 }
             }
         }
@@ -295,13 +318,14 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         grid_bar(bar, epoch);
         BT_PROF(3);
         // ================= phase 5: components (every CTA computes the same labels in shared memory) ========
-        for (int r = tid; r < n_seeds; r += BT_THREADS) { sh_label[r] = r; sh_cnt[r] = 0; }
+        for (int r = tid; r < n_seeds; r += BT_THREADS) { sh_label[r] = r; sh_cnt[r] = __ldcg(a.ecount + r); }   // edge counts cached
         __syncthreads();
         for (;;) {
             int changed = 0;
             for (int r = tid; r < n_seeds; r += BT_THREADS) {
-                const int ec = __ldcg(a.ecount + r);
-                const int n = ec == 0xFF ? BT_EMAX : ec;
+                const unsigned ec = sh_cnt[r];
+                if (!ec) continue;                                               // most seeds conflict with nobody
+                const int n = ec == 0xFF ? BT_EMAX : (int)ec;
                 for (int e = 0; e < n; ++e) {
                     const int o = __ldcg(a.edges + r * BT_EMAX + e);
                     const int lr = sh_label[r], lo_ = sh_label[o], m = min(lr, lo_);
@@ -316,6 +340,8 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
             }
             if (!__syncthreads_or(changed)) break;
         }
+        for (int r = tid; r < n_seeds; r += BT_THREADS) sh_cnt[r] = 0;
+        __syncthreads();
         for (int r = tid; r < n_seeds; r += BT_THREADS) atomicAdd(&sh_cnt[sh_label[r]], 1u);     // members per component
         __syncthreads();
         BT_PROF(4);
@@ -356,7 +382,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 warp_argmax_key(bk, k);
                 if (!(bk > theta)) break;                                        // what is left is <= theta
                 if (bk < ev || (bk == ev && k > ei)) { ev = bk; ei = k; }       // running minimum in flip order
-                if (pos >= BT_LMAX) { post = true; pv = ev; pi = ei; pp = pos; break; }
+                if (pos >= a.max_chain) { post = true; pv = ev; pi = ei; pp = pos; break; }
                 const int* rowk = a.nbr + (int64_t)k * Kp;
                 // claim the closed neighbourhood
                 bool ok = true;
@@ -467,6 +493,16 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 if (lane == 0) a.s[k] = (int8_t)(-__ldcg(a.s + k));
                 __syncwarp();
             }
+            for (int p = 0; p < keep; ++p) {                                     // spins the committed flips made switchable
+                const BatchUndo* und = a.undo + ((int64_t)r * BT_LMAX + p) * (Kp + 1);
+                for (int t = lane; t <= Kp; t += 32) {
+                    const int idx = und[t].idx;
+                    if (idx >= 0 && __ldcg(a.M + idx) > 1.0) {
+                        const unsigned bit = 1u << (idx & 31);
+                        if (!(atomicOr(a.cbits + (idx >> 5), bit) & bit)) a.cand[atomicAdd(&g->n_list, 1u)] = idx;
+                    }
+                }
+            }
             if (keep) {
                 unsigned base = 0;
                 if (lane == 0) base = atomicAdd(&g->n_commit[rot], (unsigned)keep);
@@ -500,7 +536,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         // a round costs about as much as a few dozen sequential flips: when avalanches are dominoes (every flip
         // triggers the next one) the prefixes stay short and the one-flip-at-a-time loop is faster
         lean = nc < a.min_commit ? lean + 1 : 0;
-        if (lean >= 3) { ++rounds; break; }
+        if (lean >= 4) { ++rounds; break; }
         // (no barrier: the next round's first pass only reads M, which phase 7 finished before the last barrier;
         //  clist is rewritten only after three more barriers)
     }

@@ -1048,7 +1048,7 @@ struct fs_sim {
     double st_maxdev = 0.0, st_wmax = 0.0;
     long long st_slots = 0;         // stencil slots present (sum over sublattice pairs)
     // exact batched flips (batch.cuh); library-owned scratch, freed by fs_destroy
-    void* bt_mem = nullptr; BatchArgs bt{}; bool bt_ok = false; int bt_P = 0, bt_seq = 64, bt_min_commit = 32, bt_grid = 0;
+    void* bt_mem = nullptr; BatchArgs bt{}; bool bt_ok = false; int bt_P = 0, bt_alloc = 0, bt_seq = 64, bt_min_commit = 20, bt_max_chain = BT_LMAX, bt_grid = 0;
 };
 
 namespace {
@@ -1632,7 +1632,7 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
 int launch_batch(fs_sim* sim) {
     BatchArgs a = sim->bt;
     a.cellidx = sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr;
-    a.P = sim->bt_P; a.seq_threshold = sim->bt_seq; a.min_commit = sim->bt_min_commit;
+    a.P = sim->bt_P; a.seq_threshold = sim->bt_seq; a.min_commit = sim->bt_min_commit; a.max_chain = sim->bt_max_chain;
     void* args[] = {&a};
     CUDA_TRY(cudaLaunchCooperativeKernel((const void*)k_relax_batch, dim3((unsigned)sim->bt_grid), dim3(BT_THREADS), args, 0, sim->stream));
     LAUNCHED();
@@ -1647,6 +1647,11 @@ int do_relax(fs_sim* sim, int64_t max_flips) {
     return launch_relax(sim, max_flips, 0, nullptr, 0, nullptr, nullptr, batch ? 1 : 0);
 }
 
+int batch_default_seeds(int64_t N, int K) {
+    const double p = 4.0 * std::sqrt((double)N / (double)(K + 1));
+    return (int)std::max(64.0, std::min((double)BT_PMAX, std::floor(p)));
+}
+
 // scratch of k_relax_batch; never fails the creation (no scratch = sequential relax only)
 int setup_batch(fs_sim* sim) {
     sim->bt_ok = false;
@@ -1656,15 +1661,19 @@ int setup_batch(fs_sim* sim) {
     if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_relax_batch, BT_THREADS, 0) != cudaSuccess || occ < 1) {
         cudaGetLastError(); return FS_OK;
     }
-    const int64_t pc = sim->N / (8 * (int64_t)(sim->K + 1));
-    const int P = (int)std::max<int64_t>(64, std::min<int64_t>(BT_PMAX, pc));
+    // seeds per round: commits per round grow with the seeds, collisions between growing regions with their square;
+    // measured optimum on config 4 at three sizes (125 k, 501 k, 2.0 M spins: 384-512, 768-1024, 1792-2048 seeds):
+    // about 4 sqrt(N / (K + 1)).  Scratch is sized for twice that so that fs_set_batch can raise it.
+    const int Pdef = batch_default_seeds(sim->N, sim->K);
+    const int P = std::min<int>(BT_PMAX, 2 * Pdef);
     const size_t und = sizeof(BatchUndo) * (size_t)P * BT_LMAX * (size_t)(sim->Kp + 1);
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     const size_t o_ctl = take(sizeof(BatchCtl)), o_owner = take(4 * (size_t)sim->N), o_seeds = take(sizeof(BatchSeed) * BT_PMAX),
                  o_edges = take(2 * (size_t)BT_PMAX * BT_EMAX), o_ecount = take(BT_PMAX), o_npos = take(4 * (size_t)BT_PMAX),
                  o_elems = take(sizeof(BatchElem) * (size_t)P * BT_LMAX), o_undo = take(und),
-                 o_blocks = take(sizeof(BatchBlock) * BT_PMAX), o_clist = take(sizeof(BatchCommit) * (size_t)P * BT_LMAX);
+                 o_blocks = take(sizeof(BatchBlock) * BT_PMAX), o_clist = take(sizeof(BatchCommit) * (size_t)P * BT_LMAX),
+                 o_cand = take(4 * (size_t)sim->N), o_cbits = take(4 * (size_t)((sim->N + 31) / 32));
     if (cudaMalloc(&sim->bt_mem, o) != cudaSuccess) { cudaGetLastError(); sim->bt_mem = nullptr; return FS_OK; }
     unsigned char* b = (unsigned char*)sim->bt_mem;
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
@@ -1676,12 +1685,12 @@ int setup_batch(fs_sim* sim) {
     a.ctl = (BatchCtl*)(b + o_ctl); a.owner = (unsigned*)(b + o_owner); a.seeds = (BatchSeed*)(b + o_seeds);
     a.edges = (unsigned short*)(b + o_edges); a.ecount = b + o_ecount; a.npos = (int*)(b + o_npos);
     a.elems = (BatchElem*)(b + o_elems); a.undo = (BatchUndo*)(b + o_undo); a.blocks = (BatchBlock*)(b + o_blocks);
-    a.clist = (BatchCommit*)(b + o_clist);
+    a.clist = (BatchCommit*)(b + o_clist); a.cand = (int*)(b + o_cand); a.cbits = (unsigned*)(b + o_cbits);
     if (cudaMemsetAsync(a.ctl, 0, sizeof(BatchCtl), sim->stream) != cudaSuccess ||
         cudaMemsetAsync(a.owner, 0xff, 4 * (size_t)sim->N, sim->stream) != cudaSuccess) {
         cudaGetLastError(); cudaFree(sim->bt_mem); sim->bt_mem = nullptr; return FS_OK;
     }
-    sim->bt_P = P; sim->bt_seq = 64; sim->bt_grid = sim->sm_count; sim->bt_ok = true;
+    sim->bt_P = Pdef; sim->bt_alloc = P; sim->bt_seq = 64; sim->bt_grid = sim->sm_count; sim->bt_ok = true;
     return FS_OK;
 }
 
@@ -1977,6 +1986,14 @@ int fs_debug_stencil_shape(fs_sim* sim, int nw, int rs) {
 }
 #endif
 
+#ifdef FS_DEBUG_API
+int fs_debug_batch_knobs(fs_sim* sim, int max_chain, int min_commit) {
+    if (!sim) return -1;
+    sim->bt_max_chain = std::max(1, std::min(max_chain, (int)BT_LMAX)); sim->bt_min_commit = min_commit;
+    return FS_OK;
+}
+#endif
+
 #ifdef FS_BATCH_PROFILE
 int fs_debug_batch_profile(fs_sim* sim, long long* out12) {
     CUDA_TRY(cudaDeviceSynchronize());
@@ -1999,9 +2016,7 @@ int fs_set_batch(fs_sim* sim, int32_t max_seeds, int32_t seq_threshold) {
     if (max_seeds < 0 || max_seeds > BT_PMAX || seq_threshold < 0) return fail(FS_ERR_ARG, "max_seeds must be in [0, %d], seq_threshold >= 0", BT_PMAX);
     if (max_seeds > 0 && !sim->bt_ok) return fail(FS_ERR_ARG, "batched flips unavailable for this simulation (needs R = 1, 1 <= K <= 64, N >= 16384)");
     if (sim->bt_ok) {
-        const int64_t cap = sim->N / (8 * (int64_t)(sim->K + 1));
-        const int alloc = (int)std::max<int64_t>(64, std::min<int64_t>(BT_PMAX, cap));
-        sim->bt_P = std::min<int>(max_seeds, alloc);
+        sim->bt_P = std::min<int>(max_seeds, sim->bt_alloc);
         sim->bt_seq = seq_threshold;
     }
     return FS_OK;
