@@ -377,6 +377,47 @@ def paper_workloads(B, torch):
     return out
 
 
+def phase_profile():
+    """Per-phase budgets of the two relax kernels from an instrumented build of the same sources (see build.build_profile):
+    config 4, k_relax_batch rounds (ns per phase, CTA 0) and k_relax alone (cycles per flip and phase)."""
+    import ctypes as C
+    import tempfile
+    import torch
+    from paper_2002_11401_b200 import binding as B, build as bld
+    lib = bld.build_profile(tempfile.mkdtemp(prefix="fs_profile_"))
+    L = B.load_library(lib); B._lib = L
+    L.fs_debug_batch_profile.argtypes = [C.c_void_p, C.c_void_p]
+    L.fs_debug_relax_profile.argtypes = [C.c_void_p, C.c_int]
+    out = {}
+    w = W.config("4")
+    for mode in ("batched", "sequential"):
+        sim = B.Sim(w.pos, w.angle, w.hc, w.params); sim.set_thermal(w.sigma_th, w.thermal_seed)
+        if mode == "sequential":
+            sim.set_batch(0)
+        sim.update_fields()
+        z = (C.c_longlong * 16)(); L.fs_debug_relax_profile(z, 1)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        for t, (hx, hy) in enumerate(w.fields):
+            sim.set_field(hx, hy, t); sim.relax(sync=False)
+        torch.cuda.synchronize(); wall = time.perf_counter() - t0
+        st = sim.batch_stats()
+        row = {"sweep_wall_s": wall, "batch": st}
+        if mode == "batched":
+            p = (C.c_longlong * 12)(); L.fs_debug_batch_profile(sim.h, p)
+            names = ["1 threshold (histogram over the candidate list, theta)", "2 seeds (compaction)", "3 claims", "4 conflict edges",
+                     "5 components (labels)", "6 local relaxation (CTA 0's own warps)", "6b wait for the slowest component",
+                     "7 cut, commit / undo", "8 merged order -> flip log"]
+            row["us_per_round"] = {n: p[k] / 1e3 / max(st["rounds"], 1) for k, n in enumerate(names)}
+        r = (C.c_longlong * 16)(); L.fs_debug_relax_profile(r, 1)
+        nfl = max(r[15], 1)
+        row["k_relax_cycles_per_flip"] = {"flips": int(r[15]), "top arg-max (+ prefetch engines)": r[0] / nfl, "update (row, state, margins)": r[1] / nfl,
+                                          "barrier 1": r[2] / nfl, "leaf repair + groups + supergroups": r[3] / nfl, "of which leaf rescan": r[5] / nfl,
+                                          "barrier 2": r[4] / nfl}
+        out[mode] = row
+        sim.close()
+    print(json.dumps({"phase_profile": out, "workload": w.name, "source_hash": kernel_source_hash()}), flush=True)
+
+
 def max_over_ranks(dist, values_ms, device):
     """Replicas only: every rank times its own replica; the job's time is the slowest rank's."""
     import torch
@@ -572,12 +613,16 @@ def main():
     ap.add_argument("--scale", type=int, default=None, help="debug: lattice size override for config 5")
     ap.add_argument("--relax-scale", type=int, default=None, help="debug: lattice size override for config 4")
     ap.add_argument("--no-relax", action="store_true")
+    ap.add_argument("--phase-profile", action="store_true", help="instrumented build: per-phase budgets of k_relax_batch / k_relax on config 4")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.phase_profile:
+        if rank == 0:
+            phase_profile()
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, world, local_rank)

@@ -31,5 +31,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_profile(out_dir: str) -> str:
+    """The same sources with the phase timers compiled in (-DFS_RELAX_PROFILE -DFS_BATCH_PROFILE): clock64 / %globaltimer
+    per phase of k_relax and k_relax_batch, read back through fs_debug_relax_profile / fs_debug_batch_profile.
+    Used by `bench.py --phase-profile` only; the shipped library has none of it."""
+    os.makedirs(out_dir, exist_ok=True)
+    lib = os.path.join(out_dir, "libflatspin_b200_profile.so")
+    cmd = [nvcc_path()] + NVCC_FLAGS + ["-DFS_RELAX_PROFILE", "-DFS_BATCH_PROFILE", "-I", os.path.join(ROOT, "include"), SRC, "-o", lib]
+    subprocess.check_call(cmd)
+    return lib
+
+
 if __name__ == "__main__":
     print(build(force=True, verbose=True))
