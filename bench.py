@@ -410,9 +410,10 @@ def phase_profile():
             row["us_per_round"] = {n: p[k] / 1e3 / max(st["rounds"], 1) for k, n in enumerate(names)}
         r = (C.c_longlong * 16)(); L.fs_debug_relax_profile(r, 1)
         nfl = max(r[15], 1)
-        row["k_relax_cycles_per_flip"] = {"flips": int(r[15]), "top arg-max (+ prefetch engines)": r[0] / nfl, "update (row, state, margins)": r[1] / nfl,
+        if mode == "sequential":
+            row["k_relax_cycles_per_flip"] = {"flips": int(r[15]), "top arg-max (+ prefetch engines)": r[0] / nfl, "update (row, state, margins)": r[1] / nfl,
                                           "barrier 1": r[2] / nfl, "leaf repair + groups + supergroups": r[3] / nfl, "of which leaf rescan": r[5] / nfl,
-                                          "barrier 2": r[4] / nfl}
+                                              "barrier 2": r[4] / nfl}
         out[mode] = row
         sim.close()
     print(json.dumps({"phase_profile": out, "workload": w.name, "source_hash": kernel_source_hash()}), flush=True)
