@@ -519,6 +519,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
         BT_PROF(7);
         // ================= phase 8: merged order -> flip log =================================================
         const int nc = (int)__ldcg(&g->n_commit[rot]);
+        const long long logbase = nflips % a.log_cap;                             // ring buffer, like k_relax (nc < log_cap)
         for (int q = gwarp; q < nc; q += nwarps) {
             const BatchCommit me = a.clist[q];
             int rank = 0;
@@ -527,7 +528,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                 rank += (o.nev < me.nev || (o.nev == me.nev && o.lo < me.lo)) ? 1 : 0;
             }
             rank = __reduce_add_sync(0xffffffffu, rank);
-            if (lane == 0) a.flog[(nflips + rank) % a.log_cap] = me.k;       // ring buffer, like k_relax
+            if (lane == 0) { long long lp = logbase + rank; if (lp >= a.log_cap) lp -= a.log_cap; a.flog[lp] = me.k; }
         }
         BT_PROF(8);
         nflips += nc;
