@@ -67,8 +67,13 @@ enum { FS_FIELD_TOTAL = 0, FS_FIELD_DIP = 1, FS_FIELD_EXT = 2, FS_FIELD_THERMAL 
  *       FP64-pipe bound).  FS_ERR_ARG if the geometry is not a verified regular lattice.  Where the table has an
  *       exact inversion pairing (Eq. 3 is even in r_ij: T[d] == T[-d], bit for bit) the kernel adds the two
  *       spins of a slot pair first: 3 FP64 operations per 2 interactions instead of 4;
- *   3 = lattice stencil without the inversion pairing (one DFMA pair per interaction). */
-enum { FS_GATHER_AUTO = 0, FS_GATHER_ELL_F64 = 1, FS_GATHER_STENCIL = 2, FS_GATHER_STENCIL_PLAIN = 3 };
+ *   3 = lattice stencil without the inversion pairing (one DFMA pair per interaction);
+ *   4 = the OPTIONAL fp32 field path (BASELINE.json north_star: "reported separately at 1e-5"): the same stencil
+ *       kernel in single precision (couplings rounded to fp32, fp32 accumulation), h_dip stored as double.  Fields
+ *       agree with the fp64 paths to ~1e-6 relative to max|h|; spin / flip-order parity is NOT claimed after it (the
+ *       decision gaps of the relaxation are far below fp32 resolution).  Never chosen automatically.  FS_ERR_ARG unless
+ *       the geometry is a verified lattice whose table fits constant memory. */
+enum { FS_GATHER_AUTO = 0, FS_GATHER_ELL_F64 = 1, FS_GATHER_STENCIL = 2, FS_GATHER_STENCIL_PLAIN = 3, FS_GATHER_STENCIL_F32 = 4 };
 
 /* Why the stencil is not available (fs_get_lattice info[1]); 0 = it is. */
 enum {
@@ -140,6 +145,8 @@ int fs_get_lattice(const fs_sim* sim, int32_t* info, double* dinfo);
 /* Calibration for the FP64 roofline: runs a chain of dependent-free DFMAs on every SM and
  * returns the best of 4 timed launches in DFMA/s (HOST).  Synchronises `stream`. */
 int fs_measure_fp64_peak(double* dfma_per_s, void* stream);
+/* The same for fp32 FFMA/s (denominator of the optional fp32 field path's roofline). */
+int fs_measure_fp32_peak(double* ffma_per_s, void* stream);
 
 /* Full dipolar-field gather h_dip,i = sum_k s[nbr[i][k]] * w[i][k] for every spin (Eq. 3 over the
  * neighbourhood).  Asynchronous. */

@@ -16,7 +16,7 @@ from . import build as _build
 
 FS_OK, FS_ERR_ARG, FS_ERR_COINCIDENT, FS_ERR_WORKSPACE, FS_ERR_CUDA, FS_ERR_MAXFLIPS = 0, -1, -2, -3, -4, -5
 FIELD_TOTAL, FIELD_DIP, FIELD_EXT, FIELD_THERMAL = 0, 1, 2, 3
-GATHER_AUTO, GATHER_ELL_F64, GATHER_STENCIL, GATHER_STENCIL_PLAIN = 0, 1, 2, 3
+GATHER_AUTO, GATHER_ELL_F64, GATHER_STENCIL, GATHER_STENCIL_PLAIN, GATHER_STENCIL_F32 = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "fs_workspace_bytes", "fs_create", "fs_create_ensemble", "fs_destroy", "fs_get_info", "fs_set_spins",
@@ -80,6 +80,7 @@ def load_library(path: str | None = None):
         "fs_set_local_field": [vp, vp],
         "fs_sweep_anneal": [vp, vp, vp, i32, C.c_uint32, vp, i64, vp],
         "fs_measure_fp64_peak": [P(dbl), vp],
+        "fs_measure_fp32_peak": [P(dbl), vp],
         "fs_set_batch": [vp, i32, i32],
         "fs_sweep_ex": [vp, vp, vp, vp, vp, i32, C.c_uint32, vp, i64, vp],
         "fs_correlation": [vp, dbl, i32, vp, vp],
@@ -114,6 +115,15 @@ def measure_fp64_peak(stream=None) -> float:
     v = C.c_double()
     sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     _check(L, L.fs_measure_fp64_peak(C.byref(v), sp))
+    return float(v.value)
+
+
+def measure_fp32_peak(stream=None) -> float:
+    """FFMA/s of the FFMA-chain calibration kernel (denominator of the optional fp32 field path)."""
+    L = load_library()
+    v = C.c_double()
+    sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    _check(L, L.fs_measure_fp32_peak(C.byref(v), sp))
     return float(v.value)
 
 

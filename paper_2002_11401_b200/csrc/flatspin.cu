@@ -1044,6 +1044,7 @@ struct fs_sim {
     uint8_t* lat_sub = nullptr; int *lat_cu = nullptr, *lat_cv = nullptr;
     sgcell_t* sgrid = nullptr; int* cellidx = nullptr; bool sgrid_valid = false;
     int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
+    float2* Tf = nullptr;           // fp32 copy of T (the optional fp32 field path)
     int st_nw = 4, st_rs = 1, st_pv = 0, st_ov = ST_OV; size_t st_smem = 0; bool st_ct = false;
     bool st_sym = false;            // inversion-paired stencil (c_prow / c_pstart tables below, host copies: they are tiny)
     std::vector<int4> prow; std::vector<int2> pstart; std::vector<int> ptofs, rtofs;
@@ -1214,15 +1215,19 @@ int do_gather_stencil(fs_sim* sim) {
         if (threads <= 128) FS_LAUNCH_STENCIL1(128, 7, CTV, 8);                                     \
         else FS_LAUNCH_STENCIL1(256, 3, CTV, 8);                                                    \
     } while (0)
+    const bool f32 = sim->gather_variant == FS_GATHER_STENCIL_F32;
     if (sim->st_ct) {
-        // the constant-memory table is shared by all simulations of the process: take it over if needed
+        // the constant-memory table is shared by all simulations of the process (and by the fp64 / fp32 formats of one
+        // simulation): take it over if needed
         std::lock_guard<std::mutex> lock(g_ct_mutex);
         unsigned long long& g_ct_owner = g_ct_owner_dev[sim->device & 63];
         cudaEvent_t& g_ct_event = g_ct_event_dev[sim->device & 63];
-        if (g_ct_owner != sim->st_id) {
+        const unsigned long long want = 2 * sim->st_id + (f32 ? 1 : 0);
+        if (g_ct_owner != want) {
             if (g_ct_event) CUDA_TRY(cudaStreamWaitEvent(sim->stream, g_ct_event, 0));   // previous owner's kernels first
-            CUDA_TRY(cudaMemcpyToSymbolAsync(c_T, sim->T, 16 * (size_t)g.nsub * g.nsub * g.W * g.H, 0,
-                                             cudaMemcpyDeviceToDevice, sim->stream));
+            const size_t nT = (size_t)g.nsub * g.nsub * g.W * g.H;
+            if (f32) CUDA_TRY(cudaMemcpyToSymbolAsync(c_T, sim->Tf, 8 * nT, 0, cudaMemcpyDeviceToDevice, sim->stream));
+            else CUDA_TRY(cudaMemcpyToSymbolAsync(c_T, sim->T, 16 * nT, 0, cudaMemcpyDeviceToDevice, sim->stream));
             CUDA_TRY(cudaMemcpyToSymbolAsync(c_rows, sim->rowtab, 8 * (size_t)g.nsub * g.nsub * g.W, 0,
                                              cudaMemcpyDeviceToDevice, sim->stream));
             CUDA_TRY(cudaMemcpyToSymbolAsync(c_rtofs, sim->rtofs.data(), 4 * sim->rtofs.size(), 0, cudaMemcpyHostToDevice, sim->stream));
@@ -1231,9 +1236,19 @@ int do_gather_stencil(fs_sim* sim) {
                 CUDA_TRY(cudaMemcpyToSymbolAsync(c_prow, sim->prow.data(), 16 * sim->prow.size(), 0, cudaMemcpyHostToDevice, sim->stream));
                 CUDA_TRY(cudaMemcpyToSymbolAsync(c_pstart, sim->pstart.data(), 8 * sim->pstart.size(), 0, cudaMemcpyHostToDevice, sim->stream));
             }
-            g_ct_owner = sim->st_id;
+            g_ct_owner = want;
         }
-        if (sim->st_sym && sim->gather_variant != FS_GATHER_STENCIL_PLAIN) {
+        const bool sym = sim->st_sym && sim->gather_variant != FS_GATHER_STENCIL_PLAIN;
+        if (f32) {
+#define FS_LAUNCH_F32(MAXT, MINB, SYMV)                                                                              \
+    do {                                                                                                             \
+        if (sim->st_pv == 64) k_gather_stencil<MAXT, MINB, true, 8, SYMV, 64, float><<<grid, threads, sim->st_smem, sim->stream>>>(FS_STENCIL_ARGS); \
+        else k_gather_stencil<MAXT, MINB, true, 8, SYMV, 128, float><<<grid, threads, sim->st_smem, sim->stream>>>(FS_STENCIL_ARGS);                  \
+    } while (0)
+            if (sym) { if (threads <= 128) FS_LAUNCH_F32(128, 7, true); else FS_LAUNCH_F32(256, 3, true); }
+            else { if (threads <= 128) FS_LAUNCH_F32(128, 7, false); else FS_LAUNCH_F32(256, 3, false); }
+#undef FS_LAUNCH_F32
+        } else if (sym) {
             if (threads <= 128) FS_LAUNCH_STENCIL_SYM(128, 5); else FS_LAUNCH_STENCIL_SYM(256, 2);
         } else
         FS_LAUNCH_STENCIL(true);
@@ -1512,11 +1527,12 @@ int detect_lattice(fs_sim* sim) {
     size_t slots = (size_t)nsub * nsub * wh;
     size_t o_gidx = 0, o_T = align_up(4 * (size_t)cells), o_owner = o_T + align_up(16 * slots),
            o_rows = o_owner + align_up(8 * slots), o_sg = o_rows + align_up(8 * (size_t)nsub * nsub * g.W),
-           o_cell = o_sg + align_up(sg_bytes), o_end = o_cell + align_up(4 * (size_t)N);
+           o_cell = o_sg + align_up(sg_bytes), o_tf = o_cell + align_up(4 * (size_t)N), o_end = o_tf + align_up(8 * slots);
     CUDA_TRY(cudaMalloc(&sim->st_mem, o_end));
     unsigned char* sb = (unsigned char*)sim->st_mem;
     sim->gidx = (int*)(sb + o_gidx); sim->T = (double2*)(sb + o_T); sim->owner = (unsigned long long*)(sb + o_owner);
     sim->rowtab = (int2*)(sb + o_rows); sim->sgrid = (sgcell_t*)(sb + o_sg); sim->cellidx = (int*)(sb + o_cell);
+    sim->Tf = (float2*)(sb + o_tf);
     CUDA_TRY(cudaMemsetAsync(sim->sgrid, 0, sg_bytes, st));
     CUDA_TRY(cudaMemsetAsync(sim->gidx, 0xff, 4 * (size_t)cells, st));
     CUDA_TRY(cudaMemsetAsync(sim->T, 0, 16 * slots, st));
@@ -1528,6 +1544,7 @@ int detect_lattice(fs_sim* sim) {
                                              sim->owner, sim->T, scr64 + 1); LAUNCHED();
     }
     k_stencil_rows<<<(nsub * nsub * g.W + 127) / 128, 128, 0, st>>>(g, sim->owner, sim->rowtab); LAUNCHED();
+    k_table_f32<<<(unsigned)((slots + 255) / 256), 256, 0, st>>>((int)slots, sim->T, sim->Tf); LAUNCHED();
     k_stencil_count<<<nb256, 256, 0, st>>>(N, g, sim->lat_sub, sim->lat_cu, sim->lat_cv, sim->gidx, sim->owner, scr64 + 2); LAUNCHED();
     int flags = 0; unsigned long long res64[3];
     CUDA_TRY(cudaMemcpyAsync(&flags, scr, 4, cudaMemcpyDeviceToHost, st));
@@ -1556,6 +1573,14 @@ int detect_lattice(fs_sim* sim) {
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, false, 128>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, false, 8, false, 128>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, false, 8, false, 128>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, true, 64, float>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, true, 64, float>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, false, 64, float>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, false, 64, float>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, true, 128, float>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, true, 128, float>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, false, 128, float>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, false, 128, float>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 5, true, 8, true, 64>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 2, true, 8, true, 64>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 5, true, 8, true, 128>, stb));
@@ -1927,7 +1952,9 @@ int fs_set_local_field(fs_sim* sim, const double* h_dev) {
 int fs_set_gather_variant(fs_sim* sim, int variant) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
     DeviceGuard guard_(sim->device);
-    if (variant < 0 || variant > 3) return fail(FS_ERR_ARG, "unknown gather variant %d", variant);
+    if (variant < 0 || variant > 4) return fail(FS_ERR_ARG, "unknown gather variant %d", variant);
+    if (variant == FS_GATHER_STENCIL_F32 && !(sim->stencil_ok && sim->st_ct))
+        return fail(FS_ERR_ARG, "fp32 stencil gather unavailable (needs a verified lattice whose table fits constant memory)");
     if ((variant == FS_GATHER_STENCIL || variant == FS_GATHER_STENCIL_PLAIN) && !sim->stencil_ok)
         return fail(FS_ERR_ARG, "stencil gather unavailable for this geometry (FS_LATTICE reason %d)", sim->stencil_reason);
     sim->gather_variant = variant;
@@ -1972,6 +1999,33 @@ int fs_measure_fp64_peak(double* dfma_per_s, void* stream) {
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
     CUDA_TRY(cudaGetLastError());
     *dfma_per_s = best;
+    return FS_OK;
+}
+
+int fs_measure_fp32_peak(double* ffma_per_s, void* stream) {
+    if (!ffma_per_s) return fail(FS_ERR_ARG, "null pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float* sink = nullptr;
+    CUDA_TRY(cudaMalloc(&sink, 8));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 1 << 15, blocks = sms * 8, threads = 256;
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, st);
+        k_ffma_peak<<<blocks, threads, 0, st>>>(iters, 1.0f + rep, sink); LAUNCHED();
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+        double rate = 8.0 * iters * (double)blocks * threads / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    CUDA_TRY(cudaGetLastError());
+    *ffma_per_s = best;
     return FS_OK;
 }
 

@@ -248,7 +248,24 @@ __constant__ int2 c_pstart[NSUB_MAX * NSUB_MAX];
 __constant__ int c_rtofs[CR_MAX];
 __constant__ int c_ptofs[CP_MAX];
 
-template <int MAXT, int MINB, bool CT, int OV, bool SYM, int PU>
+// scalar helpers of the stencil kernel: R = double (the parity path) or float (the optional fp32 field path of
+// BASELINE.json north_star, reported separately at 1e-5; it converts the spin cells while staging them and reads a
+// float2 copy of the table through the same constant array)
+template <typename R> __device__ __forceinline__ R st_cell(sgcell_t c);
+template <> __device__ __forceinline__ double st_cell<double>(sgcell_t c) { return __hiloint2double((int)c, 0); }
+template <> __device__ __forceinline__ float st_cell<float>(sgcell_t c) { return __uint_as_float(c); }
+template <typename R> struct StPair { R x, y; };
+template <typename R> __device__ __forceinline__ StPair<R> ct_load(int i);
+template <> __device__ __forceinline__ StPair<double> ct_load<double>(int i) { const double2 t = c_T[i]; return StPair<double>{t.x, t.y}; }
+template <> __device__ __forceinline__ StPair<float> ct_load<float>(int i) {
+    const float2 t = reinterpret_cast<const float2*>(c_T)[i]; return StPair<float>{t.x, t.y};
+}
+__device__ __forceinline__ double st_fma(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float st_fma(float a, float b, float c) { return fmaf(a, b, c); }
+// the high word of +-1.0 / 0 as a double -> the bits of +-1.0f / 0
+__device__ __forceinline__ unsigned cell_to_f32(unsigned c) { return (c & 0x80000000u) | (c ? 0x3f800000u : 0u); }
+
+template <int MAXT, int MINB, bool CT, int OV, bool SYM, int PU, typename R = double>
 __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGrid g, int NW, int Pv,
                                                                const int* __restrict__ gidx, const sgcell_t* __restrict__ sg,
                                                                const double2* __restrict__ T, const int2* __restrict__ rowtab,
@@ -257,6 +274,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     const int RS = (blockDim.x >> 5) / NW, TV = OV * NW;
     const int SUc = (ST_TU + 2 * g.Ru + 3) & ~3, SH = TV + 2 * g.Rv, WH = g.W * g.H;   // staged row: SUc cells, pitch PU
     (void)Pv;
+    constexpr bool F32 = sizeof(R) == 4;
+    static_assert(!F32 || CT, "the fp32 variant reads its table from constant memory");
     double2* Tsm = reinterpret_cast<double2*>(st_raw);                      // [nsub][WH]
     const size_t tsm_n = CT ? 0 : (size_t)g.nsub * WH;                      // no shared copy of T in the CT variant
     int2* rows = reinterpret_cast<int2*>(Tsm + tsm_n);                      // [nsub][W]
@@ -280,7 +299,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
             const sgcell_t* srcj = src + (int64_t)sj * g.Vpa * g.Upa;
             for (int t = threadIdx.x; t < SH * CPR; t += blockDim.x) {
                 const int vl = t / CPR, ch = t % CPR;                 // CPR is a power of two
-                if (ch < nch) cp_async16(dst + (size_t)vl * PU + 4 * ch, srcj + (int64_t)vl * g.Upa + 4 * ch);
+                if (ch < nch) {
+                    if (F32) {                                        // staged through registers: cells become float bits
+                        uint4 v = __ldg(reinterpret_cast<const uint4*>(srcj + (int64_t)vl * g.Upa + 4 * ch));
+                        v.x = cell_to_f32(v.x); v.y = cell_to_f32(v.y); v.z = cell_to_f32(v.z); v.w = cell_to_f32(v.w);
+                        *reinterpret_cast<uint4*>(dst + (size_t)vl * PU + 4 * ch) = v;
+                    } else cp_async16(dst + (size_t)vl * PU + 4 * ch, srcj + (int64_t)vl * g.Upa + 4 * ch);
+                }
             }
         }
     }
@@ -295,15 +320,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     cp_async_wait_all();
     __syncthreads();
 
-    double ax[OV], ay[OV], x[OV];                      // all indices below are compile-time after unrolling: registers
+    R ax[OV], ay[OV], x[OV];                           // all indices below are compile-time after unrolling: registers
 #pragma unroll
-    for (int q = 0; q < OV; ++q) { ax[q] = 0.0; ay[q] = 0.0; }
-#define FS_ST_LD(K) __hiloint2double((int)sp[(K) * PU], 0)
-#define FS_ST_LDM(K) __hiloint2double((int)sm[(K) * PU], 0)
+    for (int q = 0; q < OV; ++q) { ax[q] = (R)0; ay[q] = (R)0; }
+#define FS_ST_LD(K) st_cell<R>(sp[(K) * PU])
+#define FS_ST_LDM(K) st_cell<R>(sm[(K) * PU])
 
     if (SYM) {
         // one slot of every inversion pair: window x slides forward along row+, window y backward along row-
-        double y[OV];
+        R y[OV];
         for (int sj = 0; sj < g.nsub; ++sj) {
             const sgcell_t* Sj = S + ((size_t)sj * SH + warp * OV + g.Rv) * PU + lane;
             const int2 ps = c_pstart[si * g.nsub + sj];
@@ -320,12 +345,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
                 for (; n >= OV; n -= OV, sp += OV * PU, sm -= OV * PU, tofs += OV) {
 #pragma unroll
                     for (int K = 0; K < OV; ++K) {
-                        const double2 t = c_T[tofs + K];
+                        const StPair<R> t = ct_load<R>(tofs + K);
 #pragma unroll
                         for (int q = 0; q < OV; ++q) {
-                            const double z = x[(q + K) % OV] + y[(q - K + OV) % OV];
-                            ax[q] = fma(z, t.x, ax[q]);
-                            ay[q] = fma(z, t.y, ay[q]);
+                            const R z = x[(q + K) % OV] + y[(q - K + OV) % OV];
+                            ax[q] = st_fma(z, t.x, ax[q]);
+                            ay[q] = st_fma(z, t.y, ay[q]);
                         }
                         x[K] = FS_ST_LD(OV + K);
                         y[OV - 1 - K] = FS_ST_LDM(-(K + 1));
@@ -334,12 +359,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
                 if (n > 0) {
 #pragma unroll
                     for (int K = 0; K < OV - 1; ++K) {
-                        const double2 t = c_T[tofs + K];
+                        const StPair<R> t = ct_load<R>(tofs + K);
 #pragma unroll
                         for (int q = 0; q < OV; ++q) {
-                            const double z = x[(q + K) % OV] + y[(q - K + OV) % OV];
-                            ax[q] = fma(z, t.x, ax[q]);
-                            ay[q] = fma(z, t.y, ay[q]);
+                            const R z = x[(q + K) % OV] + y[(q - K + OV) % OV];
+                            ax[q] = st_fma(z, t.x, ax[q]);
+                            ay[q] = st_fma(z, t.y, ay[q]);
                         }
                         if (--n == 0) break;
                         x[K] = FS_ST_LD(OV + K);
@@ -370,11 +395,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
             for (; n >= OV; n -= OV, sp += OV * PU, tp += OV, tofs += OV) {
 #pragma unroll
                 for (int K = 0; K < OV; ++K) {
-                    const double2 t = CT ? c_T[tofs + K] : tp[K];
+                    StPair<R> t;
+                    if (CT) t = ct_load<R>(tofs + K); else { const double2 tt = tp[K]; t = StPair<R>{(R)tt.x, (R)tt.y}; }
 #pragma unroll
                     for (int q = 0; q < OV; ++q) {
-                        ax[q] = fma(x[(q + K) % OV], t.x, ax[q]);
-                        ay[q] = fma(x[(q + K) % OV], t.y, ay[q]);
+                        ax[q] = st_fma(x[(q + K) % OV], t.x, ax[q]);
+                        ay[q] = st_fma(x[(q + K) % OV], t.y, ay[q]);
                     }
                     x[K] = FS_ST_LD(OV + K);
                 }
@@ -382,11 +408,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
             if (n > 0) {                               // ragged tail: at most OV - 1 slots
 #pragma unroll
                 for (int K = 0; K < OV - 1; ++K) {
-                    const double2 t = CT ? c_T[tofs + K] : tp[K];
+                    StPair<R> t;
+                    if (CT) t = ct_load<R>(tofs + K); else { const double2 tt = tp[K]; t = StPair<R>{(R)tt.x, (R)tt.y}; }
 #pragma unroll
                     for (int q = 0; q < OV; ++q) {
-                        ax[q] = fma(x[(q + K) % OV], t.x, ax[q]);
-                        ay[q] = fma(x[(q + K) % OV], t.y, ay[q]);
+                        ax[q] = st_fma(x[(q + K) % OV], t.x, ax[q]);
+                        ay[q] = st_fma(x[(q + K) % OV], t.y, ay[q]);
                     }
                     if (--n == 0) break;
                     x[K] = FS_ST_LD(OV + K);
@@ -399,8 +426,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     // ---- epilogue: add the row groups' partial sums (fixed order), scatter the OV outputs to their spins
     if (RS > 1) {
         __syncthreads();                               // everyone is done with the tiles
-        double* red_base = reinterpret_cast<double*>(S);
-        double* red = red_base + ((size_t)((rs - 1) * NW + warp) * 2 * OV) * 32 + lane;
+        R* red_base = reinterpret_cast<R*>(S);
+        R* red = red_base + ((size_t)((rs - 1) * NW + warp) * 2 * OV) * 32 + lane;
         if (rs > 0) {
 #pragma unroll
             for (int q = 0; q < OV; ++q) { red[(2 * q) * 32] = ax[q]; red[(2 * q + 1) * 32] = ay[q]; }
@@ -408,7 +435,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
         __syncthreads();
         if (rs > 0) return;
         for (int k = 1; k < RS; ++k) {
-            const double* rd = red_base + ((size_t)((k - 1) * NW + warp) * 2 * OV) * 32 + lane;
+            const R* rd = red_base + ((size_t)((k - 1) * NW + warp) * 2 * OV) * 32 + lane;
 #pragma unroll
             for (int q = 0; q < OV; ++q) { ax[q] += rd[(2 * q) * 32]; ay[q] += rd[(2 * q + 1) * 32]; }
         }
@@ -418,8 +445,26 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
 #pragma unroll
     for (int q = 0; q < OV; ++q) {
         const int i = oi[q * 32];
-        if (i >= 0) hdip[i] = make_double2(ax[q], ay[q]);
+        if (i >= 0) hdip[i] = make_double2((double)ax[q], (double)ay[q]);
     }
+}
+
+__global__ void k_table_f32(int n, const double2* __restrict__ T, float2* __restrict__ Tf) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n) { const double2 v = T[t]; Tf[t] = make_float2((float)v.x, (float)v.y); }
+}
+
+// FFMA-chain calibration of the fp32 roofline denominator (the optional fp32 field path)
+__global__ void k_ffma_peak(int iters, float seed, float* __restrict__ sink) {
+    float a0 = seed, a1 = seed + 1, a2 = seed + 2, a3 = seed + 3, a4 = seed + 4, a5 = seed + 5, a6 = seed + 6, a7 = seed + 7;
+    const float m = 1.0000001f, c = 1e-9f * threadIdx.x;
+#pragma unroll 4
+    for (int k = 0; k < iters; ++k) {
+        a0 = fmaf(a0, m, c); a1 = fmaf(a1, m, c); a2 = fmaf(a2, m, c); a3 = fmaf(a3, m, c);
+        a4 = fmaf(a4, m, c); a5 = fmaf(a5, m, c); a6 = fmaf(a6, m, c); a7 = fmaf(a7, m, c);
+    }
+    float r = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (r == 12345.678f) sink[0] = r;
 }
 
 // DFMA-chain calibration: every thread runs 8 independent chains of `iters` DFMAs.

@@ -1038,3 +1038,27 @@ def test_paper_square_anneal_ensemble(B):
     # annealing lowers the dipolar energy: more minimised nearest-neighbour pairs than in the random start
     o0 = Oracle(w.pos, w.angle, w.hc[0], w.params, spins=w.spins)
     assert sm[0][1] > o0.spin_correlation(0.5, 8)[0][1]
+
+
+# ------------------------------------------------------------------ optional fp32 field path (reported separately, 1e-5)
+@pytest.mark.parametrize("which,scale", [("1", None), ("3", 30), ("5", 40), ("2", 20)])
+def test_fp32_stencil_field_path(B, which, scale):
+    """BASELINE.json north_star: "an optional fp32 field path is reported separately at 1e-5".  The single-precision
+    stencil gather against the oracle's fp64 fields, relative to max|h|; it is never the automatic choice and no
+    flip-order claim is attached to it.  Kagome (no inversion pairing) exercises the unpaired fp32 kernel."""
+    w = W.config(which, scale=scale)
+    spins = W.random_spins(w.N, seed=21)
+    sim, orc = mk(B, w, spins=spins)
+    assert sim.lattice()["active"]
+    sim.set_gather_variant(B.GATHER_STENCIL_F32); sim.update_fields()
+    a = sim.get_fields(1).cpu().numpy()
+    ref = orc.fields(1)
+    err = field_err(a, ref)
+    assert 0 < err < 1e-5, err                          # single precision: not bit-equal to the fp64 path, well inside the bar
+    sim.set_gather_variant(B.GATHER_AUTO); sim.update_fields()
+    assert field_err(sim.get_fields(1).cpu().numpy(), ref) < FIELD_TOL        # and the fp64 table is back in place
+    # an irregular geometry has no fp32 path
+    pos = w.pos + 0.01 * np.random.default_rng(1).standard_normal(w.pos.shape)
+    sim2 = B.Sim(pos, w.angle, w.hc, w.params)
+    with pytest.raises(B.FlatspinError):
+        sim2.set_gather_variant(B.GATHER_STENCIL_F32)
