@@ -25,6 +25,7 @@ EXPORTS = [
     "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
     "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep", "fs_sweep_anneal", "fs_set_local_field",
     "fs_set_batch", "fs_get_batch_stats", "fs_sweep_ex", "fs_correlation", "fs_vertex_populations", "fs_get_flip_log_window",
+    "fs_measure_fp32_peak",
 ]
 
 
