@@ -419,6 +419,33 @@ def phase_profile():
     print(json.dumps({"phase_profile": out, "workload": w.name, "source_hash": kernel_source_hash()}), flush=True)
 
 
+def scan_probe():
+    """The fused scan alone at config-4 size (2,002,000 spins, thermal field on: Philox + Box-Muller per spin), L2 flushed
+    before every launch: the command `ncu -k regex:k_scan` is pointed at."""
+    import torch
+    from paper_2002_11401_b200 import binding as B
+    w = W.config("4")
+    sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+    sim.set_spins(w.spins); sim.set_thermal(w.sigma_th, w.thermal_seed)
+    hx, hy = w.fields[100]
+    sim.set_field(hx, hy, 100); sim.update_fields()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for _ in range(3):
+        sim.scan_async()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(10)]
+    for a, b in ev:
+        flush.fill_(1); a.record(); sim.scan_async(); b.record()
+    torch.cuda.synchronize()
+    ms = np.array([a.elapsed_time(b) for a, b in ev])
+    n_sw, best, bestL = sim.scan()
+    peak, _ = measured_peaks()
+    print(json.dumps({"scan_probe": {"workload": w.name, "N": w.N, "thermal": True, "scan_us_mean": 1e3 * float(ms.mean()),
+                                     "scan_us_min": 1e3 * float(ms.min()), "algorithmic_bytes": 49 * w.N,
+                                     "hbm_frac": 49 * w.N / (float(ms.mean()) * 1e-3) / 1e9 / peak,
+                                     "n_switchable": n_sw, "best_index": best, "source_hash": kernel_source_hash()}}), flush=True)
+    sim.close()
+
+
 def max_over_ranks(dist, values_ms, device):
     """Replicas only: every rank times its own replica; the job's time is the slowest rank's."""
     import torch
@@ -637,6 +664,7 @@ def main():
     ap.add_argument("--relax-scale", type=int, default=None, help="debug: lattice size override for config 4")
     ap.add_argument("--no-relax", action="store_true")
     ap.add_argument("--phase-profile", action="store_true", help="instrumented build: per-phase budgets of k_relax_batch / k_relax on config 4")
+    ap.add_argument("--scan-probe", action="store_true", help="k_scan alone at config-4 size with the thermal field (ncu target)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     args = ap.parse_args()
@@ -645,6 +673,9 @@ def main():
     if args.phase_profile:
         if rank == 0:
             phase_profile()
+    elif args.scan_probe:
+        if rank == 0:
+            scan_probe()
     elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
