@@ -1502,6 +1502,7 @@ int detect_lattice(fs_sim* sim) {
     CUDA_TRY(cudaStreamSynchronize(st));
     LatGrid g{};
     g.nsub = nsub; g.u0 = ext[0]; g.v0 = ext[1];
+    g.inv_nsub = (unsigned)(((1ull << 32) + nsub - 1) / nsub);
     int64_t U = (int64_t)ext[2] - ext[0] + 1, V = (int64_t)ext[3] - ext[1] + 1;
     g.Ru = ext[4]; g.Rv = ext[5];
     if (g.Ru > STENCIL_RMAX || g.Rv > STENCIL_RMAX) return lattice_fail(sim, FS_LATTICE_STENCIL_TOO_WIDE);

@@ -36,6 +36,7 @@ struct LatFrame { double ox, oy, i11, i12, i21, i22; };   // (u, v) = Ainv (r - 
 struct LatGrid {
     int nsub, u0, v0, U, V, Ru, Rv, Up, Vp, W, H;         // W = 2Ru+1, H = 2Rv+1, Up = U+2Ru, Vp = V+2Rv
     int Upa, Vpa;                                         // spin-grid allocation [Vpa][Upa] (u fastest): whole tiles + halo, Upa % 4 == 0
+    unsigned inv_nsub;                                    // ceil(2^32 / nsub): z / nsub == umulhi(z, inv_nsub) for z < 2^16, without a division
 };
 
 __device__ __forceinline__ void lat_uv(const LatFrame& f, double2 p, double& u, double& v) {
@@ -281,7 +282,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     int2* rows = reinterpret_cast<int2*>(Tsm + tsm_n);                      // [nsub][W]
     int* oidx = reinterpret_cast<int*>(rows + (size_t)g.nsub * g.W);        // [TV][32] spin index of every output
     sgcell_t* S = reinterpret_cast<sgcell_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 15) & ~(size_t)15));   // [nsub][SH][PU]
-    const int si = __shfl_sync(0xffffffffu, (int)(blockIdx.z % g.nsub), 0), rep = __shfl_sync(0xffffffffu, (int)(blockIdx.z / g.nsub), 0);
+    // No division: ptxas computes one in the vector datapath and, in some instantiations (fp32, 256-thread CTAs), then kept
+    // si, the row tables indexed with it and finally the weights in vector registers (LDC + three-vector-operand DFMA).
+    const int rep = g.nsub == 1 ? (int)blockIdx.z : (int)__umulhi(blockIdx.z, g.inv_nsub), si = (int)blockIdx.z - rep * g.nsub;
     const int tu0 = blockIdx.x * ST_TU, tv0 = blockIdx.y * TV;       // tile origin, interior coordinates
     // the warp index via a shuffle from lane 0: the compiler then knows everything derived from it is
     // warp-uniform
