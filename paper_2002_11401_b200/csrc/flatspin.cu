@@ -132,14 +132,16 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 __device__ __forceinline__ double2 thermal_xy(double sigma, uint64_t seed, uint32_t step, uint32_t i) {
     uint32_t x[4];
     philox4x32_10(i, step, 0u, 0u, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32), x);
-    uint64_t a = (((uint64_t)x[0] << 32) | x[1]) >> 12;
-    uint64_t b = (((uint64_t)x[2] << 32) | x[3]) >> 12;
-    const double two_m52 = 1.0 / 4503599627370496.0;
-    double u1 = ((double)a + 0.5) * two_m52;
-    double u2 = ((double)b + 0.5) * two_m52;
-    double r = sqrt(-2.0 * log(u1));
+    // u = (a + 1/2) 2^-52 with a = the top 52 bits: the bits of a are the mantissa of a double in [1, 2), so
+    // u = (1.a - 1) + 2^-53, both steps exact (no 64-bit integer-to-double conversion)
+    const double half_ulp = 1.0 / 9007199254740992.0;
+    const double u1 = (__hiloint2double((int)(0x3ff00000u | (x[0] >> 12)), (int)((x[0] << 20) | (x[1] >> 12))) - 1.0) + half_ulp;
+    const double u2 = (__hiloint2double((int)(0x3ff00000u | (x[2] >> 12)), (int)((x[2] << 20) | (x[3] >> 12))) - 1.0) + half_ulp;
+    const double r = sqrt(-2.0 * log(u1));
+    // cos / sin of 2 pi u2 by sincospi(2 u2): the angle's range reduction is exact and cheap; the result differs from
+    // cos(fl(2 pi u2)) by the rounding of that product (<= 7e-16 absolute), like every other few-ulp difference of D-3
     double sn, cs;
-    sincos(2.0 * CUDART_PI * u2, &sn, &cs);
+    sincospi(2.0 * u2, &sn, &cs);
     return make_double2(sigma * r * cs, sigma * r * sn);
 }
 
@@ -468,10 +470,12 @@ struct ScanGroup { double v; int idx; unsigned cnt; };  // result of one group o
 // uint32 words of scan scratch per replica: per-CTA counts, group tickets, group results
 __host__ __device__ inline size_t scan_aux_stride(int ncta) { return 4 * (size_t)ncta + 4; }   // one ScanGroup per CTA
 
-constexpr int SCAN_SPB = 1024;                          // consecutive spins per CTA = 1024 / LB leaves
+constexpr int SCAN_SPB_MIN = 512;                       // the smallest CTA span (sizes the per-CTA scratch)
 
-// THREADS x SPT = 1024: SPT spins per thread (independent load chains in flight)
-template <int SCAN_SPT>
+// THREADS x SPT = SCAN_SPB consecutive spins per CTA (= SCAN_SPB / LB leaves): SPT spins per thread (independent load
+// chains in flight).  1024 spins per CTA when a leaf is that large, else 512 (256-thread CTAs, four per SM: the CTA-wide
+// barrier of the leaf reduction was the largest stall of the 512-thread version, profiles/r02_scan_cfg4.md).
+template <int SCAN_SPT, int SCAN_SPB>
 __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB, Astroid ast, FieldSpec fs, int finalize,
                                                const double2* __restrict__ hext_all /*[R] (hx,hy)*/,
                                                const double2* __restrict__ cs, const double* __restrict__ hc_all,
@@ -479,7 +483,8 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
                                                double2* __restrict__ hfix_all, double* __restrict__ M_all,
                                                double* __restrict__ bval_all, int* __restrict__ bidx_all, int nblk,
                                                unsigned* __restrict__ scnt_all /*[R][gridDim.x]*/, Counters* __restrict__ ctr,
-                                               const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/) {
+                                               const double2* __restrict__ hloc /*[N] per-spin external field or NULL*/,
+                                               int set_field, double2 field /*fs_set_field's pending global field, by value*/) {
     __shared__ double wv[32];                            // arg-max of every 32-spin slot of this CTA
     __shared__ int wi[32];
     __shared__ int is_last;
@@ -488,7 +493,9 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     constexpr int SCAN_THREADS = SCAN_SPB / SCAN_SPT;
     const int64_t base = (int64_t)blockIdx.x * SCAN_SPB + threadIdx.x;
-    const double2 he = hext_all[r];
+    // fs_set_field launches nothing: its field arrives here by value, and one thread records it for the later readers
+    const double2 he = set_field ? field : hext_all[r];
+    if (set_field && blockIdx.x == 0 && threadIdx.x == 0) const_cast<double2*>(hext_all)[r] = field;
     // loads of all four spins first
     double2 c[SCAN_SPT], hd[SCAN_SPT]; double ih[SCAN_SPT], sp[SCAN_SPT];
 #pragma unroll
@@ -536,7 +543,8 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
     if (lane == 0) wcnt[w] = (unsigned)nsw;
     __syncthreads();
     if (w == 0) {
-        double v = wv[lane]; int bi = wi[lane];              // 32 slots of 32 spins
+        double v = lane < SCAN_SPB / 32 ? wv[lane] : -CUDART_INF;                  // SCAN_SPB / 32 slots of 32 spins
+        int bi = lane < SCAN_SPB / 32 ? wi[lane] : 0x7fffffff;
         warp_argmax_margin(v, bi);
         unsigned c = lane < SCAN_THREADS / 32 ? wcnt[lane] : 0u;
         c = __reduce_add_sync(0xffffffffu, c);
@@ -617,7 +625,7 @@ __device__ __forceinline__ void repair_group(int grp, int nblk, const mkey_t* bk
 #include "batch.cuh"
 
 template <int RELAX_THREADS>                           // 512 (one big system per CTA) or 128 (ensembles of small systems)
-__global__ void __launch_bounds__(RELAX_THREADS, RELAX_THREADS == 128 ? 8 : (RELAX_THREADS == 64 ? 16 : 1))
+__global__ void __launch_bounds__(RELAX_THREADS, RELAX_THREADS == 256 ? 4 : (RELAX_THREADS == 128 ? 8 : (RELAX_THREADS == 64 ? 16 : 1)))
 k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_flips, long long log_cap,
         const int* __restrict__ nbr, const double2* __restrict__ wT, const double* __restrict__ ihc_all,
         int8_t* __restrict__ s_all, double2* __restrict__ hdip_all, double2* __restrict__ hfix_all,
@@ -734,6 +742,15 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             if (!stop && max_flips > 0 && nflips - nflips0 >= max_flips) { stop = true; status = 1; }
             if (stop) k = -1;
             if (lane == 0) { sh_k = k; sh_stop = stop ? 1 + status : 0; sh_ntouched = 0; }
+        } else if (warp == 1 && one_warp && cellidx) {
+            // Keep the stencil gather's spin grid in step.  The cell index of k is a dependent global load: issued after the
+            // update barrier (as it was) it held the repair stage back by an L2 round trip; here an idle warp finds k itself
+            // (the same arg-max as warp 0, no barrier between the two) and is done long before the update is.
+            mkey_t v = lane < nsup ? skey[lane] : 0ull;
+            int kk = lane < nsup ? sidx[lane] : 0x7fffffff;
+            warp_argmax_key(v, kk);
+            if (lane == 0 && v > KEY_ONE && !(max_flips > 0 && nflips - nflips0 >= max_flips))
+                sgrid[(int64_t)r * sgrid_stride + cellidx[kk]] = (s[kk] > 0 ? SG_DOWN : SG_UP);   // s[k] is rewritten after the barrier
         } else if (warp >= PF_W0 && one_warp) {         // (with K + 1 > 32 every warp is needed for the update itself)
             // ---- prefetch engines (not on the critical path): the best spin of every 8th group is a likely
             // future flip.  Iteration n brings its ELL row to L2; iteration n+1 reads the row (an L2 hit by
@@ -770,6 +787,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         if (!one_warp) {
             __syncthreads();
             k = sh_k;
+            if (tid == RELAX_THREADS - 32 && cellidx && k >= 0)  // (the last warp has the smallest share of the update)
+                sgrid[(int64_t)r * sgrid_stride + cellidx[k]] = (s[k] > 0 ? SG_DOWN : SG_UP);
         }
         FS_PROF_T(c1);
         // ---- A8: flip k, update its neighbours incrementally, recompute their margins
@@ -832,8 +851,6 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             // critical path (this thread's warp rescans the first touched leaf next) and cost 0.4 us per flip
             flog[logpos] = sh_k; logpos = (logpos + 1 == log_cap) ? 0 : logpos + 1;
         }
-        if (tid == RELAX_THREADS - 32 && cellidx)           // keep the stencil gather's spin grid in step (an idle warp)
-            sgrid[(int64_t)r * sgrid_stride + cellidx[sh_k]] = (sh_sold > 0 ? SG_DOWN : SG_UP);
         // ---- A7 repair, level by level, one warp per touched leaf (duplicated group work is harmless)
         const int ntouched = sh_ntouched;
         for (int t = warp; t < ntouched; t += NW) {
@@ -1030,6 +1047,8 @@ struct fs_sim {
     bool fields_dirty = true;
     double sigma = 0.0; uint64_t seed = 0; uint32_t step = 0;
     double2* hext_host = nullptr;   // pinned staging [R]
+    bool field_pending = false;     // fs_set_field's value has not reached sim->hext yet: the next k_scan takes it by value
+    double2 field_value{};
     Counters* ctr_host = nullptr;   // pinned staging [R]
     double2* hloc = nullptr;        // per-spin external field [N] (library-owned), NULL = none
     int gather_variant = FS_GATHER_AUTO;
@@ -1107,7 +1126,7 @@ void layout_rest(Layout& L, int64_t N, int R, int Kp, int nblk, int64_t log_cap)
     L.bval = take(8 * (size_t)R * nblk);
     L.bidx = take(4 * (size_t)R * nblk);
     L.flog = take(4 * (size_t)R * log_cap);
-    L.scnt = take(4 * (size_t)R * scan_aux_stride((int)((N + 1023) / 1024)));
+    L.scnt = take(4 * (size_t)R * scan_aux_stride((int)((N + SCAN_SPB_MIN - 1) / SCAN_SPB_MIN)));
     L.ctr = take(sizeof(Counters) * (size_t)R);
     L.hext = take(16 * (size_t)R);
     L.total = o;
@@ -1609,18 +1628,31 @@ int ensure_fields(fs_sim* sim) { return sim->fields_dirty ? do_gather(sim) : FS_
 int do_scan(fs_sim* sim, bool finalize) {
     int rc = ensure_fields(sim);
     if (rc) return rc;
-    dim3 grid((unsigned)((sim->N + SCAN_SPB - 1) / SCAN_SPB), (unsigned)sim->R);
+    const int spb = sim->LB > 512 ? 1024 : 512;
+    dim3 grid((unsigned)((sim->N + spb - 1) / spb), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
 #define FS_SCAN_ARGS sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc, sim->s, sim->hdip, \
-                     sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr, sim->hloc
-    k_scan<2><<<grid, SCAN_SPB / 2, 0, sim->stream>>>(FS_SCAN_ARGS);
+                     sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr, sim->hloc, \
+                     sim->field_pending ? 1 : 0, sim->field_value
+    if (spb == 1024) k_scan<2, 1024><<<grid, 512, 0, sim->stream>>>(FS_SCAN_ARGS);
+    else k_scan<2, 512><<<grid, 256, 0, sim->stream>>>(FS_SCAN_ARGS);
+    sim->field_pending = false;
 #undef FS_SCAN_ARGS
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
     return FS_OK;
 }
 
+int flush_field(fs_sim* sim) {
+    if (!sim->field_pending) return FS_OK;
+    k_set_field<<<(sim->R + 127) / 128, 128, 0, sim->stream>>>(sim->R, sim->field_value.x, sim->field_value.y, sim->hext); LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    sim->field_pending = false;
+    return FS_OK;
+}
+
 int push_field(fs_sim* sim) {
+    sim->field_pending = false;
     CUDA_TRY(cudaMemcpyAsync(sim->hext, sim->hext_host, sizeof(double2) * sim->R, cudaMemcpyHostToDevice, sim->stream));
     return FS_OK;
 }
@@ -1641,6 +1673,9 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
     // 128-thread CTAs (8 per SM, 64 registers) instead of 512-thread ones (1 per SM); beyond 8 replicas per
     // SM, 64-thread CTAs (16 per SM).  Measured on 220-spin replicas: 75k / 421k / 539k replica-sweeps per s.
     const bool small_cta = sim->R > sim->sm_count && sim->Kp + 1 <= 32 && sim->nblk <= 1024;
+    // ensembles with more than 31 neighbours per spin (e.g. section IV.B: 592 replicas, K = 632): the loop is latency-bound,
+    // so several replicas per SM beat a wide CTA per replica: 256 threads (4 per SM), 128 from 8 replicas per SM
+    const bool mid_cta = sim->R > sim->sm_count && sim->Kp + 1 > 32 && sim->nblk <= 1024;
 #define FS_RELAX_ARGS sim->N, sim->Kp, lb_shift, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr, \
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr, \
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid, \
@@ -1648,6 +1683,8 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
         T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev, lscale_dev, lseries_dev, use_base
     if (small_cta && sim->R > 8 * sim->sm_count) k_relax<64><<<sim->R, 64, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else if (small_cta) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+    else if (mid_cta && sim->R >= 8 * sim->sm_count) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+    else if (mid_cta) k_relax<256><<<sim->R, 256, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else if (sim->Kp + 1 > 512) k_relax<1024><<<sim->R, 1024, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
     else k_relax<512><<<sim->R, 512, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
 #undef FS_RELAX_ARGS
@@ -1822,7 +1859,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     CREATE_TRY(cudaMemcpyAsync(sim->pos, pos_dev, 16 * (size_t)N, cudaMemcpyDeviceToDevice, st));
     CREATE_TRY(cudaMemcpyAsync(sim->hc, hc_dev, 8 * (size_t)R * N, cudaMemcpyDeviceToDevice, st));
     CREATE_TRY(cudaMemsetAsync(sim->ctr, 0, sizeof(Counters) * R, st));
-    CREATE_TRY(cudaMemsetAsync(sim->scnt, 0, 4 * (size_t)R * scan_aux_stride((int)((N + SCAN_SPB - 1) / SCAN_SPB)), st));
+    CREATE_TRY(cudaMemsetAsync(sim->scnt, 0, 4 * (size_t)R * scan_aux_stride((int)((N + SCAN_SPB_MIN - 1) / SCAN_SPB_MIN)), st));
     CREATE_TRY(cudaMemsetAsync(sim->hdip, 0, 16 * (size_t)R * N, st));
     CREATE_TRY(cudaMemcpyAsync(sim->hext, sim->hext_host, sizeof(double2) * R, cudaMemcpyHostToDevice, st));
     int nb = (int)((N + 255) / 256);
@@ -1852,6 +1889,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     sim->relax_smem = ((size_t)nblk + (size_t)(nblk + 31) / 32 + 8) * 12 + (size_t)(Kp + 1) * 4 + 32;
     CREATE_TRY(raise_smem_limit(k_relax<512>, sim->relax_smem));
     CREATE_TRY(raise_smem_limit(k_relax<128>, sim->relax_smem));
+    CREATE_TRY(raise_smem_limit(k_relax<256>, sim->relax_smem));
     CREATE_TRY(raise_smem_limit(k_relax<64>, sim->relax_smem));
     CREATE_TRY(raise_smem_limit(k_relax<1024>, sim->relax_smem));
     int hflags = 0;
@@ -1924,8 +1962,9 @@ int fs_set_field(fs_sim* sim, double hx, double hy, uint32_t step) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
     DeviceGuard guard_(sim->device);
     sim->step = step;
-    k_set_field<<<(sim->R + 127) / 128, 128, 0, sim->stream>>>(sim->R, hx, hy, sim->hext); LAUNCHED();   // by value: no host sync
-    CUDA_TRY(cudaGetLastError());
+    // no launch and no host sync: the next scan takes the value as a kernel argument (one launch less per field step);
+    // the few other readers of sim->hext call flush_field first
+    sim->field_pending = true; sim->field_value = make_double2(hx, hy);
     return FS_OK;
 }
 
@@ -2169,6 +2208,7 @@ int fs_sweep_ex(fs_sim* sim, const double* fields_dev, const double* sigma_dev, 
                       reinterpret_cast<const double2*>(local_series_dev));
     if (rc) return rc;
     sim->step = step0 + (uint32_t)(T - 1);
+    sim->field_pending = false;                          // the sweep left its own last field in sim->hext
     if (!n_flips_out) return FS_OK;
     rc = fetch_counters(sim);
     if (rc) return rc;
@@ -2206,6 +2246,7 @@ int fs_get_fields(fs_sim* sim, int which, double* h_dev_out) {
     DeviceGuard guard_(sim->device);
     if (which < 0 || which > 3) return fail(FS_ERR_ARG, "unknown field selector %d", which);
     if (which == FS_FIELD_TOTAL || which == FS_FIELD_DIP) { int rc = ensure_fields(sim); if (rc) return rc; }
+    { int rc = flush_field(sim); if (rc) return rc; }
     dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
     FieldSpec fsp{sim->sigma, sim->seed, sim->step};
     k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, which, fsp, sim->hext, sim->cs, sim->hdip, (double2*)h_dev_out, sim->hloc);

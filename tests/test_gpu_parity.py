@@ -1040,6 +1040,39 @@ def test_paper_square_anneal_ensemble(B):
     assert sm[0][1] > o0.spin_correlation(0.5, 8)[0][1]
 
 
+@pytest.mark.parametrize("R", [200, 1300])
+def test_many_replicas_with_more_than_31_neighbors(B, R):
+    """Ensembles whose update does not fit one warp (K + 1 > 32) and with more replicas than SMs: 256-thread CTAs
+    (four replicas per SM), 128-thread ones from eight replicas per SM; a sample of the replicas against independent
+    oracles, whole protocol in one launch and stepwise."""
+    from oracle import Oracle
+    w = W.config("3", scale=6)                              # pinwheel recipe, neighbor distance 3: K = 60 > 31
+    hc = W.coercive_fields(w.N, seed=77, replicas=R)
+    sim = B.Sim(w.pos, w.angle, hc, w.params)
+    assert sim.K + 1 > 32
+    fields = w.fields[::40]
+    sim.set_spins(np.ones((R, w.N), np.int8))
+    n, per = sim.sweep(fields, step0=0)
+    s = sim.get_spins().cpu().numpy(); per = per.cpu().numpy()
+    sample = sorted({0, 1, R // 2, R - 2, R - 1})
+    for r in sample:
+        o = Oracle(w.pos, w.angle, hc[r], w.params, spins=np.ones(w.N, np.int8))
+        cnt, logs = [], []
+        for t, (hx, hy) in enumerate(fields):
+            o.set_field(hx, hy, t)
+            c, log = o.relax_B()
+            cnt.append(c); logs.append(log)
+        assert np.array_equal(s[r], o.spins()), r
+        assert list(per[r]) == cnt and int(n[r]) == sum(cnt), r
+        assert np.array_equal(sim.get_flip_log(replica=r).cpu().numpy()[: int(n[r])], np.concatenate(logs)[: 4 * w.N + 1024]), r
+    assert int(n.sum()) > 0
+    # stepwise (fs_set_field_ensemble + fs_relax_ensemble) from the same start
+    sim.set_spins(np.ones((R, w.N), np.int8)); sim.update_fields()
+    for t, (hx, hy) in enumerate(fields):
+        sim.set_field(hx, hy, t); sim.relax_ensemble()
+    assert np.array_equal(sim.get_spins().cpu().numpy(), s)
+
+
 # ------------------------------------------------------------------ optional fp32 field path (reported separately, 1e-5)
 @pytest.mark.parametrize("which,scale", [("1", None), ("3", 30), ("5", 40), ("2", 20)])
 def test_fp32_stencil_field_path(B, which, scale):
