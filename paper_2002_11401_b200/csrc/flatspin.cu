@@ -145,7 +145,9 @@ __device__ __forceinline__ double2 thermal_xy(double sigma, uint64_t seed, uint3
     return make_double2(sigma * r * cs, sigma * r * sn);
 }
 
-struct Astroid { double inv_b, inv_c, e_par, e_perp; int k_par, k_perp; };   // 1/b, 1/c, 2/gamma, 2/beta, power kinds
+struct Astroid {           // 1/b, 1/c, 2/gamma, 2/beta, power kinds; tx, ty: both terms of Eq. 5 below 1/2 (see margin())
+    double inv_b, inv_c, e_par, e_perp; int k_par, k_perp; double tx, ty;
+};
 
 // x^e for x >= 0, e > 0.  kind 1: e = 2/3 (gamma or beta = 3, the classical astroid, Eq. 4)
 // -> cbrt(x^2); kind 2: e = 1; kind 3: e = 2; else exp(e log x).  On this path (one warp, a dependent
@@ -164,6 +166,11 @@ __device__ __forceinline__ double margin(double hpar, double hperp, double s, do
     if (!(s * hpar < 0.0)) return -CUDART_INF;
     double x = fabs(hpar) * (a.inv_b * ihc);
     double y = fabs(hperp) * (a.inv_c * ihc);
+    // Well inside the astroid (each term of Eq. 5 below 1/2, with a 1e-9 guard band for the few-ulp powers): the spin cannot
+    // switch and cannot be the arg-max that matters (only margins > 1 ever win), so its margin is recorded as 0 ("not
+    // switchable", the same key as -inf) and the two fractional powers are skipped.  Whole-protocol scans spend most of
+    // their FP64 work on such spins (ensembles of small systems are FP64-bound by exactly this).
+    if (x < a.tx && y < a.ty) return 0.0;
     return pow_kind(x, a.e_par, a.k_par) + pow_kind(y, a.e_perp, a.k_perp);
 }
 
@@ -639,7 +646,8 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         const double* __restrict__ sweep_sigma /*[T] thermal std per step (annealing) or NULL*/,
         const double* __restrict__ sweep_lscale /*[T] scale of the static per-spin field per step or NULL*/,
         const double2* __restrict__ sweep_lseries /*[T,N] per-spin field per step or NULL*/,
-        int use_base /*continue the flip count and log of k_relax_batch (ctr[r].batch_flips)*/) {
+        int use_base /*continue the flip count and log of k_relax_batch (ctr[r].batch_flips)*/,
+        int state_smem /*the replica's per-spin state (h_dip, h_fix, M, 1/h_c, s: 49 B per spin) lives in shared memory*/) {
     // four-level arg-max hierarchy in shared memory:
     // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
     extern __shared__ unsigned char smem_raw[];
@@ -664,6 +672,19 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = RELAX_THREADS / 32;
     const bool one_warp = (Kp + 1 <= 32);               // the whole update fits one warp: no broadcast of k needed
+    // Small replicas ("small N entirely in shared memory"): for the duration of a sweep the per-spin state is
+    // staged into shared memory; every dependent round trip of the flip loop (neighbour state, margins, leaf rescan) then
+    // costs a shared-memory access instead of an L2 one.  The couplings stay in global memory: read-only and the same for
+    // all replicas of an SM, they hit in L1.  Written back at the end.
+    double2 *g_hdip = hdip, *g_hfix = hfix; double* g_M = M; int8_t* g_s = s;
+    if (state_smem) {
+        unsigned char* sp = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(touched + Kp + 1) + 15) & ~(uintptr_t)15);
+        double2* hd_s = reinterpret_cast<double2*>(sp); double2* hf_s = hd_s + N;
+        double* M_s = reinterpret_cast<double*>(hf_s + N); double* ih_s = M_s + N; int8_t* s_s = reinterpret_cast<int8_t*>(ih_s + N);
+        for (int64_t i = tid; i < N; i += RELAX_THREADS) { hd_s[i] = hdip[i]; hf_s[i] = hfix[i]; M_s[i] = M[i]; ih_s[i] = ihc[i]; s_s[i] = s[i]; }
+        hdip = hd_s; hfix = hf_s; M = M_s; ihc = ih_s; s = s_s;
+        __syncthreads();
+    }
 
     long long nflips = use_base ? ctr[r].batch_flips : 0;
     const long long nflips0 = nflips;
@@ -756,7 +777,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
             // future flip.  Iteration n brings its ELL row to L2; iteration n+1 reads the row (an L2 hit by
             // then) and brings its neighbours' state, its coupling row and its own leaf of margins to L2.
             const int e = warp - PF_W0, ne = NW - PF_W0;
-            if (pf_row >= 0) {
+            if (pf_row >= 0 && !state_smem) {
                 for (int t = lane; t < Kp; t += 32) {
                     int i = __ldcg(nbr + (int64_t)pf_row * Kp + t);
                     if (i >= 0) {
@@ -862,7 +883,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
                     int64_t i = base + q0 + 32 * u;
-                    m[u] = (q0 + 32 * u < LB && i < N) ? __ldcg(M + i) : -CUDART_INF;
+                    m[u] = (q0 + 32 * u < LB && i < N) ? (state_smem ? M[i] : __ldcg(M + i)) : -CUDART_INF;
                 }
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
@@ -891,6 +912,10 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
     }   // steps
     // a sweep stopped by max_flips leaves the fields of the step it actually reached (hfix, M and the spins
     // belong to that step) and zero flips for the steps it never ran
+    if (state_smem) {
+        __syncthreads();
+        for (int64_t i = tid; i < N; i += RELAX_THREADS) { g_hdip[i] = hdip[i]; g_hfix[i] = hfix[i]; g_M[i] = M[i]; g_s[i] = s[i]; }
+    }
     if (T > 0 && tid == 0) hext_all[r] = sweep_fields[st_last];
     if (T > 0 && flips_per_step)
         for (int t = st_last + 1 + tid; t < T; t += RELAX_THREADS) flips_per_step[(int64_t)r * T + t] = 0;
@@ -1676,17 +1701,25 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
     // ensembles with more than 31 neighbours per spin (e.g. section IV.B: 592 replicas, K = 632): the loop is latency-bound,
     // so several replicas per SM beat a wide CTA per replica: 256 threads (4 per SM), 128 from 8 replicas per SM
     const bool mid_cta = sim->R > sim->sm_count && sim->Kp + 1 > 32 && sim->nblk <= 1024;
+    // per-spin state in shared memory (sweeps only: a single relax would copy the state in and out for a few flips), if it
+    // fits beside the hierarchy without costing the variant its CTAs per SM
+    const int threads = small_cta ? (sim->R > 8 * sim->sm_count ? 64 : 128) : mid_cta ? (sim->R >= 8 * sim->sm_count ? 128 : 256)
+                                  : (sim->Kp + 1 > 512 ? 1024 : 512);
+    const int ctas_per_sm = threads == 64 ? 16 : threads == 128 ? 8 : threads == 256 ? 4 : 1;
+    const size_t state_bytes = 49 * (size_t)sim->N + 32;
+    const size_t smem_budget = std::min<size_t>(200 * 1024, (227 * 1024) / ctas_per_sm - 1024);
+    const int state_smem = (T > 0 && sim->relax_smem + state_bytes <= smem_budget) ? 1 : 0;
+    const size_t smem = sim->relax_smem + (state_smem ? state_bytes : 0);
 #define FS_RELAX_ARGS sim->N, sim->Kp, lb_shift, sim->nblk, sim->ast, (long long)max_flips, (long long)sim->log_cap, sim->nbr, \
         sim->wT, sim->hc, sim->s, sim->hdip, sim->hfix, sim->M, sim->bval, sim->bidx, sim->flog, sim->ctr, \
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid, \
         sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0, \
-        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev, lscale_dev, lseries_dev, use_base
-    if (small_cta && sim->R > 8 * sim->sm_count) k_relax<64><<<sim->R, 64, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
-    else if (small_cta) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
-    else if (mid_cta && sim->R >= 8 * sim->sm_count) k_relax<128><<<sim->R, 128, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
-    else if (mid_cta) k_relax<256><<<sim->R, 256, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
-    else if (sim->Kp + 1 > 512) k_relax<1024><<<sim->R, 1024, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
-    else k_relax<512><<<sim->R, 512, sim->relax_smem, sim->stream>>>(FS_RELAX_ARGS);
+        T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev, lscale_dev, lseries_dev, use_base, state_smem
+    if (threads == 64) { CUDA_TRY(raise_smem_limit(k_relax<64>, smem)); k_relax<64><<<sim->R, 64, smem, sim->stream>>>(FS_RELAX_ARGS); }
+    else if (threads == 128) { CUDA_TRY(raise_smem_limit(k_relax<128>, smem)); k_relax<128><<<sim->R, 128, smem, sim->stream>>>(FS_RELAX_ARGS); }
+    else if (threads == 256) { CUDA_TRY(raise_smem_limit(k_relax<256>, smem)); k_relax<256><<<sim->R, 256, smem, sim->stream>>>(FS_RELAX_ARGS); }
+    else if (threads == 1024) { CUDA_TRY(raise_smem_limit(k_relax<1024>, smem)); k_relax<1024><<<sim->R, 1024, smem, sim->stream>>>(FS_RELAX_ARGS); }
+    else { CUDA_TRY(raise_smem_limit(k_relax<512>, smem)); k_relax<512><<<sim->R, 512, smem, sim->stream>>>(FS_RELAX_ARGS); }
 #undef FS_RELAX_ARGS
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());
@@ -1831,7 +1864,8 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     sim->N = N; sim->R = R; sim->K = K; sim->Kp = Kp; sim->LB = LB; sim->nblk = nblk; sim->ncells = gp.ncells;
     sim->n_inter = I; sim->log_cap = log_cap; sim->p = *p; sim->grid = gp.g; sim->stream = st;
     auto kind = [](double denom) { return denom == 3.0 ? 1 : (denom == 2.0 ? 2 : (denom == 1.0 ? 3 : 0)); };
-    sim->ast = Astroid{1.0 / p->b, 1.0 / p->c, 2.0 / p->gamma, 2.0 / p->beta, kind(p->gamma), kind(p->beta)};
+    sim->ast = Astroid{1.0 / p->b, 1.0 / p->c, 2.0 / p->gamma, 2.0 / p->beta, kind(p->gamma), kind(p->beta),
+                       std::pow(0.5, p->gamma / 2.0) * (1.0 - 1e-9), std::pow(0.5, p->beta / 2.0) * (1.0 - 1e-9)};
     int dev = 0; cudaGetDevice(&dev);
     sim->device = dev;
     cudaDeviceGetAttribute(&sim->sm_count, cudaDevAttrMultiProcessorCount, dev);
