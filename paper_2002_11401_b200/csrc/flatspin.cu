@@ -60,7 +60,8 @@ int fail(int code, const char* fmt, ...) {
     } while (0)
 #define LAUNCHED() (g_launches.fetch_add(1, std::memory_order_relaxed))
 
-constexpr int MAX_LEAF_BLOCKS = 8192;   // leaf-block maxima kept in the relax CTA's shared memory
+constexpr int MAX_LEAF_BLOCKS = 16384;  // leaf-block maxima kept in the relax CTA's shared memory (12 B each + groups: 203 KB of 227):
+                                        // leaves of up to 1024 spins, so N <= 16,777,216 spins per replica
 constexpr int MAX_K = 8192;             // maximum degree supported by the warp bitonic sort
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }

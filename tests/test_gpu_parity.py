@@ -1073,6 +1073,33 @@ def test_many_replicas_with_more_than_31_neighbors(B, R):
     assert np.array_equal(sim.get_spins().cpu().numpy(), s)
 
 
+def test_more_than_8192_leaves(B):
+    """8.8 M spins: 1024-spin leaves, 8,618 of them (the hierarchy's shared memory holds up to 16,384: 16.7 M spins).
+    Config-4 recipe at 2100 x 2100 with the thermal field, a few field values around the onset of the reversal, sequential
+    and batched relax against the Tier B oracle."""
+    w = W.config("4", scale=2100)
+    assert w.N > 8192 * 1024
+    for batched in (True, False):
+        sim, orc = mk(B, w)
+        if not batched:
+            sim.set_batch(0)
+        total = 0
+        for t in (0, 120, 128, 131, 134):
+            hx, hy = w.fields[t]
+            sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+            n = sim.relax()
+            no, log = orc.relax_B()
+            assert n == no, (t, n, no)
+            if n:
+                assert np.array_equal(sim.get_flip_log().cpu().numpy(), log[: 4 * w.N + 1024]), t
+            total += n
+        assert total > 100
+        assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+        assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+        assert sim.scan()[0] == orc.scan()[0]
+        sim.close(); del orc
+
+
 # ------------------------------------------------------------------ optional fp32 field path (reported separately, 1e-5)
 @pytest.mark.parametrize("which,scale", [("1", None), ("3", 30), ("5", 40), ("2", 20)])
 def test_fp32_stencil_field_path(B, which, scale):
