@@ -84,6 +84,20 @@ cudaError_t raise_smem_limit(F* func, size_t bytes) {
     return e;
 }
 
+// Launch with programmatic stream serialisation allowed: the kernel may become resident before the kernel in front of it
+// in the stream has finished, if that kernel executed griddepcontrol.launch_dependents; it must execute griddepcontrol.wait
+// before it touches anything an earlier kernel writes or reads.  Hides the launch latency of back-to-back dependent kernels.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // every entry point runs on the simulation's device, whatever device is current in the calling thread
 struct DeviceGuard {
     int prev = -1, dev;
@@ -421,6 +435,7 @@ template <int G>
 __global__ void __launch_bounds__(256) k_gather(int64_t N, int Kp, const int* __restrict__ nbr,
                                                 const double2* __restrict__ w, const int8_t* __restrict__ s_all,
                                                 double2* __restrict__ hdip_all) {
+    asm volatile("griddepcontrol.launch_dependents;");   // lets a following k_scan become resident in this kernel's tail (see k_scan)
     const int8_t* __restrict__ s = s_all + (int64_t)blockIdx.y * N;
     double2* __restrict__ hdip = hdip_all + (int64_t)blockIdx.y * N;
     int64_t tid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -501,16 +516,27 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     constexpr int SCAN_THREADS = SCAN_SPB / SCAN_SPT;
     const int64_t base = (int64_t)blockIdx.x * SCAN_SPB + threadIdx.x;
-    // fs_set_field launches nothing: its field arrives here by value, and one thread records it for the later readers
-    const double2 he = set_field ? field : hext_all[r];
-    if (set_field && blockIdx.x == 0 && threadIdx.x == 0) const_cast<double2*>(hext_all)[r] = field;
-    // loads of all four spins first
+    // Programmatic dependent launch: this kernel may become resident while the gather kernel in front of it is still
+    // running (the gathers call griddepcontrol.launch_dependents at their start, so that happens as soon as their last CTA
+    // has started: in the tail of the gather, when SMs fall idle).  Until the wait below it reads only what no gather
+    // writes (frames, 1/h_c, spins): that cold-DRAM round trip and the launch latency overlap the gather's tail.  h_dip is
+    // read, and everything is written, after the wait.  Behind any other kernel the wait falls through at once.
+    asm volatile("griddepcontrol.launch_dependents;");   // a k_relax behind this scan may become resident (it waits at its top)
     double2 c[SCAN_SPT], hd[SCAN_SPT]; double ih[SCAN_SPT], sp[SCAN_SPT];
 #pragma unroll
     for (int q = 0; q < SCAN_SPT; ++q) {
         const int64_t i = base + q * SCAN_THREADS;
-        if (i < N) { c[q] = cs[i]; hd[q] = hdip_all[off + i]; ih[q] = hc_all[off + i]; sp[q] = (double)s_all[off + i]; }
-        else { c[q] = make_double2(1.0, 0.0); hd[q] = make_double2(0.0, 0.0); ih[q] = 1.0; sp[q] = 1.0; }
+        if (i < N) { c[q] = cs[i]; ih[q] = hc_all[off + i]; sp[q] = (double)s_all[off + i]; }
+        else { c[q] = make_double2(1.0, 0.0); ih[q] = 1.0; sp[q] = 1.0; }
+    }
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // fs_set_field launches nothing: its field arrives here by value, and one thread records it for the later readers
+    const double2 he = set_field ? field : hext_all[r];
+    if (set_field && blockIdx.x == 0 && threadIdx.x == 0) const_cast<double2*>(hext_all)[r] = field;
+#pragma unroll
+    for (int q = 0; q < SCAN_SPT; ++q) {
+        const int64_t i = base + q * SCAN_THREADS;
+        if (i < N) hd[q] = hdip_all[off + i]; else hd[q] = make_double2(0.0, 0.0);
     }
     unsigned long long nsw = 0;
 #pragma unroll
@@ -649,8 +675,10 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         const double2* __restrict__ sweep_lseries /*[T,N] per-spin field per step or NULL*/,
         int use_base /*continue the flip count and log of k_relax_batch (ctr[r].batch_flips)*/,
         int state_smem /*the replica's per-spin state (h_dip, h_fix, M, 1/h_c, s: 49 B per spin) lives in shared memory*/) {
+    // launched programmatically dependent on the k_scan in front of it (launch latency hidden): nothing is read before this
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     // four-level arg-max hierarchy in shared memory:
-    // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 8 of them) -> top
+    // spins -> leaves (LB spins) -> groups (32 leaves) -> supergroups (32 groups, <= 16 of them) -> top
     extern __shared__ unsigned char smem_raw[];
     const int ngrp = (nblk + 31) >> 5, nsup = (ngrp + 31) >> 5, LB = 1 << LBshift;
     mkey_t* bkey = reinterpret_cast<mkey_t*>(smem_raw);           // [nblk]
@@ -1660,8 +1688,8 @@ int do_scan(fs_sim* sim, bool finalize) {
 #define FS_SCAN_ARGS sim->N, sim->LB, sim->ast, fsp, finalize ? 1 : 0, sim->hext, sim->cs, sim->hc, sim->s, sim->hdip, \
                      sim->hfix, sim->M, sim->bval, sim->bidx, sim->nblk, sim->scnt, sim->ctr, sim->hloc, \
                      sim->field_pending ? 1 : 0, sim->field_value
-    if (spb == 1024) k_scan<2, 1024><<<grid, 512, 0, sim->stream>>>(FS_SCAN_ARGS);
-    else k_scan<2, 512><<<grid, 256, 0, sim->stream>>>(FS_SCAN_ARGS);
+    if (spb == 1024) CUDA_TRY(launch_pdl(k_scan<2, 1024>, grid, dim3(512), 0, sim->stream, FS_SCAN_ARGS));
+    else CUDA_TRY(launch_pdl(k_scan<2, 512>, grid, dim3(256), 0, sim->stream, FS_SCAN_ARGS));
     sim->field_pending = false;
 #undef FS_SCAN_ARGS
     LAUNCHED();
@@ -1716,11 +1744,11 @@ int launch_relax(fs_sim* sim, int64_t max_flips, int T, const double2* fields_de
         sim->stencil_ok && sim->sgrid_valid ? sim->cellidx : nullptr, sim->sgrid, \
         sim->stencil_ok ? (int64_t)sim->lg.nsub * sim->lg.Upa * sim->lg.Vpa : 0, \
         T, fields_dev, fsp, sim->cs, per_step_dev, sim->hext, sim->hloc, sigma_dev, lscale_dev, lseries_dev, use_base, state_smem
-    if (threads == 64) { CUDA_TRY(raise_smem_limit(k_relax<64>, smem)); k_relax<64><<<sim->R, 64, smem, sim->stream>>>(FS_RELAX_ARGS); }
-    else if (threads == 128) { CUDA_TRY(raise_smem_limit(k_relax<128>, smem)); k_relax<128><<<sim->R, 128, smem, sim->stream>>>(FS_RELAX_ARGS); }
-    else if (threads == 256) { CUDA_TRY(raise_smem_limit(k_relax<256>, smem)); k_relax<256><<<sim->R, 256, smem, sim->stream>>>(FS_RELAX_ARGS); }
-    else if (threads == 1024) { CUDA_TRY(raise_smem_limit(k_relax<1024>, smem)); k_relax<1024><<<sim->R, 1024, smem, sim->stream>>>(FS_RELAX_ARGS); }
-    else { CUDA_TRY(raise_smem_limit(k_relax<512>, smem)); k_relax<512><<<sim->R, 512, smem, sim->stream>>>(FS_RELAX_ARGS); }
+    if (threads == 64) { CUDA_TRY(raise_smem_limit(k_relax<64>, smem)); CUDA_TRY(launch_pdl(k_relax<64>, dim3((unsigned)sim->R), dim3(64), smem, sim->stream, FS_RELAX_ARGS)); }
+    else if (threads == 128) { CUDA_TRY(raise_smem_limit(k_relax<128>, smem)); CUDA_TRY(launch_pdl(k_relax<128>, dim3((unsigned)sim->R), dim3(128), smem, sim->stream, FS_RELAX_ARGS)); }
+    else if (threads == 256) { CUDA_TRY(raise_smem_limit(k_relax<256>, smem)); CUDA_TRY(launch_pdl(k_relax<256>, dim3((unsigned)sim->R), dim3(256), smem, sim->stream, FS_RELAX_ARGS)); }
+    else if (threads == 1024) { CUDA_TRY(raise_smem_limit(k_relax<1024>, smem)); CUDA_TRY(launch_pdl(k_relax<1024>, dim3((unsigned)sim->R), dim3(1024), smem, sim->stream, FS_RELAX_ARGS)); }
+    else { CUDA_TRY(raise_smem_limit(k_relax<512>, smem)); CUDA_TRY(launch_pdl(k_relax<512>, dim3((unsigned)sim->R), dim3(512), smem, sim->stream, FS_RELAX_ARGS)); }
 #undef FS_RELAX_ARGS
     LAUNCHED();
     CUDA_TRY(cudaGetLastError());

@@ -271,6 +271,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
                                                                const int* __restrict__ gidx, const sgcell_t* __restrict__ sg,
                                                                const double2* __restrict__ T, const int2* __restrict__ rowtab,
                                                                double2* __restrict__ hdip_all) {
+    asm volatile("griddepcontrol.launch_dependents;");   // lets a following k_scan become resident in this kernel's tail (see k_scan)
     extern __shared__ __align__(16) unsigned char st_raw[];
     const int RS = (blockDim.x >> 5) / NW, TV = OV * NW;
     const int SUc = (ST_TU + 2 * g.Ru + 3) & ~3, SH = TV + 2 * g.Rv, WH = g.W * g.H;   // staged row: SUc cells, pitch PU
