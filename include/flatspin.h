@@ -98,7 +98,8 @@ int fs_workspace_bytes(int64_t N, int32_t R, const double* pos_dev, const fs_par
  * alpha*g_ij (Eq. 3) in row-major ELL.  Spins start at +1 (fs_set_spins to change).
  * pos_dev DEVICE [N,2]; angle_dev DEVICE [N] radians; hc_dev DEVICE [N] (fs_create) or [R,N]
  * (fs_create_ensemble), all > 0.  workspace_dev: DEVICE, 256-byte aligned, >= fs_workspace_bytes.
- * Synchronises `stream` once (to read K and the validation flags). */
+ * Synchronises `stream` once (to read K and the validation flags).  N <= 16,777,216 spins per replica (the relax
+ * loop keeps up to 16,384 leaf maxima of up to 1024 spins in shared memory): FS_ERR_ARG beyond. */
 int fs_create(fs_sim** out, int64_t N, const double* pos_dev, const double* angle_dev,
               const double* hc_dev, const fs_params* p, void* workspace_dev, size_t workspace_bytes,
               void* stream);
@@ -121,7 +122,8 @@ int fs_get_spins(fs_sim* sim, int8_t* s_dev_out /*DEVICE [R,N]*/);
  * during a relaxation.  sigma_th = 0 switches it off (default). */
 int fs_set_thermal(fs_sim* sim, double sigma_th, uint64_t seed);
 
-/* Global external field for all replicas, and the step key of the thermal stream. */
+/* Global external field for all replicas, and the step key of the thermal stream.  Host values; no launch
+ * and no synchronise: the next scan / relax takes the field as a kernel argument.  Always FS_OK for a valid sim. */
 int fs_set_field(fs_sim* sim, double hx, double hy, uint32_t step);
 /* Per-replica global fields: h_host HOST [R,2] (hx,hy). */
 int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step);
