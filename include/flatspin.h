@@ -252,7 +252,8 @@ int fs_get_neighbors(fs_sim* sim, int32_t* idx_dev_out, int32_t* K_out);
 
 /* Host-buffer convenience for end-to-end timing: H2D spins [R,N] -> gather -> scan -> D2H total fields
  * [R,N,2], all on the simulation's stream, then synchronise.  s_host / h_host_out HOST (pinned for
- * full speed).  Scan outputs as fs_scan (replica 0). */
+ * full speed).  h_host_out may be NULL: then only the scan's summary returns to the host (the fields stay on the
+ * device, as they do for fs_relax).  Scan outputs as fs_scan (replica 0). */
 int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t* n_switchable,
                  int64_t* best_index, double* best_L);
 

@@ -324,11 +324,12 @@ class Sim:
         return out[:, :self.K]
 
     # ---- host-buffer entry points (end-to-end timing)
-    def step_host(self, s_host: torch.Tensor, h_host_out: torch.Tensor):
+    def step_host(self, s_host: torch.Tensor, h_host_out: torch.Tensor | None):
         assert s_host.dtype == torch.int8 and not s_host.is_cuda and s_host.numel() == self.R * self.N
-        assert h_host_out.dtype == torch.float64 and not h_host_out.is_cuda and h_host_out.numel() == 2 * self.R * self.N
+        assert h_host_out is None or (h_host_out.dtype == torch.float64 and not h_host_out.is_cuda and h_host_out.numel() == 2 * self.R * self.N)
         n, b, l = C.c_int64(), C.c_int64(), C.c_double()
-        _check(self.L, self.L.fs_step_host(self.h, s_host.data_ptr(), h_host_out.data_ptr(), C.byref(n), C.byref(b), C.byref(l)))
+        _check(self.L, self.L.fs_step_host(self.h, s_host.data_ptr(), h_host_out.data_ptr() if h_host_out is not None else None,
+                                           C.byref(n), C.byref(b), C.byref(l)))
         return int(n.value), int(b.value), float(l.value)
 
     def relax_host(self, hx, hy, step, s_host_out: torch.Tensor):

@@ -2386,7 +2386,7 @@ int fs_vertex_populations(fs_sim* sim, const int32_t* vertices_dev, int64_t V, i
 
 int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t* n_switchable, int64_t* best_index,
                  double* best_L) {
-    if (!sim || !s_host || !h_host_out) return fail(FS_ERR_ARG, "null pointer");
+    if (!sim || !s_host) return fail(FS_ERR_ARG, "null pointer");
     DeviceGuard guard_(sim->device);
     size_t rn = (size_t)sim->R * sim->N;
     CUDA_TRY(cudaMemcpyAsync(sim->s, s_host, rn, cudaMemcpyHostToDevice, sim->stream));
@@ -2395,12 +2395,14 @@ int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t*
     if (rc) return rc;
     rc = fs_scan_ensemble(sim, nullptr, nullptr, nullptr);
     if (rc) return rc;
-    // total field into hfix's sibling buffer M is not large enough; reuse hfix (rewritten by the next scan)
-    dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
-    FieldSpec fsp{sim->sigma, sim->seed, sim->step};
-    k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, FS_FIELD_TOTAL, fsp, sim->hext, sim->cs, sim->hdip, sim->hfix, sim->hloc);
-    LAUNCHED();
-    CUDA_TRY(cudaMemcpyAsync(h_host_out, sim->hfix, 16 * rn, cudaMemcpyDeviceToHost, sim->stream));
+    if (h_host_out) {                                    // NULL: only the scan's summary goes back to the host
+        // total field into hfix's sibling buffer M is not large enough; reuse hfix (rewritten by the next scan)
+        dim3 grid((unsigned)((sim->N + 255) / 256), (unsigned)sim->R);
+        FieldSpec fsp{sim->sigma, sim->seed, sim->step};
+        k_fields_out<<<grid, 256, 0, sim->stream>>>(sim->N, FS_FIELD_TOTAL, fsp, sim->hext, sim->cs, sim->hdip, sim->hfix, sim->hloc);
+        LAUNCHED();
+        CUDA_TRY(cudaMemcpyAsync(h_host_out, sim->hfix, 16 * rn, cudaMemcpyDeviceToHost, sim->stream));
+    }
     rc = fetch_counters(sim);
     if (rc) return rc;
     if (n_switchable) *n_switchable = sim->ctr_host[0].n_switchable;

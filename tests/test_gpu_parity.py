@@ -366,6 +366,8 @@ def test_host_buffer_entry_points(B):
     n, best, L = sim.step_host(s_host, h_host)
     assert (n, best) == orc.scan()[:2]
     assert field_err(h_host.numpy(), orc.fields(0)) < FIELD_TOL
+    assert sim.step_host(s_host, None)[:2] == (n, best)         # summary only: the fields stay on the device
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
     w1 = W.config("1")
     sim, orc = mk(B, w1)
     s_out = torch.empty(w1.N, dtype=torch.int8).pin_memory()
