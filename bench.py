@@ -412,8 +412,9 @@ def phase_profile():
         nfl = max(r[15], 1)
         if mode == "sequential":
             row["k_relax_cycles_per_flip"] = {"flips": int(r[15]), "top arg-max (+ prefetch engines)": r[0] / nfl, "update (row, state, margins)": r[1] / nfl,
-                                          "barrier 1": r[2] / nfl, "leaf repair + groups + supergroups": r[3] / nfl, "of which leaf rescan": r[5] / nfl,
-                                              "barrier 2": r[4] / nfl}
+                                              "wait at the update barrier (thread 0)": r[2] / nfl, "leaf repair + groups + supergroups": r[3] / nfl,
+                                              "of which: own leaf rescan": r[5] / nfl, "wait for the other warps' rescans": r[6] / nfl,
+                                              "groups + wait": r[7] / nfl, "supergroups": r[8] / nfl, "wait at the last barrier": r[4] / nfl}
         out[mode] = row
         sim.close()
     print(json.dumps({"phase_profile": out, "workload": w.name, "source_hash": kernel_source_hash()}), flush=True)

@@ -626,9 +626,13 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
 #ifdef FS_RELAX_PROFILE
 __device__ long long g_relax_prof[16];                  // cycles in: groups+top, update, barrier 1, leaf repair, barrier 2; flips
 #define FS_PROF_T(var) long long var = clock64()
+// behind a barrier: __syncthreads is BAR.SYNC.DEFER_BLOCKING, a clock read right after it sees the barrier's ISSUE; a
+// volatile shared-memory read in between blocks until the barrier has completed, so the wait lands in the right phase
+#define FS_PROF_TB(var) long long var; { const int prof_sink_ = *(volatile int*)&sh_stop; var = clock64() + (prof_sink_ & 0); }
 #define FS_PROF_ADD(slot, a, b) prof[slot] += (b) - (a)
 #else
 #define FS_PROF_T(var)
+#define FS_PROF_TB(var)
 #define FS_PROF_ADD(slot, a, b)
 #endif
 
@@ -893,7 +897,7 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         }
         FS_PROF_T(c2);
         __syncthreads();
-        FS_PROF_T(c3);
+        FS_PROF_TB(c3);
         if (sh_stop) { status = sh_stop - 1; break; }
         if (tid == 0) {
             s[sh_k] = (int8_t)(-sh_sold);
@@ -925,15 +929,17 @@ k_relax(int64_t N, int Kp, int LBshift, int nblk, Astroid ast, long long max_fli
         }
         FS_PROF_T(c3b);
         __syncthreads();
+        FS_PROF_TB(c3c);
         for (int t = warp; t < ntouched; t += NW) repair_group(touched[t] >> 5, nblk, bkey, bidx, gkey, gidx_);
         __syncthreads();
+        FS_PROF_TB(c3d);
         for (int t = warp; t < ntouched; t += NW) repair_group(touched[t] >> 10, ngrp, gkey, gidx_, skey, sidx);
         ++nflips;
         FS_PROF_T(c4);
         __syncthreads();
-        FS_PROF_T(c5);
+        FS_PROF_TB(c5);
         FS_PROF_ADD(0, c0, c1); FS_PROF_ADD(1, c1, c2); FS_PROF_ADD(2, c2, c3); FS_PROF_ADD(3, c3, c4); FS_PROF_ADD(4, c4, c5);
-        FS_PROF_ADD(5, c3, c3b);
+        FS_PROF_ADD(5, c3, c3b); FS_PROF_ADD(6, c3b, c3c); FS_PROF_ADD(7, c3c, c3d); FS_PROF_ADD(8, c3d, c4);
     }
     if (T > 0 && tid == 0 && flips_per_step) flips_per_step[(int64_t)r * T + st] = nflips - nflips_before;
     if (status) break;                                  // max_flips reached
