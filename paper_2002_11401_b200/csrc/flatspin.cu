@@ -17,6 +17,7 @@
 //                                                                             (Eq. 3 linear in s_j)
 //   k_fields_out       fs_get_fields
 //   lattice.cuh        lattice detection + stencil tables + k_gather_stencil (A3, FP64-bound variant)
+#include <cuda.h>                  // CUtensorMap (the driver entry point is fetched at run time: no link against libcuda)
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
@@ -1124,6 +1125,7 @@ struct fs_sim {
     sgcell_t* sgrid = nullptr; int* cellidx = nullptr; bool sgrid_valid = false;
     int* gidx = nullptr; double2* T = nullptr; unsigned long long* owner = nullptr; int2* rowtab = nullptr;
     float2* Tf = nullptr;           // fp32 copy of T (the optional fp32 field path)
+    CUtensorMap sg_map{};           // TMA descriptor of the spin grids [R * nsub][Vpa][Upa], box = PU x SH x 1 (paired fp64 kernel)
     int st_nw = 4, st_rs = 1, st_pv = 0, st_ov = ST_OV; size_t st_smem = 0; bool st_ct = false;
     bool st_sym = false;            // inversion-paired stencil (c_prow / c_pstart tables below, host copies: they are tiny)
     std::vector<int4> prow; std::vector<int2> pstart; std::vector<int> ptofs, rtofs;
@@ -1311,6 +1313,7 @@ int do_gather_stencil(fs_sim* sim) {
                                              cudaMemcpyDeviceToDevice, sim->stream));
             CUDA_TRY(cudaMemcpyToSymbolAsync(c_rtofs, sim->rtofs.data(), 4 * sim->rtofs.size(), 0, cudaMemcpyHostToDevice, sim->stream));
             if (sim->st_sym) {
+                CUDA_TRY(cudaMemcpyToSymbolAsync(c_sg_map, &sim->sg_map, sizeof(CUtensorMap), 0, cudaMemcpyHostToDevice, sim->stream));
                 CUDA_TRY(cudaMemcpyToSymbolAsync(c_ptofs, sim->ptofs.data(), 4 * sim->ptofs.size(), 0, cudaMemcpyHostToDevice, sim->stream));
                 CUDA_TRY(cudaMemcpyToSymbolAsync(c_prow, sim->prow.data(), 16 * sim->prow.size(), 0, cudaMemcpyHostToDevice, sim->stream));
                 CUDA_TRY(cudaMemcpyToSymbolAsync(c_pstart, sim->pstart.data(), 8 * sim->pstart.size(), 0, cudaMemcpyHostToDevice, sim->stream));
@@ -1328,7 +1331,7 @@ int do_gather_stencil(fs_sim* sim) {
             else { if (threads <= 128) FS_LAUNCH_F32(128, 7, false); else FS_LAUNCH_F32(256, 3, false); }
 #undef FS_LAUNCH_F32
         } else if (sym) {
-            if (threads <= 128) FS_LAUNCH_STENCIL_SYM(128, 5); else FS_LAUNCH_STENCIL_SYM(256, 2);
+            if (threads <= 128) FS_LAUNCH_STENCIL_SYM(128, 4); else FS_LAUNCH_STENCIL_SYM(256, 2);
         } else
         FS_LAUNCH_STENCIL(true);
         if (!g_ct_event) CUDA_TRY(cudaEventCreateWithFlags(&g_ct_event, cudaEventDisableTiming));
@@ -1360,7 +1363,7 @@ int stencil_pu(const LatGrid& g) { return ((ST_TU + 2 * g.Ru + 3) & ~3) <= 64 ? 
 size_t stencil_smem(const LatGrid& g, int nw, int rs, int ov, int* pv_out) {
     int TV = ov * nw, SH = TV + 2 * g.Rv, pu = stencil_pu(g);
     size_t tsm = stencil_ct(g) ? 0 : 16 * (size_t)g.nsub * g.W * g.H;
-    size_t tables = (tsm + 8 * (size_t)g.nsub * g.W + 128 * (size_t)TV + 15) & ~(size_t)15;
+    size_t tables = (tsm + 8 * (size_t)g.nsub * g.W + 128 * (size_t)TV + 8 + 127) & ~(size_t)127;   // the tiles are 128-byte aligned (TMA); 8 bytes in front of them hold its mbarrier
     // one spare row in front and behind: the sliding windows read one cell past the last slot of a row
     size_t tiles = 4 * (size_t)(g.nsub * SH + 1) * pu, red = (size_t)(rs - 1) * nw * 512 * ov;
     if (pv_out) *pv_out = pu;
@@ -1485,6 +1488,29 @@ int build_inversion_pairs(fs_sim* sim, const LatGrid& g, const std::vector<unsig
     if (prow.size() > (size_t)CP_MAX) return FS_OK;
     sim->prow = prow; sim->pstart = pstart; sim->ptofs = ptofs; sim->st_sym = true;
     return FS_OK;
+}
+
+// TMA descriptor of the spin grids for k_gather_stencil's paired fp64 variant: uint32 [R * nsub][Vpa][Upa] (u fastest),
+// box = (shared-memory row pitch) x (tile rows + halo) x 1, no swizzle, zero fill outside.  cuTensorMapEncodeTiled is a
+// driver call: its entry point is fetched through the runtime, so the library does not link against libcuda.
+bool make_spin_grid_map(fs_sim* sim, const LatGrid& g) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) { cudaGetLastError(); return false; }
+    const int SH = sim->st_ov * sim->st_nw + 2 * g.Rv, pu = sim->st_pv;
+    if (SH > 256 || pu > 256) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)g.Upa, (cuuint64_t)g.Vpa, (cuuint64_t)sim->R * g.nsub};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.Upa * sizeof(sgcell_t), (cuuint64_t)g.Upa * g.Vpa * sizeof(sgcell_t)};
+    const cuuint32_t box[3] = {(cuuint32_t)pu, (cuuint32_t)SH, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = ((encode_fn)fn)(&sim->sg_map, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, sim->sgrid, dims, strides, box, estr,
+                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
 }
 
 int detect_lattice(fs_sim* sim) {
@@ -1661,9 +1687,9 @@ int detect_lattice(fs_sim* sim) {
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, true, 128, float>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 7, true, 8, false, 128, float>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 3, true, 8, false, 128, float>, stb));
-    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 5, true, 8, true, 64>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 4, true, 8, true, 64>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 2, true, 8, true, 64>, stb));
-    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 5, true, 8, true, 128>, stb));
+    CUDA_TRY(raise_smem_limit(k_gather_stencil<128, 4, true, 8, true, 128>, stb));
     CUDA_TRY(raise_smem_limit(k_gather_stencil<256, 2, true, 8, true, 128>, stb));
     sim->lg = g;
     sim->st_sym = false;
@@ -1676,6 +1702,8 @@ int detect_lattice(fs_sim* sim) {
             sim->rtofs[q] = (int)(q / g.W) * wh + (int)(q % g.W) * g.H + (rt[q].x + g.Rv);
         int rc2 = build_inversion_pairs(sim, g, own);
         if (rc2) return rc2;
+        // the paired fp64 kernel stages its tiles by TMA: without a descriptor it is not used (the plain kernel is)
+        if (sim->st_sym && !make_spin_grid_map(sim, g)) sim->st_sym = false;
     }
     sim->stencil_ok = true; sim->stencil_reason = 0;
     // the build-only arrays (sub, cu, cv) are no longer needed

@@ -212,6 +212,27 @@ __device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) 
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
+// TMA (cp.async.bulk.tensor) + mbarrier, used by the inversion-paired fp64 kernel for its spin tiles: one thread issues
+// one 3-D box copy per source sublattice (box = PU cells x SH rows x 1 grid; cells outside the grid arrive as zeros).
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2),
+                   "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------
 // A3, stencil variant.  CTA = NW x RS warps; tile = 32 cells along u (one per lane) x 8*NW cells
 // along v (8 consecutive outputs per thread).  Prologue: the spin tiles (+ halo, 4-byte cells) of every
@@ -247,6 +268,7 @@ __constant__ int2 c_pstart[NSUB_MAX * NSUB_MAX];
 // derived from a row entry that also feeds vector address arithmetic, ptxas loads it into a vector register and the
 // weights follow (LDC.64, DFMA with three vector operands: 51 instead of 62 DFMA/clk/SM).
 __constant__ int c_rtofs[CR_MAX];
+__constant__ CUtensorMap c_sg_map;     // TMA descriptor of the owner's spin grids (uploaded with the tables)
 __constant__ int c_ptofs[CP_MAX];
 
 // scalar helpers of the stencil kernel: R = double (the parity path) or float (the optional fp32 field path of
@@ -272,7 +294,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
                                                                const double2* __restrict__ T, const int2* __restrict__ rowtab,
                                                                double2* __restrict__ hdip_all) {
     asm volatile("griddepcontrol.launch_dependents;");   // lets a following k_scan become resident in this kernel's tail (see k_scan)
-    extern __shared__ __align__(16) unsigned char st_raw[];
+    extern __shared__ __align__(128) unsigned char st_raw[];
     const int RS = (blockDim.x >> 5) / NW, TV = OV * NW;
     const int SUc = (ST_TU + 2 * g.Ru + 3) & ~3, SH = TV + 2 * g.Rv, WH = g.W * g.H;   // staged row: SUc cells, pitch PU
     (void)Pv;
@@ -282,7 +304,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     const size_t tsm_n = CT ? 0 : (size_t)g.nsub * WH;                      // no shared copy of T in the CT variant
     int2* rows = reinterpret_cast<int2*>(Tsm + tsm_n);                      // [nsub][W]
     int* oidx = reinterpret_cast<int*>(rows + (size_t)g.nsub * g.W);        // [TV][32] spin index of every output
-    sgcell_t* S = reinterpret_cast<sgcell_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 15) & ~(size_t)15));   // [nsub][SH][PU]
+    sgcell_t* S = reinterpret_cast<sgcell_t*>(st_raw + ((16 * tsm_n + 8 * (size_t)g.nsub * g.W + 128 * TV + 8 + 127) & ~(size_t)127));   // [nsub][SH][PU], 128-byte aligned (TMA)
+    constexpr bool TMA = SYM && CT && sizeof(R) == 8;                       // the headline variant stages its tiles by TMA
     // No division: ptxas computes one in the vector datapath and, in some instantiations (fp32, 256-thread CTAs), then kept
     // si, the row tables indexed with it and finally the weights in vector registers (LDC + three-vector-operand DFMA).
     const int rep = g.nsub == 1 ? (int)blockIdx.z : (int)__umulhi(blockIdx.z, g.inv_nsub), si = (int)blockIdx.z - rep * g.nsub;
@@ -292,6 +315,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
     const int wid_u = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31, warp = wid_u % NW, rs = wid_u / NW;
 
+    // (the mbarrier of the TMA variant: the last 8 bytes in front of the tiles, inside the 128-byte alignment pad)
+    unsigned long long* tma_bar = reinterpret_cast<unsigned long long*>(S) - 1;
+    (void)tma_bar;
     // ---- prologue: everything this CTA reads, in flight at once.  A staged row = SUc consecutive cells along u
     // (contiguous in the spin grid and in shared memory): 16-byte cp.async, 16 or 32 lanes per row
     {
@@ -300,7 +326,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
         const int nch = SUc >> 2;
         // a thread keeps its chunk column and walks down the rows with constant strides (the generic (row, chunk) = t / CPR,
         // t % CPR loop with 64-bit addresses cost ~25 instructions per copy: 6% of the kernel's instructions)
-        if constexpr (F32) {                                          // staged through registers: cells become float bits
+        if constexpr (TMA) {
+            // one thread: barrier, expected bytes, one box copy per source sublattice (coordinates in the padded spin grid;
+            // a box is PU cells wide: what lies beyond the grid arrives as zeros).  Everybody waits on the barrier below.
+            // (no loop inside a divergent branch, here or below: behind one, ptxas no longer treats the main loop as
+            // convergent and moves its weights out of the uniform datapath)
+            if (threadIdx.x == 0) mbar_init(tma_bar, 1);
+            __syncthreads();                                          // the initialised barrier is visible to every thread
+            if (threadIdx.x == 0) mbar_expect_tx(tma_bar, (unsigned)(g.nsub * SH * PU * (int)sizeof(sgcell_t)));
+            for (int sj = 0; sj < g.nsub; ++sj)
+                if (threadIdx.x == 0) tma_load_3d(S + (size_t)sj * SH * PU, &c_sg_map, tu0, tv0, rep * g.nsub + sj, tma_bar);
+        } else if constexpr (F32) {                                   // staged through registers: cells become float bits
             for (int sj = 0; sj < g.nsub; ++sj) {
                 sgcell_t* dst = S + (size_t)sj * SH * PU;
                 const sgcell_t* srcj = src + (int64_t)sj * g.Vpa * g.Upa;
@@ -315,14 +351,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
             }
         } else {
             const int ch = threadIdx.x & (CPR - 1), vl0 = threadIdx.x / CPR, vstep = blockDim.x / CPR;
-            if (ch < nch)
-                for (int sj = 0; sj < g.nsub; ++sj) {
-                    sgcell_t* d = S + ((size_t)sj * SH + vl0) * PU + 4 * ch;
-                    const sgcell_t* p = src + ((int64_t)sj * g.Vpa + vl0) * g.Upa + 4 * ch;
-                    const int64_t pstep = (int64_t)vstep * g.Upa;
+            const bool mine = ch < nch;                               // (the loops themselves stay free of divergent branches)
+            for (int sj = 0; sj < g.nsub; ++sj) {
+                sgcell_t* d = S + ((size_t)sj * SH + vl0) * PU + 4 * ch;
+                const sgcell_t* p = src + ((int64_t)sj * g.Vpa + vl0) * g.Upa + 4 * ch;
+                const int64_t pstep = (int64_t)vstep * g.Upa;
 #pragma unroll 4
-                    for (int vl = vl0; vl < SH; vl += vstep, d += vstep * PU, p += pstep) cp_async16(d, p);
-                }
+                for (int vl = vl0; vl < SH; vl += vstep, d += vstep * PU, p += pstep)
+                    if (mine) cp_async16(d, p);
+            }
         }
     }
     if (!CT)
@@ -335,6 +372,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_gather_stencil(int64_t N, LatGri
         else oidx[t] = -1;
     }
     cp_async_wait_all();
+    if constexpr (TMA) mbar_wait(tma_bar, 0);           // every thread observes the completion of the box copies itself
     __syncthreads();
 
     R ax[OV], ay[OV], x[OV];                           // all indices below are compile-time after unrolling: registers

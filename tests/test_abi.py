@@ -61,3 +61,31 @@ def test_argument_errors_are_reported_not_thrown():
     assert L.fs_workspace_bytes(10, 1, None, ctypes.byref(bad), ctypes.byref(n), None) == FS_ERR_ARG
     assert L.fs_relax(None, 0, None) == FS_ERR_ARG
     assert L.fs_destroy(None) == 0
+
+
+def test_stencil_kernels_keep_their_weights_in_uniform_registers():
+    """Compile-time property of the built library: every constant-table variant of k_gather_stencil must
+    read its couplings through the uniform datapath (LDCU -> `DFMA R, R, UR, R`, 62 against 51 DFMA/clk/SM); ptxas
+    drops that silently when the kernel's control flow changes shape (a loop inside a divergent branch in front of the
+    main loop is enough).  The inversion-paired fp64 variants stage their tiles by TMA (UTMALDG)."""
+    import shutil
+    import subprocess
+    from paper_2002_11401_b200 import build
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", build.build()], capture_output=True, text=True, check=True).stdout
+    parts = re.split(r"\n\s*Function : ", sass)
+    seen = 0
+    for p in parts:
+        name = p.split("\n")[0]
+        m = re.search(r"k_gather_stencilILi(\d+)ELi(\d+)ELb(\d)ELi8ELb(\d)ELi(\d+)E([df])", name)
+        if not m or m.group(3) != "1":                      # only the constant-table (CT) variants
+            continue
+        seen += 1
+        vec = len(re.findall(r"LDC[.\w]* R\d+, c\[0x3\]", p))          # table reads with a vector-register index
+        uni = len(re.findall(r"LDCU[.\w]* UR\d+, c\[0x3\]", p))       # ... through the uniform datapath
+        assert uni >= 16 and vec <= 2, (name, vec, uni)
+        if m.group(4) == "1" and m.group(6) == "d":
+            assert "UTMALDG" in p, name
+    assert seen >= 12
