@@ -377,6 +377,49 @@ def test_host_buffer_entry_points(B):
     assert np.array_equal(s_out.numpy(), orc.spins())
 
 
+def test_field_by_value_state_machine(B):
+    """fs_set_field launches nothing: the value waits for the next scan (kernel argument) or is flushed for the other
+    readers.  Every order of calls must see the field that was set last."""
+    import torch
+    w = W.config("1")
+    sim, orc = mk(B, w)
+
+    def ext(sim_):
+        return sim_.get_fields(2).cpu().numpy()
+
+    h1, h2, h3 = w.fields[100], w.fields[260], w.fields[300]
+    # set -> read the external field before any scan (flush path)
+    sim.set_field(*h1, 100); orc.set_field(*h1, 100)
+    assert field_err(ext(sim), orc.fields(2)) < FIELD_TOL
+    # set twice -> scan sees the second value; the total field afterwards too
+    sim.set_field(*h1, 100); sim.set_field(*h2, 260); orc.set_field(*h2, 260)
+    assert sim.scan()[:2] == orc.scan()[:2]
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    # set -> relax (scan inside) -> read
+    sim.set_field(*h3, 300); orc.set_field(*h3, 300)
+    n = sim.relax(); no, log = orc.relax_B()
+    assert n == no and np.array_equal(sim.get_flip_log().cpu().numpy(), log)
+    assert field_err(ext(sim), orc.fields(2)) < FIELD_TOL
+    # a pending value must not survive a sweep (which leaves its own last field) ...
+    sim.set_field(*h1, 100)
+    fields = w.fields[300:320]
+    sim.sweep(fields, step0=300)
+    for t, (hx, hy) in enumerate(fields):
+        orc.set_field(hx, hy, 300 + t); orc.relax_B()
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(ext(sim), orc.fields(2)) < FIELD_TOL
+    assert sim.scan()[:2] == orc.scan()[:2]
+    # ... nor an ensemble field upload, nor the host-buffer step
+    sim.set_field(*h1, 100)
+    sim.set_field_ensemble(np.array([h2]), 260); orc.set_field(*h2, 260)
+    assert sim.scan()[:2] == orc.scan()[:2]
+    sim.set_field(*h3, 300); orc.set_field(*h3, 300)
+    s_host = torch.as_tensor(orc.spins().copy()).pin_memory()
+    h_host = torch.empty((w.N, 2), dtype=torch.float64).pin_memory()
+    assert sim.step_host(s_host, h_host)[:2] == orc.scan()[:2]
+    assert field_err(h_host.numpy(), orc.fields(0)) < FIELD_TOL
+
+
 # ------------------------------------------------------------------ BASELINE.json full sizes
 def _full_protocol(B, which, stride=1):
     """Whole protocol of a config at BASELINE.json's full size, Tier B oracle beside the GPU, flip log
