@@ -420,6 +420,44 @@ def test_field_by_value_state_machine(B):
     assert field_err(h_host.numpy(), orc.fields(0)) < FIELD_TOL
 
 
+@pytest.mark.parametrize("geom,batched", [("square_open", True), ("square_open", False), ("ising", True), ("ising", False)])
+def test_other_geometries_whole_protocol(B, geom, batched):
+    """Relaxation protocols on the two flatspin geometries no BASELINE config uses: square ASI with
+    open edges (the geometry of the paper's own throughput figure: 8-spin neighbourhood) and the 2-D Ising
+    lattice (one sublattice, parallel spins), with the thermal field, a generalised astroid and a hysteresis ramp; large
+    enough for the batched kernel (>= 16,384 spins), sequential kernel beside it; flip logs against the Tier B oracle."""
+    if geom == "square_open":
+        pos, ang = W.square_open(92); nd, phi = 1.0, 45.0                # 16,744 spins
+        par = dict(alpha=0.001, b=1.0, c=1.0, beta=3.0, gamma=3.0, neighbor_distance=nd)
+    else:
+        pos, ang = W.ising(130, 130); nd, phi = 1.5, 30.0               # 16,900 spins, 8 neighbours
+        par = dict(alpha=0.0008, b=0.41, c=1.0, beta=1.5, gamma=3.9, neighbor_distance=nd)
+    N = len(ang)
+    w = W.Workload(f"{geom}_protocol", pos, ang, W.coercive_fields(N, seed=5), np.ones(N, np.int8), par,
+                   W.ramp(0.22, -0.22, 60, phi, legs=2), sigma_th=0.004, thermal_seed=3)
+    sim, orc = mk(B, w)
+    assert sim.lattice()["active"]
+    if not batched:
+        sim.set_batch(0)
+    total = 0
+    for t, (hx, hy) in enumerate(w.fields):
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        n = sim.relax()
+        no, log = orc.relax_B()
+        assert n == no, (t, n, no)
+        if n:
+            assert np.array_equal(sim.get_flip_log().cpu().numpy(), log), t
+        total += n
+    assert total >= N                                   # at least one full reversal
+    if batched:
+        assert sim.batch_stats()["flips"] > 0
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+    assert orc.monitor()[0] == 0
+    sim.update_fields()                                  # a fresh stencil gather of the final state
+    assert field_err(sim.get_fields(1).cpu().numpy(), orc.fields(1)) < FIELD_TOL
+
+
 # ------------------------------------------------------------------ BASELINE.json full sizes
 def _full_protocol(B, which, stride=1):
     """Whole protocol of a config at BASELINE.json's full size, Tier B oracle beside the GPU, flip log
