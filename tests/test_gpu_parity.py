@@ -458,6 +458,36 @@ def test_other_geometries_whole_protocol(B, geom, batched):
     assert field_err(sim.get_fields(1).cpu().numpy(), orc.fields(1)) < FIELD_TOL
 
 
+@pytest.mark.parametrize("n", [15, 24])
+def test_cutoff_covers_the_whole_system(B, n):
+    """Maximum neighbourhood: the cutoff covers the system, every spin is every other spin's neighbour (K = N - 1: 479
+    and 1199, the second more than one pass of the 1024-thread relax kernel); the stencil spans the whole lattice
+    (half-extent 15 / 24 cells).  Fields by stencil and by ELL, scan and a whole hysteresis against the oracle."""
+    w = W.config("1", scale=n)
+    w.params["neighbor_distance"] = 100.0
+    w.fields = W.ramp(0.3, -0.3, 40, 45.0, legs=2)
+    spins = W.random_spins(w.N, seed=2)
+    sim, orc = mk(B, w, spins=spins)
+    assert sim.K == w.N - 1 and orc.build_neighbors() == w.N - 1
+    lat = sim.lattice()
+    assert lat["active"] and lat["Ru"] == n, lat
+    hx, hy = w.fields[7]
+    sim.set_field(hx, hy, 7); orc.set_field(hx, hy, 7)
+    for variant in (B.GATHER_ELL_F64, B.GATHER_STENCIL):
+        sim.set_gather_variant(variant); sim.update_fields()
+        _check_all_fields(sim, orc)
+    assert sim.scan()[:2] == orc.scan()[:2]
+    total = 0
+    for t, (hx, hy) in enumerate(w.fields):
+        sim.set_field(hx, hy, t); orc.set_field(hx, hy, t)
+        nf = sim.relax(); no, log = orc.relax_B()
+        assert nf == no and (nf == 0 or np.array_equal(sim.get_flip_log().cpu().numpy(), log)), t
+        total += nf
+    assert total > w.N
+    assert np.array_equal(sim.get_spins().cpu().numpy(), orc.spins())
+    assert field_err(sim.get_fields(0).cpu().numpy(), orc.fields(0)) < FIELD_TOL
+
+
 # ------------------------------------------------------------------ BASELINE.json full sizes
 def _full_protocol(B, which, stride=1):
     """Whole protocol of a config at BASELINE.json's full size, Tier B oracle beside the GPU, flip log
