@@ -261,6 +261,40 @@ int fs_step_host(fs_sim* sim, const int8_t* s_host, double* h_host_out, int64_t*
 int fs_relax_host(fs_sim* sim, double hx, double hy, uint32_t step, int8_t* s_host_out,
                   int64_t* n_flips_out);
 
+/* The switching scan for callers that must not allocate device memory (Eqs. 2, 5, 6 and the arg-max of PAPER.md:122;
+ * SURVEY.md A4-A7).
+ *
+ * Every other scan here works on a handle whose partial results live in the workspace fs_create laid out.  Some callers
+ * cannot provide one, and cannot let this library allocate either: a program whose own memory pool already holds
+ * (nearly) all of the card (a torch caching allocator sized for config 5's workspace, a solver that reserves HBM at
+ * start-up) would see a cudaMalloc inside the library fail or eat memory the pool counts on; a program that keeps
+ * several streams busy would see every cudaMalloc / cudaFree synchronise the whole device.  fs_scan_static needs no
+ * handle and no workspace and calls no cudaMalloc, cudaFree or other allocating routine: the per-CTA partial maxima
+ * and the ticket counter of its arg-max live in a fixed array inside the library image, FS_SCAN_STATIC_SCRATCH_BYTES
+ * per GPU that loads the library, held until the process exits.  That array bounds the size: N <= FS_SCAN_STATIC_MAX_N
+ * (1024 spins per CTA, one 16-byte partial result each); larger N returns FS_ERR_ARG and launches nothing.
+ *
+ * Inputs, all DEVICE, caller-owned, read only: angle_dev [N] radians (Eq. 1), hc_dev [N] > 0 (h_k^(i) of Eq. 5),
+ * s_dev [N] int8 +1/-1, hdip_dev [N,2] = (par, perp) of h_dip in the fixed frame of theta_i, 16-byte aligned (what
+ * fs_get_fields(FS_FIELD_DIP) returns).  p: HOST; only b, c, beta, gamma are read.  (hx, hy): global external field;
+ * sigma_th, seed, step: thermal field exactly as fs_set_thermal + fs_set_field define it (sigma_th = 0: none).
+ * Output: result_dev DEVICE, 24 bytes, 8-byte aligned: { int64 number of switchable spins, int64 index of the spin
+ * furthest outside its astroid (lowest index among exact ties; -1 if none), double its Eq. 5 left-hand side (-inf if
+ * none) } -- the three values fs_scan returns for the same state, same arithmetic.  Asynchronous on `stream` (of the
+ * CURRENT device, which must own all the pointers); no synchronise.
+ *
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, which may load the library's
+ * kernels on that device).  Make that first call outside any stream capture; later calls only enqueue a 256-byte
+ * memset of the counter and one kernel.
+ * Sharing: all calls on one device use the same array.  Calls on one stream, or otherwise ordered, are safe in any
+ * number and any mix of sizes (the counter is cleared per call; stale partial results are never read).  Two calls that
+ * can overlap on the GPU (different streams, no event between them) race on the array and give undefined results. */
+#define FS_SCAN_STATIC_MAX_N 4194304
+#define FS_SCAN_STATIC_SCRATCH_BYTES 65792 /* 256 (counter) + 16 * FS_SCAN_STATIC_MAX_N / 1024 */
+int fs_scan_static(int64_t N, const double* angle_dev, const double* hc_dev, const int8_t* s_dev, const double* hdip_dev,
+                   const fs_params* p, double hx, double hy, double sigma_th, uint64_t seed, uint32_t step,
+                   void* result_dev, void* stream);
+
 /* Number of kernels this library launched since load (all sims), for the benchmark's launch count. */
 int64_t fs_kernel_launches(void);
 

@@ -25,8 +25,9 @@ EXPORTS = [
     "fs_get_fields", "fs_get_flip_log", "fs_get_neighbors", "fs_step_host", "fs_relax_host",
     "fs_kernel_launches", "fs_last_error", "fs_get_lattice", "fs_measure_fp64_peak", "fs_sweep", "fs_sweep_anneal", "fs_set_local_field",
     "fs_set_batch", "fs_get_batch_stats", "fs_sweep_ex", "fs_correlation", "fs_vertex_populations", "fs_get_flip_log_window",
-    "fs_measure_fp32_peak",
+    "fs_measure_fp32_peak", "fs_scan_static",
 ]
+SCAN_STATIC_MAX_N = 4194304          # FS_SCAN_STATIC_MAX_N of include/flatspin.h
 
 
 class FsParams(C.Structure):
@@ -88,6 +89,7 @@ def load_library(path: str | None = None):
         "fs_vertex_populations": [vp, vp, i64, vp],
         "fs_get_flip_log_window": [vp, i32, vp, i64, P(i64), P(i64)],
         "fs_get_batch_stats": [vp, vp],
+        "fs_scan_static": [i64, vp, vp, vp, vp, P(FsParams), dbl, dbl, dbl, C.c_uint64, C.c_uint32, vp, vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -126,6 +128,29 @@ def measure_fp32_peak(stream=None) -> float:
     sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     _check(L, L.fs_measure_fp32_peak(C.byref(v), sp))
     return float(v.value)
+
+
+def scan_static(angle, hc, s, hdip, params: dict, hx, hy, sigma_th=0.0, seed=0, step=0, result=None, stream=None):
+    """fs_scan_static: the switching scan without a handle, a workspace or any device allocation inside the library
+    (for programs whose own pool holds the card's memory, or that cannot take cudaMalloc's device-wide stall).  All
+    arguments are CUDA tensors the caller owns: angle [N] f64, hc [N] f64, s [N] int8, hdip [N,2] f64; `result` is
+    a 3-element int64 tensor (allocated here with torch if None; pass your own to keep this call allocation-free
+    on the Python side too).  Asynchronous; returns `result`: [n_switchable, best_index, bits of best_L] -- read the
+    last one with result[2:3].view(torch.float64).  N <= SCAN_STATIC_MAX_N, else FlatspinError(FS_ERR_ARG)."""
+    L = load_library()
+    for t, dt in ((angle, torch.float64), (hc, torch.float64), (s, torch.int8), (hdip, torch.float64)):
+        assert t.is_cuda and t.is_contiguous() and t.dtype == dt
+    N = int(angle.shape[0])
+    assert hc.numel() == N and s.numel() == N and hdip.numel() == 2 * N
+    if result is None:
+        result = torch.empty(3, dtype=torch.int64, device=angle.device)
+    assert result.is_cuda and result.dtype == torch.int64 and result.numel() >= 3
+    p = FsParams(*[float(params.get(k, 1.0)) for k in ("alpha", "b", "c", "beta", "gamma", "neighbor_distance")])
+    with torch.cuda.device(angle.device):
+        sp = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+        _check(L, L.fs_scan_static(N, angle.data_ptr(), hc.data_ptr(), s.data_ptr(), hdip.data_ptr(), C.byref(p),
+                                   float(hx), float(hy), float(sigma_th), int(seed), int(step), result.data_ptr(), sp))
+    return result
 
 
 class Sim:

@@ -2464,3 +2464,162 @@ int fs_relax_host(fs_sim* sim, double hx, double hy, uint32_t step, int8_t* s_ho
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// fs_scan_static: the switching scan (A4-A7) for callers that must not allocate device memory.
+//
+// Who needs it.  A host program that has handed (nearly) all of the GPU's memory to its own pool (a torch caching
+// allocator sized for the 11.5 GB config-5 workspace, a solver that reserves the card at start-up) cannot let a
+// library call cudaMalloc behind its back: the call fails, or it takes memory the pool counts on.  A program that keeps
+// several streams busy (one ensemble member per stream) cannot afford it either: cudaMalloc and cudaFree synchronise
+// the whole device.  Every other scan in this file works on a simulation handle, whose per-CTA partial results live
+// in the workspace that fs_create laid out; this entry point has no handle and no workspace.  Its partial results go
+// to the file-scope array below, which the CUDA module carries: FS_SCAN_STATIC_SCRATCH_BYTES (65,792 B) on every
+// device that loads the library, until the process exits.  The caller passes the inputs and the 24-byte result.
+//
+// The arithmetic is k_scan's, through the same device functions (sincos for the frame, 1 / h_c, fixed_field, margin,
+// warp_argmax_margin), so the result is the one fs_scan gives for the same h_dip.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int SCAN_STATIC_SPB = 1024;                                   // spins per CTA: 256 threads x 4 spins
+constexpr int SCAN_STATIC_THREADS = 256;
+constexpr int SCAN_STATIC_MAX_CTAS = FS_SCAN_STATIC_MAX_N / SCAN_STATIC_SPB;
+constexpr size_t SCAN_STATIC_HEADER = 256;                              // word 0: the ticket counter; must be 0 at launch
+static_assert(SCAN_STATIC_HEADER + sizeof(ScanGroup) * SCAN_STATIC_MAX_CTAS == FS_SCAN_STATIC_SCRATCH_BYTES,
+              "flatspin.h states the size of the static scratch array");
+
+// In HOST code this name is only a handle for cudaGetSymbolAddress: it is not a device address, and a kernel handed
+// `g_scan_static_scratch` itself would read host memory or fault.  static_scratch_of() below asks the runtime for the
+// address on the current device and the entry point passes that to the kernel.
+static __device__ __align__(256) unsigned char g_scan_static_scratch[FS_SCAN_STATIC_SCRATCH_BYTES];
+
+__global__ void __launch_bounds__(SCAN_STATIC_THREADS)
+k_scan_static(int64_t N, Astroid ast, FieldSpec fs, double2 he, const double* __restrict__ angle,
+              const double* __restrict__ hc, const int8_t* __restrict__ s, const double2* __restrict__ hdip,
+              unsigned char* __restrict__ scratch, long long* __restrict__ result) {
+    __shared__ double wv[SCAN_STATIC_SPB / 32];           // arg-max of every 32-spin slot of this CTA
+    __shared__ int wi[SCAN_STATIC_SPB / 32];
+    __shared__ unsigned wcnt[SCAN_STATIC_THREADS / 32];
+    __shared__ unsigned long long wc[SCAN_STATIC_THREADS / 32];
+    __shared__ int is_last;
+    unsigned* ticket = reinterpret_cast<unsigned*>(scratch);
+    ScanGroup* cres = reinterpret_cast<ScanGroup*>(scratch + SCAN_STATIC_HEADER);      // [gridDim.x]
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t base = (int64_t)blockIdx.x * SCAN_STATIC_SPB + threadIdx.x;
+    unsigned nsw = 0;
+#pragma unroll
+    for (int q = 0; q < SCAN_STATIC_SPB / SCAN_STATIC_THREADS; ++q) {
+        const int64_t i = base + q * SCAN_STATIC_THREADS;
+        double m = -CUDART_INF; int mi = 0x7fffffff;
+        if (i < N) {
+            double sn, c;
+            sincos(angle[i], &sn, &c);                     // k_frame's table entry (Eq. 1)
+            const double ih = 1.0 / hc[i];
+            const double2 hd = hdip[i];
+            const double2 hf = fixed_field(make_double2(c, sn), he, fs, 0, (uint32_t)i);
+            m = margin(hd.x + hf.x, hd.y + hf.y, (double)s[i], ih, ast);
+            mi = (int)i;
+        }
+        nsw += __popc(__ballot_sync(0xffffffffu, m > 1.0));
+        warp_argmax_margin(m, mi);
+        if (lane == 0) { wv[q * (SCAN_STATIC_THREADS / 32) + w] = m; wi[q * (SCAN_STATIC_THREADS / 32) + w] = mi; }
+    }
+    if (lane == 0) wcnt[w] = nsw;
+    __syncthreads();
+    if (w == 0) {
+        double v = wv[lane]; int bi = wi[lane];            // SCAN_STATIC_SPB / 32 == 32 slots
+        warp_argmax_margin(v, bi);
+        unsigned c = lane < SCAN_STATIC_THREADS / 32 ? wcnt[lane] : 0u;
+        c = __reduce_add_sync(0xffffffffu, c);
+        if (lane == 0) {
+            cres[blockIdx.x].v = v; cres[blockIdx.x].idx = bi; cres[blockIdx.x].cnt = c;
+            __threadfence();
+            is_last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+        }
+    }
+    __syncthreads();
+    if (!is_last) return;
+    // the last CTA to finish reduces the per-CTA results (only the gridDim.x entries this launch wrote: whatever an
+    // earlier, larger call left behind them is never read)
+    __threadfence();
+    double v = -CUDART_INF; int bi = 0x7fffffff;
+    unsigned long long cnt = 0;
+    for (int t = threadIdx.x; t < (int)gridDim.x; t += SCAN_STATIC_THREADS) {
+        const double tv = __ldcg(&cres[t].v); const int ti = __ldcg(&cres[t].idx);
+        cnt += __ldcg(&cres[t].cnt);
+        if (better(tv, ti, v, bi)) { v = tv; bi = ti; }
+    }
+    warp_argmax_margin(v, bi);
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    __syncthreads();                                       // wv / wi are reused
+    if (lane == 0) { wv[w] = v; wi[w] = bi; wc[w] = cnt; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < SCAN_STATIC_THREADS / 32; ++k) {
+            if (better(wv[k], wi[k], v, bi)) { v = wv[k]; bi = wi[k]; }
+            cnt += wc[k];
+        }
+        const bool any = v > 1.0;
+        result[0] = (long long)cnt;
+        result[1] = any ? bi : -1;
+        reinterpret_cast<double*>(result)[2] = any ? v : -CUDART_INF;
+        *ticket = 0u;                                      // leave the counter at zero (the entry point clears it as well)
+    }
+}
+
+// Device address of g_scan_static_scratch on the CURRENT device: asked for once per device, with that device current,
+// and kept.  cudaGetSymbolAddress loads this module on the device if nothing has yet (no cudaMalloc of ours).
+std::mutex g_static_mutex;
+unsigned char* g_static_scratch_dev[64] = {nullptr};
+int static_scratch_of(int dev, unsigned char** out) {
+    if (dev < 0 || dev >= 64) return fail(FS_ERR_CUDA, "device ordinal %d outside the table of 64", dev);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_scratch_dev[dev]) {
+        void* p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, g_scan_static_scratch));
+        if (!p) return fail(FS_ERR_CUDA, "cudaGetSymbolAddress returned a null address for the static scan scratch");
+        g_static_scratch_dev[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_static_scratch_dev[dev];
+    return FS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int fs_scan_static(int64_t N, const double* angle_dev, const double* hc_dev, const int8_t* s_dev, const double* hdip_dev,
+                   const fs_params* p, double hx, double hy, double sigma_th, uint64_t seed, uint32_t step,
+                   void* result_dev, void* stream) {
+    if (N <= 0) return fail(FS_ERR_ARG, "N=%lld must be positive", (long long)N);
+    if (N > (int64_t)FS_SCAN_STATIC_MAX_N)
+        return fail(FS_ERR_ARG, "N=%lld exceeds FS_SCAN_STATIC_MAX_N=%d, the most the static scratch array holds "
+                    "(use fs_create + fs_scan with a caller-allocated workspace for larger systems)", (long long)N,
+                    (int)FS_SCAN_STATIC_MAX_N);
+    if (!angle_dev || !hc_dev || !s_dev || !hdip_dev || !p || !result_dev) return fail(FS_ERR_ARG, "null pointer argument");
+    if (!(p->b > 0) || !(p->c > 0) || !(p->beta > 0) || !(p->gamma > 0)) return fail(FS_ERR_ARG, "b, c, beta, gamma must be > 0");
+    if (!(sigma_th >= 0) || !std::isfinite(sigma_th)) return fail(FS_ERR_ARG, "sigma_th must be finite and >= 0");
+    if (((uintptr_t)result_dev & 7) || ((uintptr_t)hdip_dev & 15)) return fail(FS_ERR_ARG, "result_dev needs 8-byte, hdip_dev 16-byte alignment");
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    unsigned char* scratch = nullptr;
+    int rc = static_scratch_of(dev, &scratch);
+    if (rc) return rc;
+    auto kind = [](double denom) { return denom == 3.0 ? 1 : (denom == 2.0 ? 2 : (denom == 1.0 ? 3 : 0)); };
+    const Astroid ast{1.0 / p->b, 1.0 / p->c, 2.0 / p->gamma, 2.0 / p->beta, kind(p->gamma), kind(p->beta),
+                      std::pow(0.5, p->gamma / 2.0) * (1.0 - 1e-9), std::pow(0.5, p->beta / 2.0) * (1.0 - 1e-9)};
+    const FieldSpec fs{sigma_th, seed, step};
+    cudaStream_t st = (cudaStream_t)stream;
+    // the ticket counter must start at zero whatever an earlier (possibly failed) call left in the shared array
+    CUDA_TRY(cudaMemsetAsync(scratch, 0, SCAN_STATIC_HEADER, st));
+    const int ncta = (int)((N + SCAN_STATIC_SPB - 1) / SCAN_STATIC_SPB);
+    k_scan_static<<<ncta, SCAN_STATIC_THREADS, 0, st>>>(N, ast, fs, make_double2(hx, hy), angle_dev, hc_dev, s_dev,
+                                                        reinterpret_cast<const double2*>(hdip_dev), scratch,
+                                                        static_cast<long long*>(result_dev));
+    LAUNCHED();
+    CUDA_TRY(cudaGetLastError());
+    return FS_OK;
+}
+
+}  // extern "C"
