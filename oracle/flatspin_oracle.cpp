@@ -16,7 +16,9 @@
 // Pins (tests/test_oracle_pins.py, -m "not gpu"): two-dipole closed forms, lattice sums, astroid
 // special cases, Philox known answers, brute-force neighbours, exhaustive <=12-spin flip orders,
 // energy descent, global spin-flip symmetry, kagome 29x29 = 2638 magnets; spin-spin correlation
-// and vertex populations on hand-countable states (polarised, ground state, one flipped spin).
+// and vertex populations on hand-countable states (polarised, ground state, one flipped spin); the near-tie monitor
+// (note_decision / second_best / orc_monitor) against closed-form gaps of uncoupled spins, a winner placed at
+// 1 +- eps, exact ties and a brute-force second maximum, in both tiers.
 // Unpinned by the paper: full-config flip sequences (no published values exist); they are pinned only
 // through Tier A == Tier B on small sizes plus the invariants above ("parity unpinned" for those).
 //
