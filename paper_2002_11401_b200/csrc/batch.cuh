@@ -170,7 +170,9 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
     long long tprof = bt_now();
 #endif
     for (;; ++rounds) {
-        const unsigned tag = 0xFFFFFu - (round_base + (unsigned)rounds);   // newer rounds win an atomicMin on the claim word
+        // newer rounds win an atomicMin on the claim word.  Tag 0xFFFFF is never issued: it is the tag field of 0xFFFFFFFF,
+        // the "unowned" word the claim table is filled with (round_base + rounds <= 0xF0000 + 0xFFF0, so tag >= 0xE)
+        const unsigned tag = 0xFFFFEu - (round_base + (unsigned)rounds);
         if (rounds >= 0xFFF0) break;
         // ================= phase 1: threshold theta such that <= P candidates have key > theta ==============
         // One pass over all margins builds a histogram of log-spaced bins of (key - 1); theta is the lower edge
@@ -391,7 +393,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) k_relax_batch(BatchArgs a) {
                     if (i < 0) continue;
                     unsigned o = __ldcg(a.owner + i);
                     for (;;) {
-                        if ((o >> 12) == tag) { ok &= sh_label[o & 0xFFFu] == leader; break; }
+                        if (o != 0xFFFFFFFFu && (o >> 12) == tag) { ok &= sh_label[o & 0xFFFu] == leader; break; }   // an unowned word always takes the CAS
                         const unsigned prev = atomicCAS(a.owner + i, o, (tag << 12) | (unsigned)leader);
                         if (prev == o) break;
                         o = prev;

@@ -520,15 +520,15 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
     // Programmatic dependent launch: this kernel may become resident while the gather kernel in front of it is still
     // running (the gathers call griddepcontrol.launch_dependents at their start, so that happens as soon as their last CTA
     // has started: in the tail of the gather, when SMs fall idle).  Until the wait below it reads only what no gather
-    // writes (frames, 1/h_c, spins): that cold-DRAM round trip and the launch latency overlap the gather's tail.  h_dip is
+    // writes (frames, 1/h_c): that cold-DRAM round trip and the launch latency overlap the gather's tail.  h_dip is
     // read, and everything is written, after the wait.  Behind any other kernel the wait falls through at once.
     asm volatile("griddepcontrol.launch_dependents;");   // a k_relax behind this scan may become resident (it waits at its top)
     double2 c[SCAN_SPT], hd[SCAN_SPT]; double ih[SCAN_SPT], sp[SCAN_SPT];
 #pragma unroll
     for (int q = 0; q < SCAN_SPT; ++q) {
         const int64_t i = base + q * SCAN_THREADS;
-        if (i < N) { c[q] = cs[i]; ih[q] = hc_all[off + i]; sp[q] = (double)s_all[off + i]; }
-        else { c[q] = make_double2(1.0, 0.0); ih[q] = 1.0; sp[q] = 1.0; }
+        if (i < N) { c[q] = cs[i]; ih[q] = hc_all[off + i]; }
+        else { c[q] = make_double2(1.0, 0.0); ih[q] = 1.0; }
     }
     asm volatile("griddepcontrol.wait;" ::: "memory");
     // fs_set_field launches nothing: its field arrives here by value, and one thread records it for the later readers
@@ -537,7 +537,8 @@ __global__ void __launch_bounds__(SCAN_SPB / SCAN_SPT) k_scan(int64_t N, int LB,
 #pragma unroll
     for (int q = 0; q < SCAN_SPT; ++q) {
         const int64_t i = base + q * SCAN_THREADS;
-        if (i < N) hd[q] = hdip_all[off + i]; else hd[q] = make_double2(0.0, 0.0);
+        // the spins too: the kernel in front may be a relax kernel or fs_set_spins' fill, which write them
+        if (i < N) { hd[q] = hdip_all[off + i]; sp[q] = (double)s_all[off + i]; } else { hd[q] = make_double2(0.0, 0.0); sp[q] = 1.0; }
     }
     unsigned long long nsw = 0;
 #pragma unroll
