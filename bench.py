@@ -125,32 +125,70 @@ def oracle_field_sample(w, budget_s=12.0, chunk=256, seed=123):
     return n_int / dt, n_sp, n_int, dt
 
 
-def oracle_cached_legs(scale=160, budget_s=6.0):
-    """The oracle's precomputed-neighbour-list field pass and switching scan (SURVEY.md 8(d) legs (i), (ii)): couplings
-    built once (untimed), then gather_cached (h_dip = sum_j s_j w_ij over the list) + scan_cached (Eq. 2, 5, 6 per spin,
-    arg-max), timed single-threaded and with OpenMP over spins on all host cores.  Bounded sample: the config-5 recipe
-    (square ASI, neighbor distance 10, random spins) at scale x scale."""
-    from oracle import Oracle
-    w = W.config("5", scale=scale)
-    orc = Oracle(w.pos, w.angle, w.hc, w.params, spins=w.spins)
-    hx, hy = w.fields[0]
-    orc.set_field(hx, hy, 0)
-    t0 = time.perf_counter(); orc.build_weights(); t_build = time.perf_counter() - t0
-    I = orc.num_interactions
-    cores = os.cpu_count() or 1
-    out = {"sample": f"config 5 recipe at {scale}x{scale} ({w.N} spins, {I} interactions), couplings precomputed "
-                     f"(untimed, {t_build:.1f} s); each repetition = gather over the list + switching scan",
-           "N": w.N, "interactions": I, "host_cores": cores}
-    for label, nt in (("threads_1", 1), ("threads_all", cores)):
-        orc.set_threads(nt)
-        orc.gather_cached(); orc.scan_cached()
-        reps = 0; tg = ts = 0.0
-        t_end = time.perf_counter() + budget_s
-        while time.perf_counter() < t_end or reps < 2:
-            a = time.perf_counter(); orc.gather_cached(); b = time.perf_counter(); orc.scan_cached(); c = time.perf_counter()
-            tg += b - a; ts += c - b; reps += 1
-        out[label] = {"threads": nt, "repetitions": reps, "interactions_per_s": I * reps / (tg + ts),
-                      "gather_interactions_per_s": I * reps / tg, "scan_spins_per_s": w.N * reps / ts}
+CFG5_K = 632                       # maximum degree of config 5 (316 + 316), asserted against the library in run_ours
+L2_NOTE = ("GPU arm: flushed before every timed step (256 MiB fill, untimed), step time = sum of per-step CUDA-event "
+           "intervals; reference arm: the 6.2 GB coupling list is streamed from host DRAM every pass")
+
+
+def workload_config(w, K, I):
+    """The `config` object of the JSON line, the same for the GPU arm and the reference arm: what is computed, on which
+    input.  How each arm ran it (kernel variant, lattice tables, launch details) goes under `run`."""
+    return {"workload": w.name, "N": int(w.N), "K": None if K is None else int(K), "interactions": int(I),
+            "neighbor_distance": float(w.params["neighbor_distance"]),
+            "step": "full dipolar-field gather over every spin + switching scan (fs_update_fields + fs_scan)", "l2": L2_NOTE}
+
+
+def cpu_field_workload(scale=None, need_gb=10.0):
+    """Config 5 itself (501,000 spins, 311,247,284 interactions: ~7 GB of host memory for the oracle's precomputed
+    couplings) when the host can hold it, else the same recipe at 160 x 160 under a name that says so."""
+    import psutil
+    if scale is None and psutil.virtual_memory().available < need_gb * 2**30:
+        w = W.config("5", scale=160)
+        w.name = "cfg5_recipe_160x160_sample"
+        return w
+    return W.config("5", scale=scale)
+
+
+class OracleFieldPass:
+    """The oracle's precomputed-neighbour-list field pass and switching scan (SURVEY.md 8(d) legs (i), (ii)), as it
+    stands: couplings built once (untimed), then one pass = gather_cached (h_dip = sum_j s_j w_ij over the list) +
+    scan_cached (Eq. 2, 5, 6 per spin, arg-max), single-threaded or with OpenMP over spins on all host cores."""
+
+    def __init__(self, w):
+        from oracle import Oracle
+        self.w = w
+        self.orc = Oracle(w.pos, w.angle, w.hc, w.params, spins=w.spins)
+        hx, hy = w.fields[0]
+        self.orc.set_field(hx, hy, 0)
+        t0 = time.perf_counter(); self.orc.build_weights(); self.t_build = time.perf_counter() - t0
+        self.I = self.orc.num_interactions
+        self.cores = os.cpu_count() or 1
+        self.sample = (f"{w.name}: {w.N} spins, {self.I} interactions, couplings precomputed (untimed, {self.t_build:.1f} s); "
+                       "each repetition = one gather over the whole list + one switching scan")
+
+    def one_pass(self):
+        a = time.perf_counter(); self.orc.gather_cached(); b = time.perf_counter(); self.orc.scan_cached(); c = time.perf_counter()
+        return b - a, c - b
+
+    def leg(self, threads, reps, warm=1):
+        self.orc.set_threads(threads)
+        for _ in range(warm):
+            self.one_pass()
+        tg = ts = 0.0
+        for _ in range(reps):
+            g, sc = self.one_pass(); tg += g; ts += sc
+        return {"threads": threads, "repetitions": reps, "interactions_per_s": self.I * reps / (tg + ts),
+                "gather_interactions_per_s": self.I * reps / tg, "scan_spins_per_s": self.w.N * reps / ts,
+                "s_per_pass": (tg + ts) / reps}
+
+
+def oracle_cached_legs(scale=None, reps=3):
+    """Both legs on the full config 5 (or the named sample if the host cannot hold it): `reps` passes with 1 thread and
+    with all cores ("Config 5 ... over 3 repetitions")."""
+    fp = OracleFieldPass(cpu_field_workload(scale))
+    out = {"sample": fp.sample, "workload": fp.w.name, "N": fp.w.N, "interactions": fp.I, "host_cores": fp.cores}
+    out["threads_1"] = fp.leg(1, reps)
+    out["threads_all"] = fp.leg(fp.cores, reps)
     return out
 
 
@@ -171,27 +209,27 @@ def oracle_relax_sample(scale=400):
 
 
 def run_reference(args, rank, world):
-    """The oracle as it stands on the host cores: the precomputed-list gather + scan with OpenMP over all cores (the
-    stronger of its two field tiers), on a bounded sample of config 5; each step = one bounded run."""
+    """The oracle as it stands on the host cores, on the GPU arm's workload: config 5 at full size, the precomputed-list
+    gather + scan with OpenMP over all cores (the stronger of its two field tiers).  One step = one whole pass (gather
+    + scan) over the 311 M interactions; the couplings are built once before the timed region, as fs_create builds the
+    GPU arm's tables before its timed region."""
     if rank != 0:
         return
-    w5 = W.config("5", scale=64)
-    for _ in range(min(args.warmup, 1)):
-        oracle_cached_legs(scale=96, budget_s=0.5)
-    tot_i = tot_t = 0.0; last = None
-    for k in range(args.steps):
-        r = oracle_cached_legs(scale=160, budget_s=max(1.0, 20.0 / max(args.steps, 1)))
-        a = r["threads_all"]
-        tot_i += r["interactions"] * a["repetitions"]; tot_t += r["interactions"] * a["repetitions"] / a["interactions_per_s"]
-        last = r
-    value = tot_i / tot_t
-    full = W.config("5")
+    fp = OracleFieldPass(cpu_field_workload(args.scale))
+    fp.orc.set_threads(fp.cores)
+    for _ in range(max(args.warmup, 1)):
+        fp.one_pass()
+    tot = 0.0
+    for _ in range(args.steps):
+        g, sc = fp.one_pass(); tot += g + sc
+    value = fp.I * args.steps / tot
+    one = fp.leg(1, min(args.steps, 3))
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
+            "warmup": max(args.warmup, 1), "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": full.name, "N": full.N, "neighbor_distance": 10.0},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": last["host_cores"], "kind": "oracle",
-                             "sample": last["sample"], "threads_1": last["threads_1"], "threads_all": last["threads_all"]},
+            "config": workload_config(fp.w, CFG5_K if fp.w.N == 501000 else None, fp.I),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": fp.cores, "kind": "oracle", "sample": fp.sample,
+                             "threads_1": one},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
@@ -486,6 +524,7 @@ def run_ours(args, rank, world, local_rank):
     hx, hy = w.fields[0]
     sim.set_field(hx, hy, 0)
     I, N, K = sim.n_interactions, sim.N, sim.K
+    assert N != 501000 or K == CFG5_K, K                   # the reference arm states config 5's K without a neighbour build of its own
     ell_bytes = I * 20.0 + N * 17.0     # idx + weight pair per interaction; s read + h_dip written per spin
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > L2 (126 MB)
 
@@ -606,13 +645,10 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "N": N, "K": K, "interactions": I, "neighbor_distance": w.params["neighbor_distance"],
-                   "step": "fs_update_fields + fs_scan",
-                   "gather": ("lattice stencil" + (", inversion-paired" if lat.get("inversion_pairs") and args.gather != 3 else "")) if use_stencil else "ELL fp64",
-                   "lattice": lat,
-                   "l2": "flushed before every timed step (256 MiB fill, untimed); step time = sum of per-step CUDA-event intervals",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU", "create_s": t_create,
-                   "n_switchable": n_sw, "best_index": best},
+        "config": workload_config(w, K, I),
+        "run": {"gather": ("lattice stencil" + (", inversion-paired" if lat.get("inversion_pairs") and args.gather != 3 else "")) if use_stencil else "ELL fp64",
+                "lattice": lat, "parallelism": "replicas only" if world > 1 else "1 GPU", "create_s": t_create,
+                "n_switchable": n_sw, "best_index": best},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(N), "d2h_bytes_per_step": int(16 * N + 24),
                 "ms_per_step": e2e_ms / args.steps, "call": "fs_step_host (pinned host spins in, host total fields out)",
@@ -641,7 +677,7 @@ def run_ours(args, rank, world, local_rank):
                                 "accuracy": "fields within 1e-5 of the fp64 oracle relative to max|h| (tests/test_gpu_parity.py); no flip-order claim"}
     sim.close()
     if rank == 0 and not args.no_cpu:
-        legs = oracle_cached_legs(scale=160, budget_s=args.cpu_budget / 2)
+        legs = oracle_cached_legs(scale=args.scale, reps=3)
         v, n_sp, n_int, dt = oracle_field_sample(w, budget_s=min(args.cpu_budget, 6.0))
         line["cpu_baseline"] = {"value": legs["threads_all"]["interactions_per_s"], "unit": UNIT, "cores": legs["host_cores"],
                                 "kind": "oracle", "sample": legs["sample"],
