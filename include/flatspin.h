@@ -12,8 +12,16 @@
  *   - Every DEVICE pointer is caller-owned CUDA global memory (a torch tensor's data_ptr()).  Inputs
  *     of fs_create* are consumed during the call and may be freed afterwards.  The workspace is
  *     caller-owned and must outlive the handle.  Outputs are written to caller-owned buffers.
- *     The only library-owned device memory is the lattice-stencil table set (index grids of <= 8N
- *     cells + a few KB of couplings), allocated by fs_create and freed by fs_destroy.
+ *     Library-owned device memory (cudaMalloc inside the library, NOT counted by fs_workspace_bytes, freed by
+ *     fs_destroy unless stated otherwise):
+ *       - lattice-stencil tables, spin grids and cell index (index grids of <= 8N + 2^20 cells + a few KB of couplings),
+ *         only when fs_create finds a regular lattice; the detection scratch (9N bytes) is freed before fs_create returns;
+ *       - the scratch of the batched-flip kernel, only for R = 1, 1 <= K <= 64, N >= 16384: 8.125 N bytes + 32 B x P x 16
+ *         x (K padded + 1) undo records with P = min(4096, 8 sqrt(N / (K + 1))) (35 MB at config 4).  If this allocation
+ *         fails, fs_create still succeeds and fs_relax runs one flip at a time: fs_get_batch_stats out4[0] == 0 says so;
+ *       - the per-spin external field of fs_set_local_field (16 N bytes; freed when it is cleared);
+ *       - temporaries of fs_workspace_bytes / fs_create / fs_measure_*_peak, freed before the call returns.
+ *     fs_scan_static (below) is the one entry point that touches no allocator at all.
  *   - HOST pointers to scalars (n_flips_out ...) are written after a stream synchronise; passing NULL
  *     skips the synchronise (the call is then fully asynchronous on `stream`).
  *   - All work is enqueued on the stream given at creation (a cudaStream_t passed as void*; NULL =
