@@ -204,6 +204,88 @@ def rotating(amplitude: float, periods: float, steps_per_period: int, phi0_deg: 
     return np.ascontiguousarray(np.stack([amplitude * np.cos(phi), amplitude * np.sin(phi)], axis=1))
 
 
+# --------------------------------------------------------------------------- geometries that are NOT lattices
+# The library takes any pos[N,2] / angle[N] ("each magnet has a position and a rotation"); flatspin's stock
+# geometries are lattices, user-defined ones need not be.  These two exercise the general path: cell-grid neighbour
+# lists with ragged rows, the ELL gather, relax / batched flips / sweeps without the lattice's cell index.
+def jittered_square(n: int, sigma_pos: float = 0.03, sigma_angle: float = 0.08, seed: int = 0):
+    """Closed square ASI n x n with every magnet displaced by N(0, sigma_pos) per coordinate and rotated by
+    N(0, sigma_angle) radians: fabrication disorder in the geometry itself.  2n(n+1) magnets."""
+    pos, ang = square_closed(n)
+    rng = np.random.default_rng(seed)
+    return (np.ascontiguousarray(pos + sigma_pos * rng.standard_normal(pos.shape)),
+            np.ascontiguousarray(ang + sigma_angle * rng.standard_normal(ang.shape)))
+
+
+def point_cloud(n_target: int, r_min: float = 0.7, seed: int = 0, rounds: int = 40):
+    """Random point cloud with a minimum distance (Poisson-disc sampling by vectorised dart throwing) and uniformly
+    random angles in [0, pi).  The box is sized for about n_target points at ~0.62 / r_min^2 points per unit area.
+    A background grid of cell side r_min / sqrt(2) holds at most one accepted point per cell; each round throws
+    darts, drops those in occupied cells or within r_min of an accepted point (5 x 5 cells around the dart), and
+    among the darts of one round drops every dart that has an earlier dart of the round within r_min.
+    Returns (pos [N,2], angle [N]) with N close to n_target (deterministic for a given seed)."""
+    rng = np.random.default_rng(seed)
+    side = math.sqrt(n_target * r_min * r_min / 0.62)
+    cell = r_min / math.sqrt(2.0)
+    G = int(math.ceil(side / cell))
+    grid = np.full((G + 4, G + 4), -1, np.int64)            # 2 cells of border: no bounds checks on the 5 x 5 window
+    pts = np.zeros((0, 2))
+    offs = [(a, b) for a in range(-2, 3) for b in range(-2, 3)]
+    for _ in range(rounds):
+        m = max(4 * n_target // 3, 64)
+        d = rng.random((m, 2)) * side
+        cx = (d[:, 0] / cell).astype(np.int64) + 2; cy = (d[:, 1] / cell).astype(np.int64) + 2
+        ok = np.ones(m, bool)
+        for a, b in offs:                                    # against the accepted points
+            j = grid[cx + a, cy + b]
+            has = j >= 0
+            if has.any():
+                dd = d[has] - pts[j[has]]
+                ok[np.flatnonzero(has)[(dd * dd).sum(1) < r_min * r_min]] = False
+        d, cx, cy = d[ok], cx[ok], cy[ok]
+        # among this round's darts: keep a dart only if no EARLIER dart of the round lies within r_min
+        tmp = np.full_like(grid, -1)
+        keep = np.ones(len(d), bool)
+        order = np.arange(len(d))
+        first = np.full_like(grid, len(d))
+        np.minimum.at(first, (cx, cy), order)
+        keep &= first[cx, cy] == order                       # one dart per cell: the earliest
+        d, cx, cy = d[keep], cx[keep], cy[keep]
+        tmp[cx, cy] = np.arange(len(d))
+        keep = np.ones(len(d), bool)
+        for a, b in offs:
+            if (a, b) == (0, 0):
+                continue
+            j = tmp[cx + a, cy + b]
+            has = (j >= 0) & (j < np.arange(len(d)))
+            if has.any():
+                dd = d[has] - d[j[has]]
+                keep[np.flatnonzero(has)[(dd * dd).sum(1) < r_min * r_min]] = False
+        d, cx, cy = d[keep], cx[keep], cy[keep]
+        grid[cx, cy] = len(pts) + np.arange(len(d))
+        pts = np.concatenate([pts, d])
+    ang = rng.random(len(pts)) * math.pi
+    return np.ascontiguousarray(pts), np.ascontiguousarray(ang)
+
+
+def off_lattice(kind: str, n: int, seed: int = 0, K_steps: int = 40, sigma_th: float = 0.005) -> "Workload":
+    """A whole workload on a non-lattice geometry: `kind` = "jittered_square" (n x n cells) or "point_cloud" (about n
+    magnets), 5 % h_k disorder, all spins +1, thermal ramp 0.2 -> -0.2 at 45 degrees in K_steps steps (the config-4
+    protocol, shortened)."""
+    if kind == "jittered_square":
+        pos, ang = jittered_square(n, seed=seed)
+        nd = 1.6
+    elif kind == "point_cloud":
+        pos, ang = point_cloud(n, seed=seed)
+        nd = 1.5
+    else:
+        raise ValueError(kind)
+    N = len(ang)
+    return Workload(f"{kind}_{n}_seed{seed}", pos, ang, coercive_fields(N, seed=seed), np.ones(N, np.int8),
+                    _params(0.001, 1, 1, 3, 3, nd), ramp(0.2, -0.2, K_steps, 45.0, legs=1), sigma_th=sigma_th,
+                    thermal_seed=seed)
+
+
 # --------------------------------------------------------------------------- the five configs
 @dataclass
 class Workload:
