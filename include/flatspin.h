@@ -12,15 +12,13 @@
  *   - Every DEVICE pointer is caller-owned CUDA global memory (a torch tensor's data_ptr()).  Inputs
  *     of fs_create* are consumed during the call and may be freed afterwards.  The workspace is
  *     caller-owned and must outlive the handle.  Outputs are written to caller-owned buffers.
- *     Library-owned device memory (cudaMalloc inside the library, NOT counted by fs_workspace_bytes, freed by
- *     fs_destroy unless stated otherwise):
- *       - lattice-stencil tables, spin grids and cell index (index grids of <= 8N + 2^20 cells + a few KB of couplings),
- *         only when fs_create finds a regular lattice; the detection scratch (9N bytes) is freed before fs_create returns;
- *       - the scratch of the batched-flip kernel, only for R = 1, 1 <= K <= 64, N >= 16384: 8.125 N bytes + 32 B x P x 16
- *         x (K padded + 1) undo records with P = min(4096, 8 sqrt(N / (K + 1))) (35 MB at config 4).  If this allocation
- *         fails, fs_create still succeeds and fs_relax runs one flip at a time: fs_get_batch_stats out4[0] == 0 says so;
- *       - the per-spin external field of fs_set_local_field (16 N bytes; freed when it is cleared);
- *       - temporaries of fs_workspace_bytes / fs_create / fs_measure_*_peak, freed before the call returns.
+ *     The workspace holds every per-spin and per-interaction array, the flip log, the batched-flip scratch (35 MB at
+ *     config 4) and the per-spin external field of fs_set_local_field.  The one thing the library allocates itself
+ *     (cudaMalloc in fs_create, freed by fs_destroy, NOT counted by fs_workspace_bytes) is the lattice-stencil table set,
+ *     whose size is known only after the lattice detection: index grids and dense spin grids of <= 8N + 2^20 cells per
+ *     replica, a cell index (4N bytes) and a few KB of couplings (30 MB at config 5); none when the geometry is not a
+ *     lattice.  Temporaries of fs_workspace_bytes / fs_create (detection scratch, 9N bytes) / fs_measure_*_peak are
+ *     freed before the call returns.
  *     fs_scan_static (below) is the one entry point that touches no allocator at all.
  *   - HOST pointers to scalars (n_flips_out ...) are written after a stream synchronise; passing NULL
  *     skips the synchronise (the call is then fully asynchronous on `stream`).
@@ -138,7 +136,7 @@ int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step);
 
 /* Per-spin external field h_ext^(i) ("global, per-spin or a spatial vector field"): h_dev DEVICE
  * [N,2] (global x,y components), shared by all replicas, ADDED to the global field of fs_set_field / fs_sweep
- * before the rotation into the spin's frame (reading D-4).  Copied (library-owned buffer); NULL
+ * before the rotation into the spin's frame (reading D-4).  Copied (into the workspace); NULL
  * clears it.  Takes effect at the next scan / relax / sweep. */
 int fs_set_local_field(fs_sim* sim, const double* h_dev);
 

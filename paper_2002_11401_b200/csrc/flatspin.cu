@@ -1112,7 +1112,8 @@ struct fs_sim {
     bool field_pending = false;     // fs_set_field's value has not reached sim->hext yet: the next k_scan takes it by value
     double2 field_value{};
     Counters* ctr_host = nullptr;   // pinned staging [R]
-    double2* hloc = nullptr;        // per-spin external field [N] (library-owned), NULL = none
+    double2* hloc = nullptr;        // per-spin external field [N] in use (= hloc_buf), NULL = none
+    double2* hloc_buf = nullptr;    // its place in the caller's workspace
     int gather_variant = FS_GATHER_AUTO;
     size_t relax_smem = 0;
     // regular-lattice stencil (lattice.cuh); library-owned device memory, freed by fs_destroy
@@ -1148,8 +1149,35 @@ struct Layout {
     size_t scratch, cell_of, cell_cnt, cell_start, cell_fill, items, deg;
     size_t grid_end;
     // K-dependent
-    size_t pos, cs, nbr, w, wT, hc, s, hdip, hfix, M, bval, bidx, scnt, flog, ctr, hext, total;
+    size_t pos, cs, nbr, w, wT, hc, s, hdip, hfix, M, bval, bidx, scnt, flog, ctr, hext, hloc, batch, total;
 };
+
+// Scratch of k_relax_batch (batch.cuh), carved from the caller's workspace.  The batched kernel applies to one large
+// system with a moderate degree; elsewhere the region is empty.
+struct BatchLayout { size_t ctl, owner, seeds, edges, ecount, npos, elems, undo, blocks, clist, cand, cbits, total; int Pdef, P; };
+inline bool batch_applies(int64_t N, int R, int K) { return R == 1 && K >= 1 && K <= 64 && N >= 16384; }
+int batch_default_seeds(int64_t N, int K) {
+    const double p = 4.0 * std::sqrt((double)N / (double)(K + 1));
+    return (int)std::max(64.0, std::min((double)BT_PMAX, std::floor(p)));
+}
+BatchLayout batch_layout(int64_t N, int K, int Kp) {
+    // seeds per round: commits per round grow with the seeds, collisions between growing regions with their square;
+    // measured optimum on config 4 at three sizes (125 k, 501 k, 2.0 M spins: 384-512, 768-1024, 1792-2048 seeds):
+    // about 4 sqrt(N / (K + 1)).  Scratch is sized for twice that so that fs_set_batch can raise it.
+    BatchLayout b{};
+    b.Pdef = batch_default_seeds(N, K);
+    b.P = std::min<int>(BT_PMAX, 2 * b.Pdef);
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    b.ctl = take(sizeof(BatchCtl)); b.owner = take(4 * (size_t)N); b.seeds = take(sizeof(BatchSeed) * BT_PMAX);
+    b.edges = take(2 * (size_t)BT_PMAX * BT_EMAX); b.ecount = take(BT_PMAX); b.npos = take(4 * (size_t)BT_PMAX);
+    b.elems = take(sizeof(BatchElem) * (size_t)b.P * BT_LMAX);
+    b.undo = take(sizeof(BatchUndo) * (size_t)b.P * BT_LMAX * (size_t)(Kp + 1));
+    b.blocks = take(sizeof(BatchBlock) * BT_PMAX); b.clist = take(sizeof(BatchCommit) * (size_t)b.P * BT_LMAX);
+    b.cand = take(4 * (size_t)N); b.cbits = take(4 * (size_t)((N + 31) / 32));
+    b.total = o;
+    return b;
+}
 
 int choose_leaf(int64_t N, int* LB, int* nblk) {
     for (int lb = 32; lb <= 1024; lb <<= 1) {
@@ -1172,7 +1200,7 @@ void layout_grid(Layout& L, int64_t N, int ncells) {
     L.grid_end = o;
 }
 
-void layout_rest(Layout& L, int64_t N, int R, int Kp, int nblk, int64_t log_cap) {
+void layout_rest(Layout& L, int64_t N, int R, int K, int Kp, int nblk, int64_t log_cap) {
     size_t o = L.grid_end;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     size_t NK = (size_t)N * Kp, RN = (size_t)R * N;
@@ -1192,6 +1220,8 @@ void layout_rest(Layout& L, int64_t N, int R, int Kp, int nblk, int64_t log_cap)
     L.scnt = take(4 * (size_t)R * scan_aux_stride((int)((N + SCAN_SPB_MIN - 1) / SCAN_SPB_MIN)));
     L.ctr = take(sizeof(Counters) * (size_t)R);
     L.hext = take(16 * (size_t)R);
+    L.hloc = take(16 * (size_t)N);                       // per-spin external field of fs_set_local_field
+    L.batch = take(batch_applies(N, R, K) ? batch_layout(N, K, Kp).total : 0);
     L.total = o;
 }
 
@@ -1810,35 +1840,21 @@ int do_relax(fs_sim* sim, int64_t max_flips) {
     return launch_relax(sim, max_flips, 0, nullptr, 0, nullptr, nullptr, batch ? 1 : 0);
 }
 
-int batch_default_seeds(int64_t N, int K) {
-    const double p = 4.0 * std::sqrt((double)N / (double)(K + 1));
-    return (int)std::max(64.0, std::min((double)BT_PMAX, std::floor(p)));
-}
-
 // scratch of k_relax_batch; never fails the creation (no scratch = sequential relax only)
 int setup_batch(fs_sim* sim) {
     sim->bt_ok = false;
-    if (sim->R != 1 || sim->K < 1 || sim->K > 64 || sim->N < 16384) return FS_OK;
+    if (!batch_applies(sim->N, sim->R, sim->K) || !sim->bt_mem) return FS_OK;
     int coop = 0, occ = 0;
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, sim->device);
     if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_relax_batch, BT_THREADS, 0) != cudaSuccess || occ < 1) {
         cudaGetLastError(); return FS_OK;
     }
-    // seeds per round: commits per round grow with the seeds, collisions between growing regions with their square;
-    // measured optimum on config 4 at three sizes (125 k, 501 k, 2.0 M spins: 384-512, 768-1024, 1792-2048 seeds):
-    // about 4 sqrt(N / (K + 1)).  Scratch is sized for twice that so that fs_set_batch can raise it.
-    const int Pdef = batch_default_seeds(sim->N, sim->K);
-    const int P = std::min<int>(BT_PMAX, 2 * Pdef);
-    const size_t und = sizeof(BatchUndo) * (size_t)P * BT_LMAX * (size_t)(sim->Kp + 1);
-    size_t o = 0;
-    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
-    const size_t o_ctl = take(sizeof(BatchCtl)), o_owner = take(4 * (size_t)sim->N), o_seeds = take(sizeof(BatchSeed) * BT_PMAX),
-                 o_edges = take(2 * (size_t)BT_PMAX * BT_EMAX), o_ecount = take(BT_PMAX), o_npos = take(4 * (size_t)BT_PMAX),
-                 o_elems = take(sizeof(BatchElem) * (size_t)P * BT_LMAX), o_undo = take(und),
-                 o_blocks = take(sizeof(BatchBlock) * BT_PMAX), o_clist = take(sizeof(BatchCommit) * (size_t)P * BT_LMAX),
-                 o_cand = take(4 * (size_t)sim->N), o_cbits = take(4 * (size_t)((sim->N + 31) / 32));
-    if (cudaMalloc(&sim->bt_mem, o) != cudaSuccess) { cudaGetLastError(); sim->bt_mem = nullptr; return FS_OK; }
-    unsigned char* b = (unsigned char*)sim->bt_mem;
+    const BatchLayout bl = batch_layout(sim->N, sim->K, sim->Kp);
+    const int Pdef = bl.Pdef, P = bl.P;
+    const size_t o_ctl = bl.ctl, o_owner = bl.owner, o_seeds = bl.seeds, o_edges = bl.edges, o_ecount = bl.ecount,
+                 o_npos = bl.npos, o_elems = bl.elems, o_undo = bl.undo, o_blocks = bl.blocks, o_clist = bl.clist,
+                 o_cand = bl.cand, o_cbits = bl.cbits;
+    unsigned char* b = (unsigned char*)sim->bt_mem;      // the workspace's batch region (fs_create laid it out)
     int lb_shift = 0; while ((1 << lb_shift) < sim->LB) ++lb_shift;
     BatchArgs& a = sim->bt;
     a.N = sim->N; a.Kp = sim->Kp; a.LBshift = lb_shift; a.nblk = sim->nblk; a.ast = sim->ast; a.log_cap = sim->log_cap;
@@ -1851,7 +1867,7 @@ int setup_batch(fs_sim* sim) {
     a.clist = (BatchCommit*)(b + o_clist); a.cand = (int*)(b + o_cand); a.cbits = (unsigned*)(b + o_cbits);
     if (cudaMemsetAsync(a.ctl, 0, sizeof(BatchCtl), sim->stream) != cudaSuccess ||
         cudaMemsetAsync(a.owner, 0xff, 4 * (size_t)sim->N, sim->stream) != cudaSuccess) {
-        cudaGetLastError(); cudaFree(sim->bt_mem); sim->bt_mem = nullptr; return FS_OK;
+        cudaGetLastError(); return FS_OK;
     }
     sim->bt_P = Pdef; sim->bt_alloc = P; sim->bt_seq = 64; sim->bt_grid = sim->sm_count; sim->bt_ok = true;
     return FS_OK;
@@ -1888,7 +1904,7 @@ int fs_workspace_bytes(int64_t N, int32_t R, const double* pos_dev, const fs_par
     if (K > MAX_K) return fail(FS_ERR_ARG, "max degree %d exceeds %d", K, MAX_K);
     int LB, nblk;
     if (choose_leaf(N, &LB, &nblk)) return fail(FS_ERR_ARG, "N too large for the relax hierarchy");
-    layout_rest(L, N, R, pad_k(K), nblk, 4 * N + 1024);
+    layout_rest(L, N, R, K, pad_k(K), nblk, 4 * N + 1024);
     *bytes_out = L.total;
     return FS_OK;
 }
@@ -1920,7 +1936,7 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     if (choose_leaf(N, &LB, &nblk)) return fail(FS_ERR_ARG, "N too large for the relax hierarchy");
     int Kp = pad_k(K);
     int64_t log_cap = 4 * N + 1024;
-    layout_rest(L, N, R, Kp, nblk, log_cap);
+    layout_rest(L, N, R, K, Kp, nblk, log_cap);
     if (workspace_bytes < L.total) return fail(FS_ERR_WORKSPACE, "workspace too small (%zu < %zu)", workspace_bytes, L.total);
 
     fs_sim* sim = new (std::nothrow) fs_sim();
@@ -1941,6 +1957,8 @@ int fs_create_ensemble(fs_sim** out, int64_t N, int32_t R, const double* pos_dev
     sim->bval = (double*)(base + L.bval); sim->bidx = (int*)(base + L.bidx); sim->flog = (int*)(base + L.flog);
     sim->scnt = (unsigned*)(base + L.scnt);
     sim->ctr = (Counters*)(base + L.ctr); sim->hext = (double2*)(base + L.hext);
+    sim->hloc_buf = (double2*)(base + L.hloc);
+    sim->bt_mem = batch_applies(N, R, K) ? (void*)(base + L.batch) : nullptr;
 
 #define CREATE_TRY(expr)                                                                           \
     do {                                                                                           \
@@ -2015,10 +2033,8 @@ int fs_destroy(fs_sim* sim) {
     cudaStreamSynchronize(sim->stream);                  // kernels in flight may still read the pinned staging buffers
     if (sim->hext_host) cudaFreeHost(sim->hext_host);
     if (sim->ctr_host) cudaFreeHost(sim->ctr_host);
-    if (sim->hloc) cudaFree(sim->hloc);
     if (sim->lat_mem) cudaFree(sim->lat_mem);
     if (sim->st_mem) cudaFree(sim->st_mem);
-    if (sim->bt_mem) cudaFree(sim->bt_mem);
     delete sim;
     return FS_OK;
 }
@@ -2078,11 +2094,8 @@ int fs_set_field_ensemble(fs_sim* sim, const double* h_host, uint32_t step) {
 int fs_set_local_field(fs_sim* sim, const double* h_dev) {
     if (!sim) return fail(FS_ERR_ARG, "sim is NULL");
     DeviceGuard guard_(sim->device);
-    if (!h_dev) {
-        if (sim->hloc) { CUDA_TRY(cudaStreamSynchronize(sim->stream)); cudaFree(sim->hloc); sim->hloc = nullptr; }
-        return FS_OK;
-    }
-    if (!sim->hloc) CUDA_TRY(cudaMalloc(&sim->hloc, 16 * (size_t)sim->N));
+    if (!h_dev) { sim->hloc = nullptr; return FS_OK; }   // kernels already enqueued keep reading the workspace copy
+    sim->hloc = sim->hloc_buf;
     CUDA_TRY(cudaMemcpyAsync(sim->hloc, h_dev, 16 * (size_t)sim->N, cudaMemcpyDeviceToDevice, sim->stream));
     return FS_OK;
 }
@@ -2166,28 +2179,6 @@ int fs_measure_fp32_peak(double* ffma_per_s, void* stream) {
     *ffma_per_s = best;
     return FS_OK;
 }
-
-#ifdef FS_DEBUG_API
-// experiments only (never built into the shipped library): override the stencil kernel's CTA shape
-int fs_debug_stencil_shape(fs_sim* sim, int nw, int rs) {
-    if (!sim || !sim->stencil_ok) return -1;
-    LatGrid& g = sim->lg;
-    sim->st_nw = nw; sim->st_rs = rs;
-    sim->st_smem = stencil_smem(g, nw, rs, ST_OV, &sim->st_pv);
-    int TV = ST_OV * nw;
-    int Upa = ((g.U + ST_TU - 1) / ST_TU * ST_TU + 2 * g.Ru + 3) & ~3, Vpa = (g.V + TV - 1) / TV * TV + 2 * g.Rv;
-    if (Vpa > g.Vpa || Upa > g.Upa) return -2;          // spin grid allocation too small for this tile
-    return FS_OK;
-}
-#endif
-
-#ifdef FS_DEBUG_API
-int fs_debug_batch_knobs(fs_sim* sim, int max_chain, int min_commit) {
-    if (!sim) return -1;
-    sim->bt_max_chain = std::max(1, std::min(max_chain, (int)BT_LMAX)); sim->bt_min_commit = min_commit;
-    return FS_OK;
-}
-#endif
 
 #ifdef FS_BATCH_PROFILE
 int fs_debug_batch_profile(fs_sim* sim, long long* out12) {

@@ -1352,3 +1352,41 @@ def test_off_lattice_ensemble(B):
         assert np.array_equal(s[r], o.spins())
         assert field_err(h[r], o.fields(0)) < FIELD_TOL
         assert o.monitor()[0] == 0
+
+
+# ------------------------------------------------------------------ boundary: device memory comes from the caller
+def test_device_memory_is_the_callers_workspace(B):
+    """the workspace is caller-allocated.  Driver free memory + torch's reserved pool stays constant unless
+    somebody other than torch allocates, so its drop across fs_create is exactly what the library allocated itself:
+    nothing for a geometry that is not a lattice, the stencil table set (bounded by 8N + 2^20 cells per grid) for a
+    lattice -- and nothing more during set_local_field, batched relaxation, sweeps or reads."""
+    import torch
+
+    def outside_torch():
+        torch.cuda.synchronize()
+        return torch.cuda.mem_get_info()[0] + torch.cuda.memory_reserved()
+
+    for make, lattice in ((lambda: W.off_lattice("point_cloud", 20000, seed=6), False), (lambda: W.config("4", scale=110), True)):
+        w = make()
+        for attempt in range(2):                            # the first pass loads the kernels (module memory), the second is measured
+            base = outside_torch()
+            sim = B.Sim(w.pos, w.angle, w.hc, w.params)
+            owned = base - outside_torch()
+            assert sim.lattice()["active"] == lattice and sim.batch_stats()["max_seeds"] > 0
+            sim.set_spins(w.spins); sim.set_thermal(w.sigma_th, w.thermal_seed)
+            rng = np.random.default_rng(0)
+            sim.set_local_field(1e-3 * rng.standard_normal((w.N, 2)))
+            before = outside_torch()
+            for t in (0, len(w.fields) // 2, len(w.fields) - 1):
+                sim.set_field(*w.fields[t], t); sim.relax()
+            sim.set_local_field(None); sim.set_local_field(np.zeros((w.N, 2)))
+            sim.sweep(w.fields[:2], step0=0)
+            sim.update_fields(); sim.get_fields(0); sim.scan()
+            assert sim.batch_stats()["flips"] > 0
+            if attempt == 1:
+                assert outside_torch() == before, "the library allocated device memory after fs_create"
+                if lattice:
+                    assert 0 < owned <= 3 * 4 * (8 * w.N + (1 << 20)) + 4 * w.N + (4 << 20), owned
+                else:
+                    assert owned == 0, owned
+            sim.close(); del sim
